@@ -1,0 +1,141 @@
+/* psf.h -- C ABI of libpsf_b200: Fourier-parametrised vectorial Richards-Wolf propagation of a z-stack
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations are PAPER.md = arXiv 2502.03170, line : equation):
+ *   for every plane b of a stack (or every emitter of a batch) and every pixel (x, y) of an M x M grid,
+ *
+ *     E_c(x,y;b) = -(i f k / 2 pi) * sum over the pupil disc s_x^2+s_y^2 <= s_max^2 of
+ *                    a(s) exp{i W(s)} e_inf,c(s) / s_z * exp{i k s_z z_b} exp{i k (s_x x + s_y y)} ds_x ds_y
+ *                                                 (Eq. 9 with the corrections of :146 Eq. 15)
+ *     I(x,y;b)   = |E_x|^2 + |E_y|^2 + |E_z|^2
+ *
+ *   with  k = 2 pi n_i / lambda, s_max = NA / n_i, f = 1;
+ *         e_inf = polarisation-rotation matrix applied to the input Jones vector (Eq. 6);
+ *         a(s)  = sqrt(cos theta) apodisation (Eq. 19) when PSF_FLAG_APODIZE;
+ *         W(s)  = Gibson-Lanni phase (Eq. 16 with t_i from :167 Eq. 17) when
+ *                 PSF_FLAG_GIBSON_LANNI, plus sum_j c_j Z_j(s) in Noll-indexed Zernike polynomials
+ *                 (Eq. 18), plus an optional per-plane tilt -k (s_x x_b + s_y y_b);
+ *   discretised on the N x N midpoint pupil grid u_p = (2p+1-N)/N, s = s_max u, weight (s_max 2/N)^2,
+ *   output coordinates x_m = (m - (M-1)/2) * pixel.  The readings taken where the paper is silent are
+ *   listed in DESIGN.md.  The zoomed DFT is evaluated as two real-matrix product stages (rows, then
+ *   columns) on the GPU; the per-plane pupil is generated inside the first product and never stored.
+ *
+ * Conventions
+ *   - all lengths in micrometres; all `const T *` arguments marked "host" are read before the call returns;
+ *   - device pointers are CUDA device memory of the plan's device, 16-byte aligned, owned by the caller;
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - every call returns a psf_status; nothing throws or aborts across the ABI; on error outputs are
+ *     unspecified and *out is NULL; the message is available from psf_last_error();
+ *   - psf_plan_create / psf_set_* may allocate device memory and synchronise; psf_compute only enqueues
+ *     kernels on `cuda_stream`: it never allocates, never synchronises and never touches host memory;
+ *   - a plan is not thread-safe; distinct plans are independent;
+ *   - there is no CPU fallback: without a CUDA device of compute capability 10.x, psf_plan_create fails.
+ */
+#ifndef PSF_B200_H
+#define PSF_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psf_plan psf_plan; /* opaque, owned by the library */
+
+typedef enum {
+  PSF_OK = 0,
+  PSF_ERR_INVALID_ARG = 1, /* NA<=0, NA>=n_immersion, lambda<=0, N<2, M<1, pixel<=0, n_planes<1, non-finite z,
+                              noll_first<1, null pointers, misaligned outputs                                 */
+  PSF_ERR_UNSUPPORTED = 2, /* field output with PSF_POL_UNPOLARIZED, PSF_FLAG_FRESNEL, device without sm_100   */
+  PSF_ERR_ALLOC = 3,       /* host or device allocation failed                                                 */
+  PSF_ERR_CUDA = 4,        /* any CUDA runtime failure (message via psf_last_error)                            */
+  PSF_ERR_STATE = 5        /* call order violated (e.g. shifts given for another n_planes)                     */
+} psf_status;
+
+typedef enum {
+  PSF_POL_X = 0,          /* (1, 0)                                                                             */
+  PSF_POL_Y = 1,          /* (0, 1)                                                                             */
+  PSF_POL_CIRC_L = 2,     /* (1, +i)/sqrt(2)                                                                    */
+  PSF_POL_CIRC_R = 3,     /* (1, -i)/sqrt(2)                                                                    */
+  PSF_POL_JONES = 4,      /* custom complex (px, py) from psf_plan_desc.jones, used as given                    */
+  PSF_POL_UNPOLARIZED = 5 /* 1/2 (I_x + I_y): x and y inputs summed incoherently, unit input power              */
+} psf_pol;
+
+enum {
+  PSF_FLAG_APODIZE = 1,      /* a(s) = sqrt(cos theta), Eq. 19                                     */
+  PSF_FLAG_GIBSON_LANNI = 2, /* W(s) of PAPER.md:154 Eq. 16                                                     */
+  PSF_FLAG_FRESNEL = 4       /* q_s, q_p of PAPER.md:102-107 Eq. 7-8: not built yet -> PSF_ERR_UNSUPPORTED      */
+};
+
+typedef enum {
+  PSF_PREC_AUTO = 0,   /* the library picks per problem size                                                    */
+  PSF_PREC_3XTF32 = 1, /* tcgen05 tensor cores, both operands split hi/lo in TF32 (fp32-level accuracy)         */
+  PSF_PREC_FP32 = 2    /* plain fp32 FFMA tiles                                                                 */
+} psf_precision;
+
+typedef struct {
+  double NA, wavelength_um, n_immersion, n_sample;
+  /* Gibson-Lanni, PAPER.md:154-167 (read iff PSF_FLAG_GIBSON_LANNI) */
+  double particle_depth_um;                         /* t_s                                                      */
+  double n_glass, t_glass_um;                       /* n_g, t_g                                                 */
+  double n_glass_design, t_glass_design_um;         /* n_g*, t_g*                                               */
+  double n_immersion_design, t_immersion_design_um; /* n_i*, t_i*                                               */
+  double t_immersion_um;                            /* t_i; NaN -> derived from Eq. 17 as printed               */
+  int pupil_n;                                      /* N: the pupil grid is N x N                               */
+  int out_m;                                        /* M: the image grid is M x M                               */
+  double pixel_um;                                  /* output pixel size                                        */
+  int n_planes;                                     /* Z: number of planes (or emitters)                        */
+  const double *z_um;                               /* host, length n_planes, copied                            */
+  psf_pol pol;
+  double jones[4];                                  /* re px, im px, re py, im py (PSF_POL_JONES only)          */
+  unsigned flags;                                   /* PSF_FLAG_*                                               */
+  psf_precision precision;
+  int device;                                       /* CUDA device ordinal                                      */
+} psf_plan_desc;
+
+/* Build a plan: validates `desc`, evaluates every z-independent factor of the integrand in fp64 on the host
+ * (disc mask in integers, rotation matrix x Jones vector, apodisation / s_z, Gibson-Lanni phase incl. the
+ * evanescent branch, wavenumber tables, zoomed-DFT matrices), rounds to fp32 and uploads.  *out owns all
+ * device memory of the plan (tables + scratch) until psf_plan_destroy. */
+psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out);
+
+/* Zernike phase W = sum_{i<n_coeffs} coeffs[i] * Z_{noll_first+i}, radians, Noll-normalised (Eq. 18).
+ * per_plane == 0: coeffs[n_coeffs] shared by all planes (folded into the static pupil);
+ * per_plane == 1: coeffs[n_planes][n_coeffs], row b for plane b (evaluated in the pupil producer).
+ * coeffs == NULL or n_coeffs == 0 clears the Zernike term.  coeffs is host memory, copied. */
+psf_status psf_set_zernike(psf_plan *plan, const float *coeffs, int noll_first, int n_coeffs, int per_plane);
+
+/* Per-plane lateral emitter position (x_b, y_b): plane b becomes I(x - x_b, y - y_b; z_b), applied as the pupil
+ * tilt phase -k (s_x x_b + s_y y_b).  xy_um is host [n_planes][2]; NULL clears. */
+psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
+
+/* Enqueue the whole stack on `cuda_stream`:
+ *   intensity : device fp32 [n_planes][M][M], x fastest (required);
+ *   field     : device complex64 (interleaved re, im) [3][n_planes][M][M] = (E_x, E_y, E_z), or NULL.
+ * Asynchronous; results are valid once the stream has passed this point. */
+psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void *field);
+
+psf_status psf_plan_destroy(psf_plan *plan);
+
+/* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /
+ * psf_host_tables.  Never NULL; valid until the next call on the same plan / thread. */
+const char *psf_last_error(const psf_plan *plan);
+
+/* Number of kernel launches one psf_compute call of this plan enqueues (for benchmarking records). */
+int psf_launches_per_compute(const psf_plan *plan);
+
+/* Name of the kernel path the plan selected: "ffma", "tc3xtf32", ... (static string). */
+const char *psf_path_name(const psf_plan *plan);
+
+/* Host-only diagnostic (no device needed): the plan-time static pupil in fp64, before folding and rounding.
+ *   n_components : out, 3 (coherent input) or 5 (unpolarised: the distinct scalar pupils a, b, d, c_x, c_y);
+ *   weights      : out [5], intensity weight of each component;
+ *   base         : out [n_components][N][N][2] (re, im) = prefactor * a / s_z * e_inf,c * exp(i W_static), 0 outside
+ *                  the disc; W_static includes the shared Zernike term given here (coeffs may be NULL);
+ *   kappa        : out [N][N], k cos(theta) in rad/um;     mask : out [N][N], 1 inside the disc.
+ * Any output pointer may be NULL.  base must hold 5*N*N*2 doubles. */
+psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int noll_first, int n_coeffs,
+                           int *n_components, double *weights, double *base, double *kappa, unsigned char *mask);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSF_B200_H */

@@ -1,0 +1,8 @@
+"""paper_2502_03170_b200: B200-native (sm_100a) Fourier-parametrised vectorial Richards-Wolf PSF stacks.
+
+The product is the C-ABI library `libpsf_b200.so` (include/psf.h); this package is its thin Python binding."""
+from ._binding import (PsfError, PsfPlan, plan_from_case, host_tables, load_library, lib_path, make_desc,
+                       psf_plan_desc, EXPORTS)
+
+__all__ = ["PsfError", "PsfPlan", "plan_from_case", "host_tables", "load_library", "lib_path", "make_desc",
+           "psf_plan_desc", "EXPORTS"]

@@ -1,0 +1,295 @@
+// C-ABI implementation (include/psf.h): validation, plan-time table upload, launch sequencing.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "plan.hpp"
+
+using namespace psf;
+
+namespace {
+
+thread_local std::string g_create_err = "";
+
+const size_t kScratchBudget = (size_t)48 << 20;   // T scratch ring: small enough to live in the 126 MB L2
+
+#define CU_TRY(p, call)                                                                         \
+  do {                                                                                          \
+    cudaError_t e_ = (call);                                                                    \
+    if (e_ != cudaSuccess) {                                                                    \
+      (p)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                            \
+      return PSF_ERR_CUDA;                                                                      \
+    }                                                                                           \
+  } while (0)
+
+template <typename T>
+psf_status upload(psf_plan *p, void **dptr, const std::vector<T> &h) {
+  if (*dptr) { cudaFree(*dptr); *dptr = nullptr; }
+  if (h.empty()) return PSF_OK;
+  cudaError_t e = cudaMalloc(dptr, h.size() * sizeof(T));
+  if (e != cudaSuccess) { p->err = std::string("cudaMalloc: ") + cudaGetErrorString(e); *dptr = nullptr; return PSF_ERR_ALLOC; }
+  CU_TRY(p, cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return PSF_OK;
+}
+
+// (hi, lo) float pair of a double
+inline void split2(double v, float &hi, float &lo) { hi = (float)v; lo = (float)(v - (double)hi); }
+
+// Folds the static pupil about both axes into the four parity classes and uploads every static table.
+psf_status upload_static(psf_plan *p) {
+  const psf_plan_desc &d = p->desc;
+  HostPupil hp;
+  const bool shared_z = !p->zern_shared.empty();
+  build_host_pupil(d, shared_z ? p->zern_shared.data() : nullptr, p->noll_first, (int)p->zern_shared.size(), hp);
+  const int N = d.pupil_n, n = (N + 1) / 2, C = hp.C;
+  const size_t NN = (size_t)N * N, nn = (size_t)n * n;
+  DevPlan &P = p->dp;
+  P.C = C;
+  for (int c = 0; c < 5; ++c) P.weight[c] = (float)hp.weight[c];
+
+  std::vector<float4> bfold((size_t)C * nn * 2);
+  std::vector<float2> kt(nn);
+  const double twopi = 6.283185307179586476925287;
+  for (int qy = 0; qy < n; ++qy) {
+    for (int qx = 0; qx < n; ++qx) {
+      const int ry = N - 1 - qy, rx = N - 1 - qx;
+      const bool sy = ry == qy, sx = rx == qx;
+      float hi, lo;
+      split2(hp.kappa[(size_t)qy * N + qx] / twopi, hi, lo);
+      kt[(size_t)qy * n + qx] = make_float2(hi, lo);
+      for (int c = 0; c < C; ++c) {
+        const cplx *B = hp.base.data() + (size_t)c * NN;
+        const cplx p00 = B[(size_t)qy * N + qx];
+        const cplx p01 = sx ? cplx(0, 0) : B[(size_t)qy * N + rx];
+        const cplx p10 = sy ? cplx(0, 0) : B[(size_t)ry * N + qx];
+        const cplx p11 = (sx || sy) ? cplx(0, 0) : B[(size_t)ry * N + rx];
+        const cplx e0 = p00 + p01, o0 = sx ? cplx(0, 0) : p00 - p01;     // row qy:      even / odd in x
+        const cplx e1 = p10 + p11, o1 = sx ? cplx(0, 0) : p10 - p11;     // mirror row
+        const cplx ee = e0 + e1, eo = o0 + o1;
+        const cplx oe = sy ? cplx(0, 0) : e0 - e1, oo = sy ? cplx(0, 0) : o0 - o1;
+        float4 *o = &bfold[((size_t)c * nn + (size_t)qy * n + qx) * 2];
+        o[0] = make_float4((float)ee.real(), (float)ee.imag(), (float)eo.real(), (float)eo.imag());
+        o[1] = make_float4((float)oe.real(), (float)oe.imag(), (float)oo.real(), (float)oo.imag());
+      }
+    }
+  }
+  psf_status s;
+  if ((s = upload(p, &p->d_bfold, bfold)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_kt, kt)) != PSF_OK) return s;
+  P.bfold = (const float4 *)p->d_bfold;
+  P.kt = (const float2 *)p->d_kt;
+
+  if (P.per_plane) {
+    std::vector<float2> bunf((size_t)C * NN);
+    for (size_t i = 0; i < bunf.size(); ++i) bunf[i] = make_float2((float)hp.base[i].real(), (float)hp.base[i].imag());
+    if ((s = upload(p, &p->d_bunf, bunf)) != PSF_OK) return s;
+    P.bunf = (const float2 *)p->d_bunf;
+    const int K = p->K_rows;
+    std::vector<float> zb((size_t)K * NN, 0.f);
+    for (int j = 0; j < K; ++j)
+      for (size_t i = 0; i < NN; ++i)
+        if (hp.mask[i]) zb[(size_t)j * NN + i] = (float)(zernike_noll(p->noll_first + j, hp.rho[i], hp.cosphi[i], hp.sinphi[i]) / twopi);
+    if ((s = upload(p, &p->d_zb, zb)) != PSF_OK) return s;
+    if ((s = upload(p, &p->d_coef, p->zern_rows)) != PSF_OK) return s;
+    P.zb = (const float *)p->d_zb;
+    P.coef = (const float *)p->d_coef;
+    P.K = K;
+  } else {
+    P.K = 0;
+  }
+  // plane table
+  std::vector<float4> planes(d.n_planes);
+  const double tscale = d.NA / d.wavelength_um;   // k s_max / 2 pi
+  P.has_shift = p->shifts.empty() ? 0 : 1;
+  for (int b = 0; b < d.n_planes; ++b) {
+    float zh, zl;
+    split2(p->z[b], zh, zl);
+    float tx = 0.f, ty = 0.f;
+    if (P.has_shift) { tx = (float)(tscale * (double)p->shifts[2 * b]); ty = (float)(tscale * (double)p->shifts[2 * b + 1]); }
+    planes[b] = make_float4(zh, zl, tx, ty);
+  }
+  if ((s = upload(p, &p->d_planes, planes)) != PSF_OK) return s;
+  P.planes = (const float4 *)p->d_planes;
+  return PSF_OK;
+}
+
+psf_status upload_dft(psf_plan *p) {
+  std::vector<double> phi;
+  build_dft_phase(p->desc, phi);
+  std::vector<float> c(phi.size()), s(phi.size());
+  for (size_t i = 0; i < phi.size(); ++i) { c[i] = (float)std::cos(phi[i]); s[i] = (float)std::sin(phi[i]); }
+  psf_status st;
+  if ((st = upload(p, &p->d_cos, c)) != PSF_OK) return st;
+  if ((st = upload(p, &p->d_sin, s)) != PSF_OK) return st;
+  p->dp.cosT = (const float *)p->d_cos;
+  p->dp.sinT = (const float *)p->d_sin;
+  return PSF_OK;
+}
+
+psf_status alloc_scratch(psf_plan *p) {
+  const DevPlan &P = p->dp;
+  const size_t per_plane = (size_t)P.C * 8 * P.n * P.m * sizeof(float);
+  size_t zc = kScratchBudget / per_plane;
+  if (zc < 1) zc = 1;
+  if (zc > (size_t)P.Z) zc = P.Z;
+  if (zc > 65535 / (size_t)P.C) zc = 65535 / P.C;       // gridDim.z limit of the stage-1 launch
+  p->zchunk = (int)zc;
+  const size_t need = zc * per_plane;
+  if (need > p->T_bytes) {
+    if (p->d_T) { cudaFree(p->d_T); p->d_T = nullptr; p->T_bytes = 0; }
+    cudaError_t e = cudaMalloc(&p->d_T, need);
+    if (e != cudaSuccess) { p->err = std::string("cudaMalloc(T scratch): ") + cudaGetErrorString(e); return PSF_ERR_ALLOC; }
+    p->T_bytes = need;
+  }
+  return PSF_OK;
+}
+
+psf_status refresh(psf_plan *p) {
+  psf_status s = upload_static(p);
+  if (s != PSF_OK) return s;
+  return alloc_scratch(p);     // C is fixed per plan, but keep the scratch consistent with it
+}
+
+void free_all(psf_plan *p) {
+  void **bufs[] = {&p->d_bfold, &p->d_kt, &p->d_bunf, &p->d_zb, &p->d_coef, &p->d_planes, &p->d_cos, &p->d_sin, &p->d_T};
+  for (void **b : bufs)
+    if (*b) { cudaFree(*b); *b = nullptr; }
+}
+
+}  // namespace
+
+extern "C" {
+
+psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
+  if (out) *out = nullptr;
+  if (!out) { g_create_err = "out is NULL"; return PSF_ERR_INVALID_ARG; }
+  std::string err;
+  psf_status s = validate_desc(desc, err);
+  if (s != PSF_OK) { g_create_err = err; return s; }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    g_create_err = std::string("no CUDA device: ") + cudaGetErrorString(e) + " (libpsf_b200 has no CPU fallback)";
+    return PSF_ERR_CUDA;
+  }
+  if (desc->device < 0 || desc->device >= ndev) { g_create_err = "device ordinal out of range"; return PSF_ERR_INVALID_ARG; }
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, desc->device)) != cudaSuccess) {
+    g_create_err = std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e);
+    return PSF_ERR_CUDA;
+  }
+  if (prop.major != 10) {
+    g_create_err = "device is not sm_100 (compute capability 10.x): this library is built for B200 only";
+    return PSF_ERR_UNSUPPORTED;
+  }
+  psf_plan *p = new (std::nothrow) psf_plan();
+  if (!p) { g_create_err = "out of host memory"; return PSF_ERR_ALLOC; }
+  p->desc = *desc;
+  p->z.assign(desc->z_um, desc->z_um + desc->n_planes);
+  p->desc.z_um = p->z.data();
+  if (std::isnan(p->desc.n_immersion_design)) p->desc.n_immersion_design = desc->n_immersion;
+  p->device = desc->device;
+  p->sm_count = prop.multiProcessorCount;
+  DevPlan &P = p->dp;
+  P.N = desc->pupil_n; P.M = desc->out_m; P.n = (P.N + 1) / 2; P.m = (P.M + 1) / 2; P.Z = desc->n_planes;
+  P.per_plane = 0; P.K = 0; P.has_shift = 0;
+  if ((e = cudaSetDevice(p->device)) != cudaSuccess) {
+    g_create_err = std::string("cudaSetDevice: ") + cudaGetErrorString(e);
+    delete p;
+    return PSF_ERR_CUDA;
+  }
+  p->path = 0;
+  if ((s = upload_dft(p)) != PSF_OK || (s = refresh(p)) != PSF_OK) {
+    g_create_err = p->err;
+    free_all(p);
+    delete p;
+    return s;
+  }
+  *out = p;
+  return PSF_OK;
+}
+
+psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int n_coeffs, int per_plane) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (n_coeffs < 0) { p->err = "n_coeffs < 0"; return PSF_ERR_INVALID_ARG; }
+  if (n_coeffs > 0 && coeffs && noll_first < 1) { p->err = "noll_first must be >= 1"; return PSF_ERR_INVALID_ARG; }
+  if (n_coeffs > 64) { p->err = "at most 64 Zernike terms"; return PSF_ERR_INVALID_ARG; }
+  const size_t cnt = (size_t)n_coeffs * (per_plane ? p->dp.Z : 1);
+  if (coeffs)
+    for (size_t i = 0; i < cnt; ++i)
+      if (!std::isfinite(coeffs[i])) { p->err = "non-finite Zernike coefficient"; return PSF_ERR_INVALID_ARG; }
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  p->zern_shared.clear();
+  p->zern_rows.clear();
+  p->K_rows = 0;
+  if (coeffs && n_coeffs > 0) {
+    p->noll_first = noll_first;
+    if (per_plane) { p->zern_rows.assign(coeffs, coeffs + cnt); p->K_rows = n_coeffs; }
+    else p->zern_shared.assign(coeffs, coeffs + n_coeffs);
+  }
+  p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;
+  return refresh(p);
+}
+
+psf_status psf_set_shifts(psf_plan *p, const float *xy_um) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (xy_um)
+    for (int i = 0; i < 2 * p->dp.Z; ++i)
+      if (!std::isfinite(xy_um[i])) { p->err = "non-finite shift"; return PSF_ERR_INVALID_ARG; }
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  p->shifts.clear();
+  if (xy_um) p->shifts.assign(xy_um, xy_um + 2 * (size_t)p->dp.Z);
+  p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;
+  return refresh(p);
+}
+
+psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *field) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (!intensity) { p->err = "intensity is NULL"; return PSF_ERR_INVALID_ARG; }
+  if (((uintptr_t)intensity & 15) || ((uintptr_t)field & 15)) { p->err = "output pointers must be 16-byte aligned"; return PSF_ERR_INVALID_ARG; }
+  if (field && p->desc.pol == PSF_POL_UNPOLARIZED) {
+    p->err = "field output is undefined for PSF_POL_UNPOLARIZED (two incoherent fields)";
+    return PSF_ERR_UNSUPPORTED;
+  }
+  cudaError_t e = launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
+  if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  return PSF_OK;
+}
+
+psf_status psf_plan_destroy(psf_plan *p) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  cudaSetDevice(p->device);
+  free_all(p);
+  delete p;
+  return PSF_OK;
+}
+
+const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_create_err.c_str(); }
+
+int psf_launches_per_compute(const psf_plan *p) { return p ? ffma_launches(p) : 0; }
+
+const char *psf_path_name(const psf_plan *p) { return (p && p->path == 1) ? "tc3xtf32" : "ffma"; }
+
+psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int noll_first, int n_coeffs, int *n_components,
+                           double *weights, double *base, double *kappa, unsigned char *mask) {
+  std::string err;
+  psf_status s = validate_desc(desc, err);
+  if (s != PSF_OK) { g_create_err = err; return s; }
+  if (coeffs && n_coeffs > 0 && noll_first < 1) { g_create_err = "noll_first must be >= 1"; return PSF_ERR_INVALID_ARG; }
+  psf_plan_desc d = *desc;
+  if (std::isnan(d.n_immersion_design)) d.n_immersion_design = d.n_immersion;
+  HostPupil hp;
+  build_host_pupil(d, coeffs, noll_first, coeffs ? n_coeffs : 0, hp);
+  const size_t NN = (size_t)d.pupil_n * d.pupil_n;
+  if (n_components) *n_components = hp.C;
+  if (weights) for (int c = 0; c < 5; ++c) weights[c] = hp.weight[c];
+  if (base)
+    for (size_t i = 0; i < (size_t)hp.C * NN; ++i) { base[2 * i] = hp.base[i].real(); base[2 * i + 1] = hp.base[i].imag(); }
+  if (kappa) std::memcpy(kappa, hp.kappa.data(), NN * sizeof(double));
+  if (mask) std::memcpy(mask, hp.mask.data(), NN);
+  return PSF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,111 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/psf.h declares, validates
+descriptors, and its plan-time fp64 tables (host code, independent of the oracle) agree with the oracle's."""
+import ctypes as C
+import os
+import re
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import paper_2502_03170_b200 as psf
+import psf_workloads as W
+from oracle import psf_oracle as O
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = psf.load_library()
+    hdr = open(os.path.join(ROOT, "include", "psf.h")).read()
+    declared = set(re.findall(r"\b(psf_[a-z_]+)\s*\(", hdr))
+    assert declared == set(psf.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_descriptor_layout_matches_header_order():
+    hdr = open(os.path.join(ROOT, "include", "psf.h")).read()
+    body = hdr[hdr.index("typedef struct {"):hdr.index("} psf_plan_desc;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.replace("typedef struct {", "").strip()
+        if not decl:
+            continue
+        for part in decl.split(","):
+            tok = re.findall(r"[A-Za-z_][A-Za-z0-9_]*", part)
+            if tok:
+                names.append(tok[-1] if tok[-1] != "4" else tok[-2])
+    assert names == [f[0] for f in psf.psf_plan_desc._fields_]
+
+
+@pytest.mark.parametrize("field,value,status", [
+    ("NA", 0.0, 1), ("NA", 1.6, 1), ("wavelength_um", -1.0, 1), ("pupil_n", 1, 1), ("out_m", 0, 1),
+    ("pixel_um", 0.0, 1), ("n_sample", 0.0, 1),
+])
+def test_invalid_descriptors_are_rejected_before_any_device_work(field, value, status):
+    case = replace(W.config1(), **{field: value})
+    with pytest.raises(psf.PsfError) as e:
+        psf.PsfPlan(case)
+    assert e.value.status == status
+
+
+def test_non_finite_z_and_null_out_are_rejected():
+    case = replace(W.config1(), z_um=np.array([0.0, np.nan]))
+    with pytest.raises(psf.PsfError) as e:
+        psf.PsfPlan(case)
+    assert e.value.status == 1
+    lib = psf.load_library()
+    desc, keep = psf.make_desc(W.config1())
+    assert lib.psf_plan_create(C.byref(desc), None) == 1
+    assert b"NULL" in lib.psf_last_error(None)
+    desc.flags = 4   # PSF_FLAG_FRESNEL
+    h = C.c_void_p()
+    assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 2 and not h.value
+
+
+def _oracle_base(case, jones=None):
+    pup = O.Pupil(case, jones=jones)
+    N = case.pupil_n
+    out = np.zeros((len(pup.g), N, N), dtype=np.complex128)
+    W_static = pup.W_static.copy()
+    if case.zernike is not None and not case.per_plane_zernike:
+        W_static = W_static + np.asarray(case.zernike, dtype=np.float64) @ pup.zernike_basis()
+    for c, g in enumerate(pup.g):
+        out[c][pup.py, pup.px] = pup.prefactor * pup.amp * g * np.exp(1j * W_static)
+    kap = np.zeros((N, N))
+    kap[pup.py, pup.px] = pup.k * pup.costh
+    return out, kap, pup.mask
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_host_tables_match_oracle_pupil(cfg):
+    case = W.get_config(cfg)
+    if cfg == 3:
+        case = replace(case, pupil_n=96)
+    t = psf.host_tables(case, case.zernike, case.noll_first)
+    base, kap, mask = _oracle_base(case)
+    assert t["n_components"] == 3 and np.array_equal(t["mask"], mask)
+    assert np.abs(t["kappa"] - kap).max() < 1e-12 * kap.max()
+    assert np.abs(t["base"] - base).max() < 1e-11 * np.abs(base).max()
+
+
+def test_host_tables_unpolarised_five_pupils_reproduce_both_inputs():
+    case = replace(W.config5(), pupil_n=48)
+    t = psf.host_tables(case, case.zernike, case.noll_first)
+    assert t["n_components"] == 5 and np.allclose(t["weights"], [0.5, 1.0, 0.5, 0.5, 0.5])
+    bx, _, _ = _oracle_base(case, jones=(1.0 + 0j, 0j))
+    by, _, _ = _oracle_base(case, jones=(0j, 1.0 + 0j))
+    a, b, d, cx, cy = t["base"]
+    scale = np.abs(bx).max()
+    for got, want in ((a, bx[0]), (b, bx[1]), (cx, bx[2]), (b, by[0]), (d, by[1]), (cy, by[2])):
+        assert np.abs(got - want).max() < 1e-11 * scale
+
+
+def test_host_tables_odd_grid_and_jones():
+    case = W.small_random_case(21, pupil_n=13, out_m=7, per_plane=False, shifts=False)
+    t = psf.host_tables(case, case.zernike, case.noll_first)
+    base, kap, mask = _oracle_base(case)
+    assert np.array_equal(t["mask"], mask)
+    assert np.abs(t["base"] - base).max() < 1e-11 * np.abs(base).max()

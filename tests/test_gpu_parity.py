@@ -1,0 +1,191 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 oracle, element by element, on the same seeded
+inputs.  Bar (BASELINE.json north_star): for every plane, max|I_gpu - I_oracle| <= 2e-5 max(I_oracle)."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import psf_workloads as W
+from oracle import psf_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def psf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2502_03170_b200 as lib
+    return lib
+
+
+def gpu_stack(psf, case, precision="auto", want_field=False):
+    import torch
+    plan = psf.plan_from_case(case, precision=precision)
+    out = plan.compute(want_field=want_field)
+    torch.cuda.synchronize()
+    if want_field:
+        I, F = out
+        res = I.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.complex128)
+    else:
+        res = out.cpu().numpy().astype(np.float64)
+    path = plan.path
+    plan.destroy()
+    return res, path
+
+
+def plane_errors(I_gpu, I_ref):
+    peak = I_ref.reshape(I_ref.shape[0], -1).max(axis=1)
+    err = np.abs(I_gpu - I_ref).reshape(I_ref.shape[0], -1).max(axis=1)
+    return err / peak
+
+
+PRECISIONS = ["fp32", "auto"]
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config1_full_volume(psf, precision):
+    case = W.config1()
+    I, path = gpu_stack(psf, case, precision)
+    ref = O.stack_T2(case)
+    rel = plane_errors(I, ref)
+    assert rel.max() <= TOL, (path, rel.max())
+    # and against the literal T1 sum on one full plane
+    ref1 = O.intensity_T1(case, planes=[8])[0]
+    assert np.abs(I[8] - ref1).max() <= TOL * ref1.max()
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config2_full_volume(psf, precision):
+    case = W.config2()
+    I, path = gpu_stack(psf, case, precision)
+    ref = O.stack_T2(case)
+    rel = plane_errors(I, ref)
+    assert rel.max() <= TOL, (path, rel.max())
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config3_all_planes(psf, precision):
+    case = W.config3()
+    I, path = gpu_stack(psf, case, precision)
+    ref = O.stack_T2(case)
+    rel = plane_errors(I, ref)
+    assert rel.max() <= TOL, (path, rel.max(), int(rel.argmax()))
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config4_all_emitters(psf, precision):
+    case = W.config4()
+    I, path = gpu_stack(psf, case, precision)
+    assert I.shape == (4096, 32, 32)
+    idx = np.arange(0, 4096, 7)                     # 586 emitters in full through T2 ...
+    ref = O.stack_T2(case.with_planes(idx))
+    rel = plane_errors(I[idx], ref)
+    assert rel.max() <= TOL, (path, rel.max())
+    rng = np.random.default_rng(4)                 # ... and 4096 random voxels over all emitters through T1
+    b = rng.integers(0, 4096, 4096)
+    iy, ix = rng.integers(0, 32, 4096), rng.integers(0, 32, 4096)
+    v1 = O.voxel_intensity(case, b, iy, ix)
+    peaks = I.reshape(4096, -1).max(axis=1)[b]
+    assert (np.abs(I[b, iy, ix] - v1) / peaks).max() <= 1.5 * TOL
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config5_sampled_planes_and_voxels(psf, precision):
+    """Full BASELINE size in the launch configuration bench.py times; the oracle covers 6 full planes (T2) and
+    4096 seeded voxels over all 256 planes (T1)."""
+    case = W.config5()
+    I, path = gpu_stack(psf, case, precision)
+    planes = [0, 37, 101, 128, 200, 255]
+    ref = O.stack_T2(case, planes)
+    rel = plane_errors(I[planes], ref)
+    assert rel.max() <= TOL, (path, rel)
+    rng = np.random.default_rng(5)
+    b = rng.integers(0, 256, 4096)
+    iy, ix = rng.integers(0, 512, 4096), rng.integers(0, 512, 4096)
+    v1 = O.voxel_intensity(case, b, iy, ix)
+    peaks = I.reshape(256, -1).max(axis=1)[b]       # plane peaks of the GPU stack (within 2e-5 of the oracle's on the checked planes)
+    assert (np.abs(I[b, iy, ix] - v1) / peaks).max() <= 1.5 * TOL
+    # property valid at any size: unpolarised intensity is symmetric under (x,y) -> (-x,-y) only without Zernike;
+    # with it, check positivity and finiteness of every voxel instead
+    assert np.isfinite(I).all() and (I >= 0).all()
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+@pytest.mark.parametrize("seed,N,M,Z", [(31, 12, 9, 3), (32, 13, 8, 2), (33, 37, 33, 5), (34, 70, 45, 2), (35, 2, 1, 1),
+                                         (36, 130, 67, 3)])
+def test_small_cases_every_option_odd_even_ragged(psf, precision, seed, N, M, Z):
+    """Jones polarisation, Gibson-Lanni with design != actual, per-plane Zernike, shifts; odd/even N and M, sizes
+    that are not multiples of any tile."""
+    case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z)
+    I, path = gpu_stack(psf, case, precision)
+    ref = O.stack_T2(case)
+    rel = plane_errors(I, ref)
+    assert rel.max() <= TOL, (path, rel)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_shared_zernike_static_path_odd_sizes(psf, precision):
+    for seed, N, M in ((41, 33, 21), (42, 64, 40), (43, 9, 4)):
+        case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=4, per_plane=False, shifts=False,
+                                   pol=W.POL_CIRC_R)
+        I, path = gpu_stack(psf, case, precision)
+        ref = O.stack_T2(case)
+        assert plane_errors(I, ref).max() <= TOL, (path, seed)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_field_output_matches_oracle_field(psf, precision):
+    case = replace(W.config2(), z_um=np.linspace(-2.0, 2.0, 5), pupil_n=96, out_m=50)
+    (I, F), path = gpu_stack(psf, case, precision, want_field=True)
+    Eref = O.field_T2(case)
+    scale = np.abs(Eref).max()
+    assert np.abs(F - Eref).max() <= 2e-5 * scale
+    assert np.abs(np.sum(np.abs(F) ** 2, axis=0) - I).max() <= 1e-5 * I.max()
+
+
+def test_unpolarised_is_mean_of_x_and_y_and_field_is_refused(psf):
+    base = W.small_random_case(51, pupil_n=40, out_m=24, n_planes=3, per_plane=False, shifts=False)
+    Iu, _ = gpu_stack(psf, replace(base, pol=W.POL_UNPOLARIZED))
+    Ix, _ = gpu_stack(psf, replace(base, pol=W.POL_X))
+    Iy, _ = gpu_stack(psf, replace(base, pol=W.POL_Y))
+    assert np.abs(Iu - 0.5 * (Ix + Iy)).max() <= 1e-5 * Iu.max()
+    ref = O.stack_T2(replace(base, pol=W.POL_UNPOLARIZED))
+    assert plane_errors(Iu, ref).max() <= TOL
+    plan = psf.plan_from_case(replace(base, pol=W.POL_UNPOLARIZED))
+    with pytest.raises(psf.PsfError) as e:
+        plan.compute(want_field=True)
+    assert e.value.status == 2
+    plan.destroy()
+
+
+def test_exact_symmetries_hold_on_gpu(psf):
+    """x-pol, no aberration: mirror symmetry in x and y is exact in the folded formulation (bit-exact on the GPU)."""
+    case = replace(W.config1(), out_m=48)
+    I, _ = gpu_stack(psf, case)
+    assert np.array_equal(I, I[:, :, ::-1]) and np.array_equal(I, I[:, ::-1, :])
+
+
+def test_replan_zernike_and_shift_updates(psf):
+    """psf_set_zernike / psf_set_shifts after creation: shared -> per-plane -> cleared."""
+    import torch
+    base = W.small_random_case(61, pupil_n=30, out_m=16, n_planes=3, per_plane=False, shifts=False)
+    plan = psf.PsfPlan(base)
+    plan.set_zernike(base.zernike, base.noll_first)
+    a = plan.compute().cpu().numpy()
+    assert plane_errors(a, O.stack_T2(base)).max() <= TOL
+    per = W.small_random_case(62, pupil_n=30, out_m=16, n_planes=3)
+    per = replace(base, zernike=per.zernike, shifts_um=per.shifts_um)
+    plan.set_zernike(per.zernike, per.noll_first)
+    plan.set_shifts(per.shifts_um)
+    b = plan.compute().cpu().numpy()
+    assert plane_errors(b, O.stack_T2(per)).max() <= TOL
+    plan.set_zernike(None)
+    plan.set_shifts(None)
+    c = plan.compute().cpu().numpy()
+    torch.cuda.synchronize()
+    assert plane_errors(c, O.stack_T2(replace(base, zernike=None))).max() <= TOL
+    plan.destroy()
