@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- PSF voxels/s of the hot path (pupil producer -> row DFT -> column DFT -> |E|^2) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl ours|reference]
+
+One "step" is one psf_compute over the whole workload (all planes / emitters).  Prints ONE JSON line (rank 0).
+See DESIGN.md §7 for what every key means and how the roofline figures are derived.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import psf_workloads as W  # noqa: E402
+
+METRIC = "psf_voxels_per_s"
+UNIT = "voxels/s"
+WORKLOADS = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
+SM_COUNT, FMA_LANES_PER_SM = 148, 128
+TF32_OVER_BF16 = 1.1 / 2.25            # nominal dense ratio (B200_PROFILING.md table)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu captures
+# (profiles/*.md name the command); keyed by (path, workload).  None where no capture exists yet.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            d["_source"] = "measured"
+            return d
+        except Exception:
+            pass
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+def rank_case(cfg: int, rank: int):
+    """Weak scaling: every rank owns a full-size shard of a longer stack (rank r: z shifted by r * 10 nm; the
+    emitter batch of config 4 is redrawn with another z offset).  No data-path collective."""
+    case = W.get_config(cfg)
+    if rank:
+        from dataclasses import replace
+        case = replace(case, z_um=case.z_um + 0.010 * rank)
+    return case
+
+
+def folded_flops(case):
+    """Algorithmic real flop of the two DFT stages in the folded formulation:
+    stage 1 = C Z 8 chains 2 n^2 m, stage 2 = C Z 8 chains 2 m^2 n; n = ceil(N/2), m = ceil(M/2)."""
+    n, m = (case.pupil_n + 1) // 2, (case.out_m + 1) // 2
+    C = 5 if case.pol == "unpolarized" else 3
+    Z = case.n_planes
+    return C * Z * 16.0 * n * n * m, C * Z * 16.0 * m * m * n
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "20", "-i", str(index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v == "Active":
+                    reasons.add(nme)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_workload(torch, psf, case, device, steps, warmup, flush, profile=True):
+    """Device-timed steps: per step L2 flush (untimed), event, psf_compute, event.  Returns dict."""
+    plan = psf.plan_from_case(case, device=device)
+    dev = torch.device("cuda", device)
+    out = torch.empty((case.n_planes, case.out_m, case.out_m), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    if profile:
+        plan.profile_enable(True)
+    for _ in range(warmup):
+        plan.compute(out)
+    torch.cuda.synchronize(dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    stage_ms = np.zeros(4)
+    stage_launches = np.zeros(4, dtype=np.int64)
+    for i in range(steps):
+        flush.fill_(float(i))                     # > L2: evicts tables, scratch and outputs of the previous step
+        ev[i][0].record(stream)
+        plan.compute(out)
+        ev[i][1].record(stream)
+        if profile:
+            torch.cuda.synchronize(dev)
+            ms, ln = plan.profile_read()
+            stage_ms += np.array(ms)
+            stage_launches += np.array(ln)
+    torch.cuda.synchronize(dev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    res = {"plan": plan, "out": out, "step_ms": step_ms, "stage_ms": stage_ms / max(steps, 1),
+           "stage_launches": stage_launches // max(steps, 1), "path": plan.path,
+           "launches": plan.launches_per_compute}
+    return res
+
+
+def e2e_workload(torch, plan, case, device, steps, warmup):
+    """End to end through the public API with HOST buffers: per step, host Zernike coefficients / shifts go in through
+    psf_set_zernike / psf_set_shifts (host->device table refresh), psf_compute runs, and the intensity stack is copied
+    device->host into pinned memory.  Wall clock around the whole step."""
+    dev = torch.device("cuda", device)
+    out = torch.empty((case.n_planes, case.out_m, case.out_m), dtype=torch.float32, device=dev)
+    host = torch.empty(out.shape, dtype=torch.float32, pin_memory=True)
+    h2d = 0
+    times = []
+    for i in range(warmup + steps):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        plan.set_zernike(case.zernike, case.noll_first)
+        h2d = plan.last_upload_bytes
+        if case.shifts_um is not None:
+            plan.set_shifts(case.shifts_um)
+            h2d = plan.last_upload_bytes + (case.zernike.nbytes if case.zernike is not None else 0)
+        plan.compute(out)
+        host.copy_(out, non_blocking=True)
+        torch.cuda.synchronize(dev)
+        t1 = time.perf_counter()
+        if i >= warmup:
+            times.append(t1 - t0)
+    return {"s_per_step": statistics.mean(times), "h2d": int(h2d), "d2h": int(out.numel() * 4),
+            "checksum": float(host.double().sum())}
+
+
+def oracle_sample(case, budget_planes):
+    """A bounded, evenly spaced sample of planes for the CPU baseline."""
+    Z = case.n_planes
+    k = max(1, min(Z, budget_planes))
+    return np.unique(np.linspace(0, Z - 1, k).round().astype(int))
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads", 0) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return int(max(n))
+    except Exception:
+        pass
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+ORACLE_PLANES = {1: 16, 2: 32, 3: 24, 4: 1024, 5: 4}    # about 5-30 s of CPU work each on the 16-core B200 host
+
+
+def run_oracle_once(case, planes):
+    from oracle import psf_oracle as O
+    t0 = time.perf_counter()
+    I = O.stack_T2(case, planes)
+    dt = time.perf_counter() - t0
+    return dt, I
+
+
+def cpu_baseline(case, cfg):
+    planes = oracle_sample(case, ORACLE_PLANES[cfg])
+    dt, I = run_oracle_once(case, planes)
+    vox = len(planes) * case.out_m * case.out_m
+    return {"value": vox / dt, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+            "sample": f"oracle stack_T2 (fp64 separable direct sum, numpy) on {len(planes)} of {case.n_planes} "
+                      f"planes of {case.name}, {dt:.2f} s wall"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, timed on the host cores, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = WORKLOADS[args.workload]
+    case = W.get_config(cfg)
+    planes = oracle_sample(case, max(1, ORACLE_PLANES[cfg] // 2))
+    vox = len(planes) * case.out_m * case.out_m
+    for _ in range(args.warmup):
+        run_oracle_once(case, planes[:1])
+    times = []
+    for _ in range(args.steps):
+        dt, _ = run_oracle_once(case, planes)
+        times.append(dt)
+    mean = statistics.mean(times)
+    val = vox / mean
+    sample = (f"each step = oracle stack_T2 on {len(planes)} of {case.n_planes} planes of {case.name} "
+              f"({vox} voxels); value scales that to voxels/s")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": mean * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": case.name, "N": case.pupil_n, "M": case.out_m, "Z": case.n_planes,
+                       "sample_planes": int(len(planes))},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import paper_2502_03170_b200 as psf   # raises if the CUDA library is missing: no CPU fallback
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    peaks = load_peaks()
+    cfg = WORKLOADS[args.workload]
+    case = rank_case(cfg, rank)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # 256 MiB > 126 MB L2
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    res = time_workload(torch, psf, case, local, args.steps, args.warmup, flush)
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+
+    total_ms = torch.tensor([sum(res["step_ms"])], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(total_ms.item()) / args.steps
+    voxels = case.voxels() * world
+    value = voxels / (ms_per_step * 1e-3)
+
+    # end to end through the API with host buffers
+    e2e = e2e_workload(torch, res["plan"], case, local, max(3, min(args.steps, 10)), 2)
+    e2e_s = torch.tensor([e2e["s_per_step"]], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_val = voxels / float(e2e_s.item())
+
+    # roofline of the dominant kernel
+    f1, f2 = folded_flops(case)
+    stage_ms = res["stage_ms"]
+    dom = int(np.argmax(stage_ms[:2]))
+    flop_dom = (f1, f2)[dom]
+    launches_dom = max(int(res["stage_launches"][dom]), 1)
+    dur_ms = stage_ms[dom] / launches_dom
+    path = res["path"]
+    if path == "ffma":
+        bound = "alu"
+        peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+        executed = flop_dom
+        peak_note = f"148 SM x 128 FFMA lanes x 2 flop x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (fp32 FFMA pipe)"
+    else:
+        bound = "tensor"
+        long_step = ms_per_step > 1000.0
+        bf16 = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
+        peak = bf16 * TF32_OVER_BF16
+        executed = 3.0 * flop_dom
+        peak_note = (f"{peaks['_source']} bf16 {'sustained' if long_step else 'burst'} {bf16:.1f} TF/s x nominal tf32/bf16 "
+                     f"ratio {TF32_OVER_BF16:.3f}; achieved counts executed TF32 flop (3 products per fp32 product)")
+    achieved = executed / launches_dom / (dur_ms * 1e-3) / 1e12
+    traffic = NCU_TRAFFIC_BYTES.get((path, case.name))
+    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": traffic, "kernel": ("stage1_rowdft_producer", "stage2_coldft_intensity")[dom],
+                "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
+                "algorithmic_tflops": flop_dom / launches_dom / (dur_ms * 1e-3) / 1e12, "peak_source": peak_note,
+                "stage_ms_per_step": [float(stage_ms[0]), float(stage_ms[1])]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if path == "ffma" else "tf32x3", "data": "synthetic",
+            "config": {"workload": case.name, "N": case.pupil_n, "M": case.out_m, "Z": case.n_planes,
+                       "pol": case.pol, "path": path, "planes_per_s": case.n_planes * world / (ms_per_step * 1e-3),
+                       "l2": "256 MiB buffer written between timed iterations (flush)", "sharding": "z-shards, no collective"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]},
+            "gpu_launches": int(res["launches"]) * args.steps,
+            "roofline": roofline}
+    res["plan"].destroy()
+
+    if rank == 0 and world == 1:
+        line["cpu_baseline"] = cpu_baseline(case, cfg)
+        if not args.no_sweep:
+            sweep = {}
+            for name, c in WORKLOADS.items():
+                if c == cfg:
+                    sweep[name] = {"voxels_per_s": value, "ms_per_step": ms_per_step, "path": path}
+                    continue
+                cs = W.get_config(c)
+                r = time_workload(torch, psf, cs, local, min(args.steps, 10), 3, flush, profile=False)
+                ms = statistics.mean(r["step_ms"])
+                sweep[name] = {"voxels_per_s": cs.voxels() / (ms * 1e-3), "planes_per_s": cs.n_planes / (ms * 1e-3),
+                               "ms_per_step": ms, "path": r["path"], "launches": r["launches"]}
+                r["plan"].destroy()
+            line["workloads"] = sweep
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-sweep", action="store_true", help="skip the per-workload table of the other four configs")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

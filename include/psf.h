@@ -125,6 +125,20 @@ int psf_launches_per_compute(const psf_plan *plan);
 /* Name of the kernel path the plan selected: "ffma", "tc3xtf32", ... (static string). */
 const char *psf_path_name(const psf_plan *plan);
 
+/* Profiling aid for bench.py.  enable != 0: create CUDA events (this call may allocate) and make every later
+ * psf_compute bracket each of its kernel launches with cudaEventRecord on the compute stream; enable == 0: stop. */
+psf_status psf_profile_enable(psf_plan *plan, int enable);
+
+/* After the caller has synchronised the stream of the last psf_compute: device time per stage of that call.
+ *   stage_ms : host out [4], milliseconds summed over the launches of each stage
+ *              (0 = stage-1 row DFT with the fused pupil producer, 1 = stage-2 column DFT + intensity, 2, 3 = unused);
+ *   launches : host out [4], number of launches of each stage.
+ * PSF_ERR_STATE if profiling is not enabled or no psf_compute ran since. */
+psf_status psf_profile_read(psf_plan *plan, float *stage_ms, int *launches);
+
+/* Bytes copied host->device by the last psf_plan_create / psf_set_zernike / psf_set_shifts of this plan. */
+long long psf_last_upload_bytes(const psf_plan *plan);
+
 /* Host-only diagnostic (no device needed): the plan-time static pupil in fp64, before folding and rounding.
  *   n_components : out, 3 (coherent input) or 5 (unpolarised: the distinct scalar pupils a, b, d, c_x, c_y);
  *   weights      : out [5], intensity weight of each component;

@@ -18,7 +18,8 @@ FLAG_APODIZE, FLAG_GIBSON_LANNI, FLAG_FRESNEL = 1, 2, 4
 PREC = {"auto": 0, "3xtf32": 1, "fp32": 2}
 
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_compute", "psf_plan_destroy",
-           "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables"]
+           "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
+           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes"]
 
 
 class PsfError(RuntimeError):
@@ -72,6 +73,12 @@ def load_library(build_if_missing: bool = True):
     lib.psf_launches_per_compute.restype = C.c_int
     lib.psf_path_name.argtypes = [P]
     lib.psf_path_name.restype = C.c_char_p
+    lib.psf_profile_enable.argtypes = [P, C.c_int]
+    lib.psf_profile_enable.restype = C.c_int
+    lib.psf_profile_read.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_int)]
+    lib.psf_profile_read.restype = C.c_int
+    lib.psf_last_upload_bytes.argtypes = [P]
+    lib.psf_last_upload_bytes.restype = C.c_longlong
     lib.psf_host_tables.argtypes = [C.POINTER(psf_plan_desc), C.POINTER(C.c_float), C.c_int, C.c_int,
                                     C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double), C.POINTER(C.c_ubyte)]
@@ -167,6 +174,20 @@ class PsfPlan:
         s = torch.cuda.current_stream(dev) if stream is None else stream
         self.compute_raw(s.cuda_stream, intensity.data_ptr(), field.data_ptr() if field is not None else 0)
         return (intensity, field) if field is not None else intensity
+
+    def profile_enable(self, enable: bool = True):
+        self._check(self._lib.psf_profile_enable(self._h, int(bool(enable))))
+
+    def profile_read(self):
+        """(stage_ms[4], launches[4]) of the last compute; the caller must have synchronised its stream."""
+        ms = (C.c_float * 4)()
+        ln = (C.c_int * 4)()
+        self._check(self._lib.psf_profile_read(self._h, ms, ln))
+        return list(ms), list(ln)
+
+    @property
+    def last_upload_bytes(self) -> int:
+        return int(self._lib.psf_last_upload_bytes(self._h))
 
     @property
     def launches_per_compute(self) -> int:

@@ -23,12 +23,17 @@ const size_t kScratchBudget = (size_t)48 << 20;   // T scratch ring: small enoug
   } while (0)
 
 template <typename T>
-psf_status upload(psf_plan *p, void **dptr, const std::vector<T> &h) {
-  if (*dptr) { cudaFree(*dptr); *dptr = nullptr; }
-  if (h.empty()) return PSF_OK;
-  cudaError_t e = cudaMalloc(dptr, h.size() * sizeof(T));
-  if (e != cudaSuccess) { p->err = std::string("cudaMalloc: ") + cudaGetErrorString(e); *dptr = nullptr; return PSF_ERR_ALLOC; }
-  CU_TRY(p, cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+psf_status upload(psf_plan *p, void **dptr, size_t *cap, const std::vector<T> &h) {
+  const size_t bytes = h.size() * sizeof(T);
+  if (bytes == 0) return PSF_OK;
+  if (bytes > *cap) {
+    if (*dptr) { cudaFree(*dptr); *dptr = nullptr; *cap = 0; }
+    cudaError_t e = cudaMalloc(dptr, bytes);
+    if (e != cudaSuccess) { p->err = std::string("cudaMalloc: ") + cudaGetErrorString(e); *dptr = nullptr; return PSF_ERR_ALLOC; }
+    *cap = bytes;
+  }
+  CU_TRY(p, cudaMemcpy(*dptr, h.data(), bytes, cudaMemcpyHostToDevice));
+  p->upload_bytes += (long long)bytes;
   return PSF_OK;
 }
 
@@ -38,9 +43,15 @@ inline void split2(double v, float &hi, float &lo) { hi = (float)v; lo = (float)
 // Folds the static pupil about both axes into the four parity classes and uploads every static table.
 psf_status upload_static(psf_plan *p) {
   const psf_plan_desc &d = p->desc;
-  HostPupil hp;
-  const bool shared_z = !p->zern_shared.empty();
-  build_host_pupil(d, shared_z ? p->zern_shared.data() : nullptr, p->noll_first, (int)p->zern_shared.size(), hp);
+  const HostPupil &hp = p->hp0;
+  const int Kneed = p->zern_shared.empty() ? p->K_rows : (int)p->zern_shared.size();
+  if (Kneed > 0 && (p->zb_first != p->noll_first || p->zb_K != Kneed)) {
+    build_zernike_basis(hp, p->noll_first, Kneed, p->zbasis);
+    p->zb_first = p->noll_first;
+    p->zb_K = Kneed;
+  }
+  std::vector<cplx> base_z;
+  apply_shared_zernike(hp, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis, base_z);
   const int N = d.pupil_n, n = (N + 1) / 2, C = hp.C;
   const size_t NN = (size_t)N * N, nn = (size_t)n * n;
   DevPlan &P = p->dp;
@@ -58,7 +69,7 @@ psf_status upload_static(psf_plan *p) {
       split2(hp.kappa[(size_t)qy * N + qx] / twopi, hi, lo);
       kt[(size_t)qy * n + qx] = make_float2(hi, lo);
       for (int c = 0; c < C; ++c) {
-        const cplx *B = hp.base.data() + (size_t)c * NN;
+        const cplx *B = base_z.data() + (size_t)c * NN;
         const cplx p00 = B[(size_t)qy * N + qx];
         const cplx p01 = sx ? cplx(0, 0) : B[(size_t)qy * N + rx];
         const cplx p10 = sy ? cplx(0, 0) : B[(size_t)ry * N + qx];
@@ -74,23 +85,21 @@ psf_status upload_static(psf_plan *p) {
     }
   }
   psf_status s;
-  if ((s = upload(p, &p->d_bfold, bfold)) != PSF_OK) return s;
-  if ((s = upload(p, &p->d_kt, kt)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_bfold, &p->cap_bfold, bfold)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_kt, &p->cap_kt, kt)) != PSF_OK) return s;
   P.bfold = (const float4 *)p->d_bfold;
   P.kt = (const float2 *)p->d_kt;
 
   if (P.per_plane) {
     std::vector<float2> bunf((size_t)C * NN);
-    for (size_t i = 0; i < bunf.size(); ++i) bunf[i] = make_float2((float)hp.base[i].real(), (float)hp.base[i].imag());
-    if ((s = upload(p, &p->d_bunf, bunf)) != PSF_OK) return s;
+    for (size_t i = 0; i < bunf.size(); ++i) bunf[i] = make_float2((float)base_z[i].real(), (float)base_z[i].imag());
+    if ((s = upload(p, &p->d_bunf, &p->cap_bunf, bunf)) != PSF_OK) return s;
     P.bunf = (const float2 *)p->d_bunf;
     const int K = p->K_rows;
     std::vector<float> zb((size_t)K * NN, 0.f);
-    for (int j = 0; j < K; ++j)
-      for (size_t i = 0; i < NN; ++i)
-        if (hp.mask[i]) zb[(size_t)j * NN + i] = (float)(zernike_noll(p->noll_first + j, hp.rho[i], hp.cosphi[i], hp.sinphi[i]) / twopi);
-    if ((s = upload(p, &p->d_zb, zb)) != PSF_OK) return s;
-    if ((s = upload(p, &p->d_coef, p->zern_rows)) != PSF_OK) return s;
+    for (size_t i = 0; i < zb.size(); ++i) zb[i] = (float)(p->zbasis[i] / twopi);
+    if ((s = upload(p, &p->d_zb, &p->cap_zb, zb)) != PSF_OK) return s;
+    if ((s = upload(p, &p->d_coef, &p->cap_coef, p->zern_rows)) != PSF_OK) return s;
     P.zb = (const float *)p->d_zb;
     P.coef = (const float *)p->d_coef;
     P.K = K;
@@ -108,7 +117,7 @@ psf_status upload_static(psf_plan *p) {
     if (P.has_shift) { tx = (float)(tscale * (double)p->shifts[2 * b]); ty = (float)(tscale * (double)p->shifts[2 * b + 1]); }
     planes[b] = make_float4(zh, zl, tx, ty);
   }
-  if ((s = upload(p, &p->d_planes, planes)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_planes, &p->cap_planes, planes)) != PSF_OK) return s;
   P.planes = (const float4 *)p->d_planes;
   return PSF_OK;
 }
@@ -119,8 +128,8 @@ psf_status upload_dft(psf_plan *p) {
   std::vector<float> c(phi.size()), s(phi.size());
   for (size_t i = 0; i < phi.size(); ++i) { c[i] = (float)std::cos(phi[i]); s[i] = (float)std::sin(phi[i]); }
   psf_status st;
-  if ((st = upload(p, &p->d_cos, c)) != PSF_OK) return st;
-  if ((st = upload(p, &p->d_sin, s)) != PSF_OK) return st;
+  if ((st = upload(p, &p->d_cos, &p->cap_cos, c)) != PSF_OK) return st;
+  if ((st = upload(p, &p->d_sin, &p->cap_sin, s)) != PSF_OK) return st;
   p->dp.cosT = (const float *)p->d_cos;
   p->dp.sinT = (const float *)p->d_sin;
   return PSF_OK;
@@ -145,6 +154,7 @@ psf_status alloc_scratch(psf_plan *p) {
 }
 
 psf_status refresh(psf_plan *p) {
+  p->upload_bytes = 0;
   psf_status s = upload_static(p);
   if (s != PSF_OK) return s;
   return alloc_scratch(p);     // C is fixed per plan, but keep the scratch consistent with it
@@ -154,6 +164,8 @@ void free_all(psf_plan *p) {
   void **bufs[] = {&p->d_bfold, &p->d_kt, &p->d_bunf, &p->d_zb, &p->d_coef, &p->d_planes, &p->d_cos, &p->d_sin, &p->d_T};
   for (void **b : bufs)
     if (*b) { cudaFree(*b); *b = nullptr; }
+  for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
+  p->prof_ev.clear();
 }
 
 }  // namespace
@@ -199,7 +211,8 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
     return PSF_ERR_CUDA;
   }
   p->path = 0;
-  if ((s = upload_dft(p)) != PSF_OK || (s = refresh(p)) != PSF_OK) {
+  build_host_pupil(p->desc, nullptr, 1, 0, p->hp0);
+  if ((s = refresh(p)) != PSF_OK || (s = upload_dft(p)) != PSF_OK) {
     g_create_err = p->err;
     free_all(p);
     delete p;
@@ -253,6 +266,11 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
     p->err = "field output is undefined for PSF_POL_UNPOLARIZED (two incoherent fields)";
     return PSF_ERR_UNSUPPORTED;
   }
+  if (p->prof) {
+    p->prof_n = 0;
+    p->prof_valid = true;
+    cudaEventRecord(p->prof_ev[0], (cudaStream_t)cuda_stream);
+  }
   cudaError_t e = launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
@@ -271,6 +289,42 @@ const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_cr
 int psf_launches_per_compute(const psf_plan *p) { return p ? ffma_launches(p) : 0; }
 
 const char *psf_path_name(const psf_plan *p) { return (p && p->path == 1) ? "tc3xtf32" : "ffma"; }
+
+psf_status psf_profile_enable(psf_plan *p, int enable) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  p->prof = false;
+  p->prof_valid = false;
+  if (!enable) return PSF_OK;
+  const size_t need = (size_t)psf_launches_per_compute(p) + 1;
+  while (p->prof_ev.size() < need) {
+    cudaEvent_t ev;
+    if ((e = cudaEventCreate(&ev)) != cudaSuccess) { p->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
+    p->prof_ev.push_back(ev);
+  }
+  p->prof_stage.assign(p->prof_ev.size(), 0);
+  p->prof = true;
+  return PSF_OK;
+}
+
+psf_status psf_profile_read(psf_plan *p, float *stage_ms, int *launches) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (!stage_ms || !launches) { p->err = "NULL output"; return PSF_ERR_INVALID_ARG; }
+  if (!p->prof || !p->prof_valid) { p->err = "profiling is not enabled or no psf_compute ran since"; return PSF_ERR_STATE; }
+  for (int i = 0; i < 4; ++i) { stage_ms[i] = 0.f; launches[i] = 0; }
+  for (int i = 0; i < p->prof_n; ++i) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventElapsedTime(&ms, p->prof_ev[i], p->prof_ev[i + 1]);
+    if (e != cudaSuccess) { p->err = std::string("cudaEventElapsedTime: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
+    const int st = p->prof_stage[i] & 3;
+    stage_ms[st] += ms;
+    launches[st] += 1;
+  }
+  return PSF_OK;
+}
+
+long long psf_last_upload_bytes(const psf_plan *p) { return p ? p->upload_bytes : 0; }
 
 psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int noll_first, int n_coeffs, int *n_components,
                            double *weights, double *base, double *kappa, unsigned char *mask) {

@@ -173,6 +173,28 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
   }
 }
 
+void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<double> &out) {
+  const size_t NN = (size_t)P.N * P.N;
+  out.assign((size_t)K * NN, 0.0);
+  for (int j = 0; j < K; ++j)
+    for (size_t i = 0; i < NN; ++i)
+      if (P.mask[i]) out[(size_t)j * NN + i] = zernike_noll(noll_first + j, P.rho[i], P.cosphi[i], P.sinphi[i]);
+}
+
+void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
+                          std::vector<cplx> &base) {
+  const size_t NN = (size_t)P0.N * P0.N;
+  base = P0.base;
+  if (!coeffs || K <= 0) return;
+  for (size_t i = 0; i < NN; ++i) {
+    if (!P0.mask[i]) continue;
+    double W = 0.0;
+    for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];
+    const cplx e(std::cos(W), std::sin(W));
+    for (int c = 0; c < P0.C; ++c) base[(size_t)c * NN + i] *= e;
+  }
+}
+
 void build_dft_phase(const psf_plan_desc &d, std::vector<double> &phi) {
   const int N = d.pupil_n, M = d.out_m;
   const int n = (N + 1) / 2, m = (M + 1) / 2;

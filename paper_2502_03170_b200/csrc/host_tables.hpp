@@ -36,6 +36,13 @@ double zernike_noll(int j, double rho, double cosphi, double sinphi);
 // Builds the static pupil. `coeffs` (may be null) is a shared Zernike term folded into W_static.
 void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_first, int n_coeffs, HostPupil &out);
 
+// Zernike basis values Z_{noll_first+j} at every in-disc sample: out[j][N][N] (0 outside the disc).
+void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<double> &out);
+
+// base[c][i] = P0.base[c][i] * exp(i sum_j coeffs[j] basis[j][i]): the shared Zernike term folded into the static pupil.
+void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
+                          std::vector<cplx> &base);
+
 // Zoomed-DFT phase table: phi[mi][qi] = k s_max u_qi x_mi for mi < m = ceil(M/2), qi < n = ceil(N/2).
 void build_dft_phase(const psf_plan_desc &d, std::vector<double> &phi);
 

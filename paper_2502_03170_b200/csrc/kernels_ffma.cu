@@ -235,9 +235,11 @@ cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, fl
     dim3 g1((P.m + K1_COLS - 1) / K1_COLS, (P.n + K1_ROWS - 1) / K1_ROWS, zc * P.C);
     if (P.per_plane) k1_stage1<true><<<g1, K1_THREADS, 0, st>>>(P, z0, T);
     else k1_stage1<false><<<g1, K1_THREADS, 0, st>>>(P, z0, T);
+    prof_mark(p, st, 0);
     dim3 g2((P.m + K2_MX - 1) / K2_MX, (P.m + K2_MY - 1) / K2_MY, zc);
     if (field) k2_stage2<true><<<g2, K2_THREADS, 0, st>>>(P, z0, T, intensity, field);
     else k2_stage2<false><<<g2, K2_THREADS, 0, st>>>(P, z0, T, intensity, nullptr);
+    prof_mark(p, st, 1);
   }
   return cudaGetLastError();
 }

@@ -48,15 +48,33 @@ struct psf_plan {
   std::vector<float> zern_rows;  // [Z][K]
   int K_rows = 0;
   std::vector<float> shifts;     // [Z][2]
+  // host caches: static pupil without any Zernike term, and the Zernike basis of the last (noll_first, K)
+  psf::HostPupil hp0;
+  std::vector<double> zbasis;    // [K][N][N]
+  int zb_first = 0, zb_K = 0;
+  long long upload_bytes = 0;
+  // profiling (psf_profile_enable)
+  bool prof = false, prof_valid = false;
+  std::vector<cudaEvent_t> prof_ev;
+  std::vector<int> prof_stage;   // stage of the launch that ends at event i+1
+  int prof_n = 0;
   // device buffers (owned)
   void *d_bfold = nullptr, *d_kt = nullptr, *d_bunf = nullptr, *d_zb = nullptr, *d_coef = nullptr;
   void *d_planes = nullptr, *d_cos = nullptr, *d_sin = nullptr, *d_T = nullptr;
   size_t T_bytes = 0;
+  size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
   int path = 0;                  // 0 = ffma, 1 = tc3xtf32
   psf::TcState *tc = nullptr;
 };
 
 namespace psf {
+// Marks the end of one kernel launch of `stage` for the profiler (no-op unless psf_profile_enable is on).
+inline void prof_mark(const psf_plan *p, cudaStream_t st, int stage) {
+  psf_plan *q = const_cast<psf_plan *>(p);
+  if (!q->prof || q->prof_n + 1 >= (int)q->prof_ev.size()) return;
+  q->prof_stage[q->prof_n] = stage;
+  cudaEventRecord(q->prof_ev[++q->prof_n], st);
+}
 // kernels_ffma.cu
 cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 int ffma_launches(const psf_plan *p);
