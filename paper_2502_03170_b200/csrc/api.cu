@@ -119,12 +119,16 @@ psf_status upload_static(psf_plan *p) {
   }
   if ((s = upload(p, &p->d_planes, &p->cap_planes, planes)) != PSF_OK) return s;
   P.planes = (const float4 *)p->d_planes;
+  // path: tensor cores for the static (shared-pupil) mode when asked for or when the problem is large enough
+  const psf_precision prec = d.precision;
+  const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || tc_eligible(p));
+  p->path = want_tc ? 1 : 0;
+  if (want_tc && (s = tc_setup(p, bfold, kt, p->phi)) != PSF_OK) return s;
   return PSF_OK;
 }
 
 psf_status upload_dft(psf_plan *p) {
-  std::vector<double> phi;
-  build_dft_phase(p->desc, phi);
+  const std::vector<double> &phi = p->phi;
   std::vector<float> c(phi.size()), s(phi.size());
   for (size_t i = 0; i < phi.size(); ++i) { c[i] = (float)std::cos(phi[i]); s[i] = (float)std::sin(phi[i]); }
   psf_status st;
@@ -166,6 +170,7 @@ void free_all(psf_plan *p) {
     if (*b) { cudaFree(*b); *b = nullptr; }
   for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
   p->prof_ev.clear();
+  tc_free(p);
 }
 
 }  // namespace
@@ -212,6 +217,7 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
   }
   p->path = 0;
   build_host_pupil(p->desc, nullptr, 1, 0, p->hp0);
+  build_dft_phase(p->desc, p->phi);
   if ((s = refresh(p)) != PSF_OK || (s = upload_dft(p)) != PSF_OK) {
     g_create_err = p->err;
     free_all(p);
@@ -271,7 +277,8 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
     p->prof_valid = true;
     cudaEventRecord(p->prof_ev[0], (cudaStream_t)cuda_stream);
   }
-  cudaError_t e = launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
+  cudaError_t e = (p->path == 1 && !field) ? launch_tc(p, (cudaStream_t)cuda_stream, intensity)
+                                            : launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
 }
@@ -286,7 +293,10 @@ psf_status psf_plan_destroy(psf_plan *p) {
 
 const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_create_err.c_str(); }
 
-int psf_launches_per_compute(const psf_plan *p) { return p ? ffma_launches(p) : 0; }
+int psf_launches_per_compute(const psf_plan *p) {
+  if (!p) return 0;
+  return (p->path == 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
+}
 
 const char *psf_path_name(const psf_plan *p) { return (p && p->path == 1) ? "tc3xtf32" : "ffma"; }
 
@@ -297,7 +307,8 @@ psf_status psf_profile_enable(psf_plan *p, int enable) {
   p->prof = false;
   p->prof_valid = false;
   if (!enable) return PSF_OK;
-  const size_t need = (size_t)psf_launches_per_compute(p) + 1;
+  size_t need = (size_t)ffma_launches(p) + 1;
+  if (p->tc && (size_t)tc_launches(p) + 1 > need) need = (size_t)tc_launches(p) + 1;
   while (p->prof_ev.size() < need) {
     cudaEvent_t ev;
     if ((e = cudaEventCreate(&ev)) != cudaSuccess) { p->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }

@@ -65,6 +65,7 @@ struct psf_plan {
   size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
   int path = 0;                  // 0 = ffma, 1 = tc3xtf32
   psf::TcState *tc = nullptr;
+  std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
 
 namespace psf {
@@ -78,4 +79,10 @@ inline void prof_mark(const psf_plan *p, cudaStream_t st, int stage) {
 // kernels_ffma.cu
 cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 int ffma_launches(const psf_plan *p);
+// kernels_tc.cu
+bool tc_eligible(const psf_plan *p);
+psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::vector<float2> &kt, const std::vector<double> &phi);
+void tc_free(psf_plan *p);
+int tc_launches(const psf_plan *p);
+cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity);
 }  // namespace psf
