@@ -68,7 +68,9 @@ enum {
 typedef enum {
   PSF_PREC_AUTO = 0,   /* the library picks per problem size                                                    */
   PSF_PREC_3XTF32 = 1, /* tcgen05 tensor cores, both operands split hi/lo in TF32 (fp32-level accuracy)         */
-  PSF_PREC_FP32 = 2    /* plain fp32 FFMA tiles                                                                 */
+  PSF_PREC_FP32 = 2,   /* plain fp32 FFMA tiles                                                                 */
+  PSF_PREC_3XF16 = 3   /* tcgen05 tensor cores, both operands pre-scaled by powers of two and split hi/lo in FP16:
+                          same 11-bit parts as 3XTF32, half the bytes, twice the tensor rate     */
 } psf_precision;
 
 typedef struct {

@@ -15,7 +15,7 @@ STATUS_NAMES = {0: "PSF_OK", 1: "PSF_ERR_INVALID_ARG", 2: "PSF_ERR_UNSUPPORTED",
                 4: "PSF_ERR_CUDA", 5: "PSF_ERR_STATE"}
 POL = {"x": 0, "y": 1, "circ_l": 2, "circ_r": 3, "jones": 4, "unpolarized": 5}
 FLAG_APODIZE, FLAG_GIBSON_LANNI, FLAG_FRESNEL = 1, 2, 4
-PREC = {"auto": 0, "3xtf32": 1, "fp32": 2}
+PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_compute", "psf_plan_destroy",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",

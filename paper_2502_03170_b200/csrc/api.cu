@@ -121,9 +121,9 @@ psf_status upload_static(psf_plan *p) {
   P.planes = (const float4 *)p->d_planes;
   // path: tensor cores for the static (shared-pupil) mode when asked for or when the problem is large enough
   const psf_precision prec = d.precision;
-  const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || tc_eligible(p));
-  p->path = want_tc ? 1 : 0;
-  if (want_tc && (s = tc_setup(p, bfold, kt, p->phi)) != PSF_OK) return s;
+  const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || prec == PSF_PREC_3XF16 || tc_eligible(p));
+  p->path = want_tc ? (prec == PSF_PREC_3XF16 ? 2 : 1) : 0;
+  if (want_tc && (s = tc_setup(p, bfold, kt, p->phi, p->path == 2)) != PSF_OK) return s;
   return PSF_OK;
 }
 
@@ -277,7 +277,7 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
     p->prof_valid = true;
     cudaEventRecord(p->prof_ev[0], (cudaStream_t)cuda_stream);
   }
-  cudaError_t e = (p->path == 1 && !field) ? launch_tc(p, (cudaStream_t)cuda_stream, intensity)
+  cudaError_t e = (p->path >= 1 && !field) ? launch_tc(p, (cudaStream_t)cuda_stream, intensity)
                                             : launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
@@ -295,10 +295,10 @@ const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_cr
 
 int psf_launches_per_compute(const psf_plan *p) {
   if (!p) return 0;
-  return (p->path == 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
+  return (p->path >= 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
 }
 
-const char *psf_path_name(const psf_plan *p) { return (p && p->path == 1) ? "tc3xtf32" : "ffma"; }
+const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
 
 psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!p) return PSF_ERR_INVALID_ARG;

@@ -63,7 +63,7 @@ struct psf_plan {
   void *d_planes = nullptr, *d_cos = nullptr, *d_sin = nullptr, *d_T = nullptr;
   size_t T_bytes = 0;
   size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
-  int path = 0;                  // 0 = ffma, 1 = tc3xtf32
+  int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16
   psf::TcState *tc = nullptr;
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
@@ -81,7 +81,8 @@ cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, fl
 int ffma_launches(const psf_plan *p);
 // kernels_tc.cu
 bool tc_eligible(const psf_plan *p);
-psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::vector<float2> &kt, const std::vector<double> &phi);
+psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::vector<float2> &kt, const std::vector<double> &phi,
+                    bool f16);
 void tc_free(psf_plan *p);
 int tc_launches(const psf_plan *p);
 cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity);
