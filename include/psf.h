@@ -66,7 +66,7 @@ enum {
 };
 
 typedef enum {
-  PSF_PREC_AUTO = 0,   /* the library picks per problem size                                                    */
+  PSF_PREC_AUTO = 0,   /* the library picks per problem size: 3XF16 when the tensor tiles fill, FP32 otherwise  */
   PSF_PREC_3XTF32 = 1, /* tcgen05 tensor cores, both operands split hi/lo in TF32 (fp32-level accuracy)         */
   PSF_PREC_FP32 = 2,   /* plain fp32 FFMA tiles                                                                 */
   PSF_PREC_3XF16 = 3   /* tcgen05 tensor cores, both operands pre-scaled by powers of two and split hi/lo in FP16:
@@ -124,7 +124,7 @@ const char *psf_last_error(const psf_plan *plan);
 /* Number of kernel launches one psf_compute call of this plan enqueues (for benchmarking records). */
 int psf_launches_per_compute(const psf_plan *plan);
 
-/* Name of the kernel path the plan selected: "ffma", "tc3xtf32", ... (static string). */
+/* Name of the kernel path the plan selected: "ffma", "tc3xtf32", "tc3xf16" (static string). */
 const char *psf_path_name(const psf_plan *plan);
 
 /* Profiling aid for bench.py.  enable != 0: create CUDA events (this call may allocate) and make every later

@@ -43,7 +43,7 @@ def plane_errors(I_gpu, I_ref):
     return err / peak
 
 
-PRECISIONS = ["fp32", "auto"]
+PRECISIONS = ["fp32", "auto", "3xtf32", "3xf16"]
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
