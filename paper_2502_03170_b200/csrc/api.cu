@@ -103,8 +103,32 @@ psf_status upload_static(psf_plan *p) {
     P.zb = (const float *)p->d_zb;
     P.coef = (const float *)p->d_coef;
     P.K = K;
+    // folded, parity-sorted copy for the fused small-grid kernel: Z_j(-x, y) = +-Z_j(x, y), Z_j(x, -y) = +-Z_j(x, y)
+    //   m = 0: even/even;  cos(m phi): even in y, odd in x iff m odd;  sin(m phi): odd in y, odd in x iff m even
+    std::vector<int> order;
+    for (int i = 0; i < 4; ++i) P.zcnt[i] = 0;
+    for (int cls = 0; cls < 4; ++cls)
+      for (int j = 0; j < K; ++j) {
+        int zn, zm, kind;
+        noll_to_nm(p->noll_first + j, zn, zm, kind);
+        const int xo = (kind == 0) ? 0 : (kind == 1 ? (zm & 1) : ((zm + 1) & 1));
+        const int yo = (kind == 2) ? 1 : 0;
+        if (xo + 2 * yo == cls) { order.push_back(j); P.zcnt[cls]++; }
+      }
+    std::vector<float> zbq((size_t)K * nn, 0.f), coefq(p->zern_rows.size(), 0.f);
+    for (int k = 0; k < K; ++k) {
+      const int j = order[k];
+      for (int qy = 0; qy < n; ++qy)
+        for (int qx = 0; qx < n; ++qx) zbq[(size_t)k * nn + (size_t)qy * n + qx] = (float)(p->zbasis[(size_t)j * NN + (size_t)qy * N + qx] / twopi);
+      for (int b = 0; b < d.n_planes; ++b) coefq[(size_t)b * K + k] = p->zern_rows[(size_t)b * K + j];
+    }
+    if ((s = upload(p, &p->d_zbq, &p->cap_zbq, zbq)) != PSF_OK) return s;
+    if ((s = upload(p, &p->d_coefq, &p->cap_coefq, coefq)) != PSF_OK) return s;
+    P.zbq = (const float *)p->d_zbq;
+    P.coefq = (const float *)p->d_coefq;
   } else {
     P.K = 0;
+    for (int i = 0; i < 4; ++i) P.zcnt[i] = 0;
   }
   // plane table
   std::vector<float4> planes(d.n_planes);
@@ -123,6 +147,7 @@ psf_status upload_static(psf_plan *p) {
   const psf_precision prec = d.precision;
   const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || prec == PSF_PREC_3XF16 || tc_eligible(p));
   p->path = want_tc ? (prec == PSF_PREC_3XTF32 ? 1 : 2) : 0;     // AUTO: the fp16 split (same accuracy, about twice as fast)
+  if (!want_tc && small_eligible(p)) p->path = 3;                // whole path fused in one CTA per plane
   if (want_tc && (s = tc_setup(p, bfold, kt, p->phi, p->path == 2)) != PSF_OK) return s;
   return PSF_OK;
 }
@@ -165,7 +190,8 @@ psf_status refresh(psf_plan *p) {
 }
 
 void free_all(psf_plan *p) {
-  void **bufs[] = {&p->d_bfold, &p->d_kt, &p->d_bunf, &p->d_zb, &p->d_coef, &p->d_planes, &p->d_cos, &p->d_sin, &p->d_T};
+  void **bufs[] = {&p->d_bfold, &p->d_kt, &p->d_bunf, &p->d_zb, &p->d_coef, &p->d_planes, &p->d_cos, &p->d_sin, &p->d_T,
+                   &p->d_zbq, &p->d_coefq};
   for (void **b : bufs)
     if (*b) { cudaFree(*b); *b = nullptr; }
   for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
@@ -277,8 +303,11 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
     p->prof_valid = true;
     cudaEventRecord(p->prof_ev[0], (cudaStream_t)cuda_stream);
   }
-  cudaError_t e = (p->path >= 1 && !field) ? launch_tc(p, (cudaStream_t)cuda_stream, intensity)
-                                            : launch_ffma(p, (cudaStream_t)cuda_stream, intensity, (float2 *)field);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool tc = (p->path == 1 || p->path == 2) && !field;
+  cudaError_t e = tc ? launch_tc(p, st, intensity)
+                     : (p->path == 3 || small_eligible(p)) ? launch_small(p, st, intensity, (float2 *)field)
+                                                            : launch_ffma(p, st, intensity, (float2 *)field);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
 }
@@ -295,10 +324,11 @@ const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_cr
 
 int psf_launches_per_compute(const psf_plan *p) {
   if (!p) return 0;
+  if (p->path == 3) return 1;
   return (p->path >= 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
 }
 
-const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
+const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 3 ? "ffma_fused" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
 
 psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!p) return PSF_ERR_INVALID_ARG;

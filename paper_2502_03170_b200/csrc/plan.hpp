@@ -25,6 +25,9 @@ struct DevPlan {
   const float2 *bunf;            // [C][N][N]     unfolded base pupil (per-plane mode)
   const float *zb;               // [K][N][N]     Zernike basis / 2 pi (turns per radian of coefficient)
   const float *coef;             // [Z][K]        per-plane coefficients
+  const float *zbq;              // [K][n][n]     the same basis on the folded quadrant, terms sorted by parity class
+  const float *coefq;            // [Z][K]        coefficient rows in that order
+  int zcnt[4];                   // terms per parity class: even/even, odd in x, odd in y, odd/odd
   const float4 *planes;          // [Z]           (z_hi, z_lo, t_x, t_y): t = k s_max x_b / 2 pi
   const float *cosT, *sinT;      // [m][n]        cos / sin of k s_max u_q x_mi
 };
@@ -60,10 +63,11 @@ struct psf_plan {
   int prof_n = 0;
   // device buffers (owned)
   void *d_bfold = nullptr, *d_kt = nullptr, *d_bunf = nullptr, *d_zb = nullptr, *d_coef = nullptr;
-  void *d_planes = nullptr, *d_cos = nullptr, *d_sin = nullptr, *d_T = nullptr;
+  void *d_planes = nullptr, *d_cos = nullptr, *d_sin = nullptr, *d_T = nullptr, *d_zbq = nullptr, *d_coefq = nullptr;
+  size_t cap_zbq = 0, cap_coefq = 0;
   size_t T_bytes = 0;
   size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
-  int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16
+  int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16, 3 = ffma_fused (small grids)
   psf::TcState *tc = nullptr;
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
@@ -79,6 +83,9 @@ inline void prof_mark(const psf_plan *p, cudaStream_t st, int stage) {
 // kernels_ffma.cu
 cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 int ffma_launches(const psf_plan *p);
+// kernels_small.cu
+bool small_eligible(const psf_plan *p);
+cudaError_t launch_small(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 // kernels_tc.cu
 bool tc_eligible(const psf_plan *p);
 psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::vector<float2> &kt, const std::vector<double> &phi,
