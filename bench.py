@@ -30,8 +30,14 @@ SM_COUNT, FMA_LANES_PER_SM = 148, 128
 TF32_OVER_BF16 = 1.1 / 2.25            # nominal dense ratio (B200_PROFILING.md table)
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu captures
-# (profiles/*.md name the command); keyed by (path, workload).  None where no capture exists yet.
-NCU_TRAFFIC_BYTES = {}
+# (profiles/*.md name the command); keyed by (path, workload, stage), in bytes PER PLANE of the captured launch (scaled to
+# the mean planes per launch below).  None where no capture exists yet.
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1c_ncu_tc_cfg5.md: k2_tc<f16>, 146-plane launch: 1.676 GB read + 0.208 GB written
+    ("tc3xf16", "cfg5_large_stack", 1): (1.675852e9 + 0.208072e9) / 146,
+    # same capture, k1_tc<f16>: 0.018 GB read + 1.551 GB written
+    ("tc3xf16", "cfg5_large_stack", 0): (0.018017e9 + 1.551206e9) / 146,
+}
 
 
 def load_peaks():
@@ -183,7 +189,7 @@ def blas_threads():
     return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
 
 
-ORACLE_PLANES = {1: 16, 2: 32, 3: 24, 4: 1024, 5: 4}    # about 5-30 s of CPU work each on the 16-core B200 host
+ORACLE_PLANES = {1: 16, 2: 64, 3: 128, 4: 4096, 5: 128}    # about 10-30 s of CPU work each on the 16-core B200 host
 
 
 def run_oracle_once(case, planes):
@@ -287,7 +293,7 @@ def run_ours(args):
     launches_dom = max(int(res["stage_launches"][dom]), 1)
     dur_ms = stage_ms[dom] / launches_dom
     path = res["path"]
-    if path == "ffma":
+    if path in ("ffma", "ffma_fused"):
         bound = "alu"
         peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
         executed = flop_dom
@@ -296,12 +302,19 @@ def run_ours(args):
         bound = "tensor"
         long_step = ms_per_step > 1000.0
         bf16 = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
-        peak = bf16 * TF32_OVER_BF16
+        which = f"{peaks['_source']} bf16 {'sustained' if long_step else 'burst'} {bf16:.1f} TF/s"
         executed = 3.0 * flop_dom
-        peak_note = (f"{peaks['_source']} bf16 {'sustained' if long_step else 'burst'} {bf16:.1f} TF/s x nominal tf32/bf16 "
-                     f"ratio {TF32_OVER_BF16:.3f}; achieved counts executed TF32 flop (3 products per fp32 product)")
+        if path == "tc3xf16":      # kind::f16 runs at the bf16 rate: the measured cuBLAS bf16 figure is the peak itself
+            peak = bf16
+            peak_note = f"{which} (fp16 = bf16 tensor rate); achieved counts executed FP16 flop (3 products per fp32 product)"
+        else:
+            peak = bf16 * TF32_OVER_BF16
+            peak_note = (f"{which} x nominal tf32/bf16 ratio {TF32_OVER_BF16:.3f}; achieved counts executed TF32 flop "
+                         f"(3 products per fp32 product)")
     achieved = executed / launches_dom / (dur_ms * 1e-3) / 1e12
-    traffic = NCU_TRAFFIC_BYTES.get((path, case.name))
+    traffic = NCU_TRAFFIC_BYTES.get((path, case.name, dom))
+    if traffic is not None:
+        traffic *= case.n_planes / launches_dom
     roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "kernel": ("stage1_rowdft_producer", "stage2_coldft_intensity")[dom],
                 "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
@@ -310,7 +323,7 @@ def run_ours(args):
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if path == "ffma" else "tf32x3", "data": "synthetic",
+            "dtype": {"tc3xf16": "f16x3", "tc3xtf32": "tf32x3"}.get(path, "f32"), "data": "synthetic",
             "config": {"workload": case.name, "N": case.pupil_n, "M": case.out_m, "Z": case.n_planes,
                        "pol": case.pol, "path": path, "planes_per_s": case.n_planes * world / (ms_per_step * 1e-3),
                        "l2": "256 MiB buffer written between timed iterations (flush)", "sharding": "z-shards, no collective"},
