@@ -1,0 +1,552 @@
+// CTA-pair (cta_group::2) versions of the two tcgen05 stages for the 3xFP16 path.  Two CTAs on the SMs of one TPC form a
+// cluster and execute each UMMA together: M = 256 rows (128 per CTA), N = 256 columns of which each CTA stages one half
+// (128 rows of the B operand).  Per CTA this halves the B-operand bytes per flop: the L2 -> SM ingress and the
+// shared-memory read bandwidth stop being the limit they are for single-CTA 128 x 256 tiles with hi + lo operands
+// (DESIGN.md §5).  Only the leader CTA (cluster rank 0) issues tcgen05.mma; both CTAs load / generate operands, both
+// drain their own 128 TMEM lanes.
+//
+//   k1_pair (stage 1):  D[mx, (half, slot, ql)] = X_g[mx, qx] * Q[(half, slot, ql), qx]^T      M = 256 mx, N = 256
+//       A = cos / sin table rows of the CTA's own 128 mx, by TMA;
+//       B = pupil field: CTA `half` generates slots (4 chains of the x-parity group) x 32 q_y = 128 rows straight into its
+//           swizzled shared memory (each pupil element is generated once per pair);
+//       epilogue: one thread per mx row holds 64 consecutive q_y of a chain -> scale, fp16 hi / lo, 16-byte stores into a
+//           swizzled staging tile, TMA store into T^T[chain][mx][qy].
+//   k2_pair (stage 2):  D[my, (slot, mx)] = Y_a[my, qy] * T^T[(slot, mx), qy]^T                 M = 256 my, N = 4 x 64
+//       both operands by TMA (each CTA: its own 128 my rows of the table, 2 of the 4 chains of T^T);
+//       epilogue as k2_tc (mirror butterfly, |E|^2, running sums over the components) with a coalesced final store
+//       through a padded shared-memory tile.
+#pragma once
+#include <cuda.h>
+#include <cuda_fp16.h>
+
+#include "pupil_gen.cuh"
+#include "tc_common.cuh"
+
+namespace psf {
+namespace pair {
+
+using namespace tc;
+
+// ---- cluster / pair primitives ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of `saddr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {   // acquire at cluster scope
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// TMA loads whose completion bytes are credited to an mbarrier of the pair's leader CTA (`bar_cluster` = mapa(bar, 0))
+__device__ __forceinline__ void tma2_load_2d(uint32_t smem_dst, const void *tmap, uint32_t bar_cluster, int x, int y) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_dst), "l"((uint64_t)tmap), "r"(bar_cluster), "r"(x), "r"(y)
+      : "memory");
+}
+__device__ __forceinline__ void tma2_load_3d(uint32_t smem_dst, const void *tmap, uint32_t bar_cluster, int x, int y, int z) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(smem_dst), "l"((uint64_t)tmap), "r"(bar_cluster), "r"(x), "r"(y), "r"(z)
+      : "memory");
+}
+// TMA store shared -> global (bulk async-group completion)
+__device__ __forceinline__ void tma_store_3d(const void *tmap, uint32_t smem_src, int x, int y, int z) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"((uint64_t)tmap), "r"(smem_src), "r"(x), "r"(y), "r"(z)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ void tmem_alloc2(uint32_t *slot, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc2(uint32_t base, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void umma2_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// arrive on the barrier at the same shared-memory offset in both CTAs once the pair's previously issued UMMAs are done
+__device__ __forceinline__ void umma2_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(smem_u32(bar)), "h"((uint16_t)3)
+               : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void st_shared_v4(uint32_t saddr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+
+constexpr int TILE16K = 128 * 128;                       // 128 rows x one 128-byte swizzle row
+constexpr int P_STAGE = 4 * TILE16K;                     // A hi, A lo, B-half hi, B-half lo = 64 KB per CTA
+constexpr uint32_t P_IDESC = umma_idesc_f16(256, 256);
+
+// one stage = 64 contraction indices: D += A_lo B_hi + A_hi B_lo + A_hi B_hi, four K = 16 steps
+__device__ __forceinline__ void issue_stage_mmas2(uint32_t sbase, uint32_t d_tmem, bool first) {
+  const uint32_t ah = sbase, al = sbase + TILE16K, bh = sbase + 2 * TILE16K, bl = sbase + 3 * TILE16K;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t o = k * 32;
+    umma2_f16(d_tmem, umma_desc_sw128(al + o), umma_desc_sw128(bh + o), P_IDESC, (first && k == 0) ? 0u : 1u);
+    umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bl + o), P_IDESC, 1u);
+    umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bh + o), P_IDESC, 1u);
+  }
+}
+
+// ---- stage 2 ----------------------------------------------------------------------------------------------------------
+struct K2PArgs {
+  float *intensity;     // [Z][M][M]
+  int C, n_pad, m_pad, m, M, z0, zc;
+  float weight[5];      // intensity weights times the inverse operand scales squared
+};
+
+constexpr int K2P_NST = 3;
+constexpr int K2P_EPI_WARPS = 16;
+constexpr int K2P_THREADS = 32 * (4 + K2P_EPI_WARPS);
+constexpr int K2P_PITCH = 65;                                    // staging row pitch in floats (conflict-free column writes)
+constexpr int K2P_STAGING = 128 * K2P_PITCH * 4;
+constexpr int K2P_SMEM = 1024 + K2P_NST * P_STAGE + K2P_STAGING;
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K2P_THREADS, 1)
+k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
+        const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo, const K2PArgs P) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
+  __shared__ uint64_t full[K2P_NST], empty[K2P_NST], acc_full, acc_empty;
+  __shared__ uint32_t tmem_slot;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const bool leader = rank == 0;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < K2P_NST; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+    mbar_init(&acc_full, 1);
+    mbar_init(&acc_empty, 2 * K2P_EPI_WARPS);
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_thi); prefetch_tmap(&map_tlo); }
+  if (warp == 1) tmem_alloc2(&tmem_slot, 512);
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();                       // the peer's barriers are initialised before anything remote touches them
+  tcgen05_fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  const int nk = P.n_pad / 64;
+  const int tiles_yp = (P.m_pad / 128 + 1) / 2, tiles_x = P.m_pad / 64;
+  const int ntiles = P.zc * tiles_yp * tiles_x;
+  const int ncl = gridDim.x >> 1, cid = blockIdx.x >> 1;
+
+  if (warp == 0) {
+    // ---------------- TMA: own 128 table rows (A) and 2 of the 4 chains of T^T (B half) ----------------
+    if (elect_one()) {
+      int st = 0, ph = 0;
+      uint32_t full_leader[K2P_NST];
+      for (int i = 0; i < K2P_NST; ++i) full_leader[i] = mapa(smem_u32(&full[i]), 0);
+      for (int t = cid; t < ntiles; t += ncl) {
+        const int typ = t % tiles_yp;
+        int r = t / tiles_yp;
+        const int tx = r % tiles_x;
+        const int zl = r / tiles_x;
+        const int ty = typ * 2 + (int)rank;
+        for (int c = 0; c < P.C; ++c) {
+          for (int a = 0; a < 2; ++a) {
+            const int arow = a * P.m_pad + ty * 128;
+            const int chain0 = (zl * P.C + c) * 8 + 4 * a + 2 * (int)rank;
+            for (int kc = 0; kc < nk; ++kc) {
+              mbar_wait(&empty[st], ph ^ 1);
+              const uint32_t s = smem_u32(smem + st * P_STAGE);
+              if (leader) mbar_arrive_expect_tx(&full[st], 2 * P_STAGE);
+              tma2_load_2d(s, &map_xhi, full_leader[st], kc * 64, arow);
+              tma2_load_2d(s + TILE16K, &map_xlo, full_leader[st], kc * 64, arow);
+              tma2_load_3d(s + 2 * TILE16K, &map_thi, full_leader[st], kc * 64, tx * 64, chain0);
+              tma2_load_3d(s + 3 * TILE16K, &map_tlo, full_leader[st], kc * 64, tx * 64, chain0);
+              if (++st == K2P_NST) { st = 0; ph ^= 1; }
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ---------------- MMA issuer (leader CTA only) ----------------
+    if (leader && elect_one()) {
+      int st = 0, ph = 0, item = 0;
+      for (int t = cid; t < ntiles; t += ncl) {
+        for (int c = 0; c < P.C; ++c, ++item) {
+          mbar_wait_cluster(&acc_empty, (item & 1) ^ 1);
+          tcgen05_fence_after();
+          for (int a = 0; a < 2; ++a) {
+            const uint32_t d = tmem + a * 256;
+            for (int kc = 0; kc < nk; ++kc) {
+              mbar_wait_cluster(&full[st], ph);
+              tcgen05_fence_after();
+              issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
+              umma2_commit(&empty[st]);
+              if (++st == K2P_NST) { st = 0; ph ^= 1; }
+            }
+          }
+          umma2_commit(&acc_full);
+        }
+      }
+    }
+  } else if (warp >= 4) {
+    // ---------------- epilogue: butterfly + |E|^2, running sums over components ----------------
+    const int q = warp & 3;                 // TMEM lane quarter
+    const int e = (warp - 4) >> 2;          // 16-column slice of the 64 mx of the tile
+    const int wi = warp - 4;
+    const uint32_t acc_empty_leader = mapa(smem_u32(&acc_empty), 0);
+    int item = 0;
+    for (int t = cid; t < ntiles; t += ncl) {
+      const int typ = t % tiles_yp;
+      int r = t / tiles_yp;
+      const int tx = r % tiles_x;
+      const int zl = r / tiles_x;
+      const int ty = typ * 2 + (int)rank;
+      float sum[4][16];
+#pragma unroll
+      for (int qd = 0; qd < 4; ++qd)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) sum[qd][i] = 0.f;
+      for (int c = 0; c < P.C; ++c, ++item) {
+        const float w = P.weight[c];
+        mbar_wait(&acc_full, item & 1);
+        tcgen05_fence_after();
+#pragma unroll
+        for (int i4 = 0; i4 < 4; ++i4) {
+          uint32_t v[8][4];
+#pragma unroll
+          for (int ch = 0; ch < 8; ++ch)
+            tmem_ld_32x32b_x4(tmem + ((uint32_t)(q * 32) << 16) + (ch >> 2) * 256 + (ch & 3) * 64 + e * 16 + i4 * 4, v[ch]);
+          tmem_ld_wait();
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const float a0 = __uint_as_float(v[0][u]), a1 = __uint_as_float(v[1][u]), a2 = __uint_as_float(v[2][u]),
+                        a3 = __uint_as_float(v[3][u]), a4 = __uint_as_float(v[4][u]), a5 = __uint_as_float(v[5][u]),
+                        a6 = __uint_as_float(v[6][u]), a7 = __uint_as_float(v[7][u]);
+            const float pr = a0 - a5, qr = a0 + a5, rr = a3 + a6, sr = a3 - a6;
+            const float pi = a1 + a4, qi = a1 - a4, ri = a2 - a7, si = a2 + a7;
+            const float re0 = pr - rr, im0 = pi + ri;   // (my, mx)
+            const float re1 = pr + rr, im1 = pi - ri;   // (my, mirrored mx)
+            const float re2 = qr - sr, im2 = qi + si;   // (mirrored my, mx)
+            const float re3 = qr + sr, im3 = qi - si;   // (mirrored my, mirrored mx)
+            const int i = i4 * 4 + u;
+            sum[0][i] = fmaf(w, re0 * re0 + im0 * im0, sum[0][i]);
+            sum[1][i] = fmaf(w, re1 * re1 + im1 * im1, sum[1][i]);
+            sum[2][i] = fmaf(w, re2 * re2 + im2 * im2, sum[2][i]);
+            sum[3][i] = fmaf(w, re3 * re3 + im3 * im3, sum[3][i]);
+          }
+        }
+        tcgen05_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(acc_empty_leader);
+      }
+      // coalesced store of the four mirrored quadrants through the padded staging tile
+      float *Ib = P.intensity + (size_t)(P.z0 + zl) * P.M * P.M;
+#pragma unroll
+      for (int qd = 0; qd < 4; ++qd) {
+        named_bar_sync(1, 32 * K2P_EPI_WARPS);
+        float *srow = staging + (q * 32 + lane) * K2P_PITCH + e * 16;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) srow[i] = sum[qd][i];
+        named_bar_sync(1, 32 * K2P_EPI_WARPS);
+#pragma unroll
+        for (int rr = 0; rr < 8; ++rr) {
+          const int row = wi * 8 + rr;
+          const int my = ty * 128 + row;
+          if (my < P.m) {
+            const int y = (qd & 2) ? P.M - 1 - my : my;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const int col = h * 32 + lane;
+              const int mx = tx * 64 + col;
+              if (mx < P.m) {
+                const int x = (qd & 1) ? P.M - 1 - mx : mx;
+                Ib[(size_t)y * P.M + x] = staging[row * K2P_PITCH + col];
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == 1) tmem_dealloc2(tmem, 512);
+}
+
+// ---- stage 1 ----------------------------------------------------------------------------------------------------------
+struct K1PArgs {
+  const float4 *bgrp;   // [2][C][n_pad][n_pad]  pre-scaled by s_Q
+  const float2 *ktp;    // [n_pad][n_pad]
+  const float4 *planes; // [Z]
+  int C, n_pad, m_pad, z0, zc;
+  float f1;             // epilogue factor s_T / (s_Q s_X)
+};
+
+constexpr int K1P_NST = 2;
+constexpr int K1P_PRODUCER_WARPS = 8;
+constexpr int K1P_THREADS = 32 * (2 + K1P_PRODUCER_WARPS + 4);
+constexpr int K1P_STAGING = 2 * TILE16K;                          // hi + lo tile of one chain: 128 mx x 64 qy
+constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + 2 * K1P_STAGING;
+constexpr int K1P_QY = 64;                                        // q_y per tile (32 generated by each CTA)
+
+// Producer work item: one pipeline stage of one (plane, jt, c, g): this thread's 8 consecutive q_x of one q_y row.
+struct K1PIter {
+  int t, c, g, kc;      // tile, component, x-parity group, k-chunk
+  int jt;               // decoded tile
+  float zh, zl;
+};
+__device__ __forceinline__ void k1p_decode(K1PIter &it, const K1PArgs &P, int tiles_j, int tiles_m, int ntiles) {
+  if (it.t >= ntiles) return;
+  int r = it.t / tiles_m;
+  it.jt = r % tiles_j;
+  const float4 pl = __ldg(P.planes + P.z0 + r / tiles_j);
+  it.zh = pl.x; it.zl = pl.y;
+}
+__device__ __forceinline__ void k1p_advance(K1PIter &it, const K1PArgs &P, int nk, int tiles_j, int tiles_m, int ntiles, int ncl) {
+  if (++it.kc < nk) return;
+  it.kc = 0;
+  if (++it.g < 2) return;
+  it.g = 0;
+  if (++it.c < P.C) return;
+  it.c = 0;
+  it.t += ncl;
+  k1p_decode(it, P, tiles_j, tiles_m, ntiles);
+}
+// loads for one item: 8 (kappa hi, lo) pairs and 8 base-pupil float4 (4 slots) of row `qy`, columns kc*64 + cg*8 + 0..7
+__device__ __forceinline__ void k1p_load(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&kt)[4], float4 (&bb)[8]) {
+  const size_t s = (size_t)(it.jt * K1P_QY + qyl) * P.n_pad + it.kc * 64 + cg * 8;
+  const float4 *k4 = reinterpret_cast<const float4 *>(P.ktp + s);
+  const float4 *b4 = P.bgrp + ((size_t)(it.g * P.C + it.c) * P.n_pad) * P.n_pad + s;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) bb[i] = __ldg(b4 + i);
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K1P_THREADS, 1)
+k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
+        const __grid_constant__ CUtensorMap map_this, const __grid_constant__ CUtensorMap map_tlos, const K1PArgs P) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
+  __shared__ uint32_t tmem_slot;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const bool leader = rank == 0;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < K1P_NST; ++i) { mbar_init(&full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 8); }
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_this); prefetch_tmap(&map_tlos); }
+  if (warp == 1) tmem_alloc2(&tmem_slot, 512);
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tcgen05_fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  const int nk = P.n_pad / 64;
+  const int tiles_j = P.n_pad / K1P_QY, tiles_m = P.m_pad / 256;
+  const int ntiles = P.zc * tiles_j * tiles_m;                    // a tile = (plane, jt, mx pair-tile); c and g loop inside
+  const int ncl = gridDim.x >> 1, cid = blockIdx.x >> 1;
+
+  if (warp == 0) {
+    // ---------------- TMA: cos / sin table rows of this CTA's 128 mx (A operand) ----------------
+    if (elect_one()) {
+      int st = 0, ph = 0;
+      uint32_t full_leader[K1P_NST];
+      for (int i = 0; i < K1P_NST; ++i) full_leader[i] = mapa(smem_u32(&full[i]), 0);
+      for (int t = cid; t < ntiles; t += ncl) {
+        const int mt = t % tiles_m;
+        for (int cg = 0; cg < 2 * P.C; ++cg) {
+          const int row = (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
+          for (int kc = 0; kc < nk; ++kc) {
+            mbar_wait(&empty[st], ph ^ 1);
+            const uint32_t s = smem_u32(smem + st * P_STAGE);
+            if (leader) mbar_arrive_expect_tx(&full[st], 4 * TILE16K);
+            tma2_load_2d(s, &map_xhi, full_leader[st], kc * 64, row);
+            tma2_load_2d(s + TILE16K, &map_xlo, full_leader[st], kc * 64, row);
+            if (++st == K1P_NST) { st = 0; ph ^= 1; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ---------------- MMA issuer (leader CTA only) ----------------
+    if (leader && elect_one()) {
+      int st = 0, ph = 0, it = 0;
+      for (int t = cid; t < ntiles; t += ncl) {
+        for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
+          const int g = cg & 1;
+          mbar_wait_cluster(&acc_empty[g], ((it >> 1) & 1) ^ 1);
+          tcgen05_fence_after();
+          const uint32_t d = tmem + g * 256;
+          for (int kc = 0; kc < nk; ++kc) {
+            mbar_wait_cluster(&full[st], ph);
+            tcgen05_fence_after();
+            issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
+            umma2_commit(&empty[st]);
+            if (++st == K1P_NST) { st = 0; ph ^= 1; }
+          }
+          umma2_commit(&acc_full[g]);
+        }
+      }
+    }
+  } else if (warp < 2 + K1P_PRODUCER_WARPS) {
+    // ---------------- pupil-field producers: this CTA's 32 q_y x 4 slots = 128 B-operand rows ----------------
+    const int tid = threadIdx.x - 64;
+    const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
+    const int qyl = (int)rank * 32 + ql;                           // q_y within the tile
+    // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
+    const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
+    const uint32_t full_leader0 = mapa(smem_u32(&full[0]), 0);
+    const uint32_t smem0 = smem_u32(smem);
+    int st = 0, ph = 0;
+    K1PIter cur{cid, 0, 0, 0, 0, 0.f, 0.f};
+    k1p_decode(cur, P, tiles_j, tiles_m, ntiles);
+    float4 kt[4], bb[8];
+    if (cur.t < ntiles) k1p_load(cur, P, qyl, cgp, kt, bb);
+    while (cur.t < ntiles) {
+      K1PIter nxt = cur;
+      k1p_advance(nxt, P, nk, tiles_j, tiles_m, ntiles, ncl);
+      float4 ktn[4], bbn[8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) ktn[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) bbn[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (nxt.t < ntiles) k1p_load(nxt, P, qyl, cgp, ktn, bbn);   // prefetch: covers the L2 latency with this stage's math
+      uint32_t hi[4][4], lo[4][4];                                 // [slot][pair of q_x]
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {                                // two samples per iteration
+        float sn0, cs0, sn1, cs1;
+        {
+          const float t0 = kz_turns(make_float2(kt[i].x, kt[i].y), cur.zh, cur.zl);
+          const float t1 = kz_turns(make_float2(kt[i].z, kt[i].w), cur.zh, cur.zl);
+          sn0 = __sinf(6.283185307179586f * t0); cs0 = __cosf(6.283185307179586f * t0);
+          sn1 = __sinf(6.283185307179586f * t1); cs1 = __cosf(6.283185307179586f * t1);
+        }
+        const float4 b0 = bb[2 * i], b1 = bb[2 * i + 1];
+        split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
+        split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
+        split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
+        split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
+      }
+      mbar_wait(&empty[st], ph ^ 1);
+      const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
+        st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
+      }
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
+      if (++st == K1P_NST) { st = 0; ph ^= 1; }
+      cur = nxt;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) kt[i] = ktn[i];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) bb[i] = bbn[i];
+    }
+  } else {
+    // ---------------- epilogue: TMEM -> scale -> fp16 hi / lo -> swizzled staging -> TMA store of T^T ----------------
+    const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
+    const int row = q * 32 + lane;
+    const int et = threadIdx.x - 32 * (2 + K1P_PRODUCER_WARPS);   // 0..127
+    const uint32_t stg0 = smem_u32(smem + K1P_NST * P_STAGE);
+    const uint32_t acc_empty_leader = mapa(smem_u32(&acc_empty[0]), 0);
+    const uint32_t rbase = (uint32_t)row * 128u;
+    int it = 0, sbuf = 0;
+    for (int t = cid; t < ntiles; t += ncl) {
+      const int mt = t % tiles_m;
+      int r = t / tiles_m;
+      const int jt = r % tiles_j;
+      const int zl = r / tiles_j;
+      for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
+        const int g = cg & 1, c = cg >> 1;
+        mbar_wait(&acc_full[g], (it >> 1) & 1);
+        tcgen05_fence_after();
+#pragma unroll 1
+        for (int s = 0; s < 4; ++s) {
+          // the staging buffer used two slots ago has been read by its TMA store
+          if (et == 0) bulk_wait_read<1>();
+          named_bar_sync(2, 128);
+          const uint32_t sh = stg0 + sbuf * K1P_STAGING + rbase, sl = sh + TILE16K;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {            // q_y half h was generated by CTA h: columns h*128 + s*32 + 0..31
+            uint32_t v[32];
+            tmem_ld_32x32b_x32(tmem + ((uint32_t)(q * 32) << 16) + g * 256 + h * 128 + s * 32, v);
+            tmem_ld_wait();
+            uint32_t ph[16], pl[16];
+#pragma unroll
+            for (int e = 0; e < 16; ++e)
+              split_f16x2(__uint_as_float(v[2 * e]) * P.f1, __uint_as_float(v[2 * e + 1]) * P.f1, ph[e], pl[e]);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {          // 16-byte chunk h*4 + j of the 128-byte row
+              const uint32_t o = (((uint32_t)(h * 4 + j) ^ ((uint32_t)row & 7u)) << 4);
+              st_shared_v4(sh + o, ph[4 * j], ph[4 * j + 1], ph[4 * j + 2], ph[4 * j + 3]);
+              st_shared_v4(sl + o, pl[4 * j], pl[4 * j + 1], pl[4 * j + 2], pl[4 * j + 3]);
+            }
+          }
+          fence_proxy_async_smem();
+          named_bar_sync(2, 128);
+          if (et == 0) {
+            const int j = (s >> 1) * 4 + g * 2 + (s & 1);          // chain index of slot s in group g
+            const int chain = (zl * P.C + c) * 8 + j;
+            const int mx0 = mt * 256 + (int)rank * 128;
+            tma_store_3d(&map_this, stg0 + sbuf * K1P_STAGING, jt * K1P_QY, mx0, chain);
+            tma_store_3d(&map_tlos, stg0 + sbuf * K1P_STAGING + TILE16K, jt * K1P_QY, mx0, chain);
+            bulk_commit();
+          }
+          sbuf ^= 1;
+        }
+        tcgen05_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + g * 8);
+      }
+    }
+    if (et == 0) bulk_wait_all();
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == 1) tmem_dealloc2(tmem, 512);
+}
+
+}  // namespace pair
+}  // namespace psf
