@@ -43,9 +43,14 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
   return r;
 }
+// default semantics (release at CTA scope): a cluster-scope release compiles to MEMBAR.ALL.GPU + ERRBAR, microseconds per
+// arrive; what the waiter needs here (shared-memory operand writes made visible to the async proxy, TMEM reads
+// completed) is ordered by the fence.proxy.async / tcgen05.wait::ld + tcgen05.fence issued before the arrive
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {   // acquire at cluster scope
   uint32_t ok;
   do {
@@ -137,37 +142,18 @@ constexpr int K2P_PITCH = 65;                                    // staging row 
 constexpr int K2P_STAGING = 128 * K2P_PITCH * 4;
 constexpr int K2P_SMEM = 1024 + K2P_NST * P_STAGE + K2P_STAGING;
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K2P_THREADS, 1)
-k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
-        const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo, const K2PArgs P) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
-  __shared__ uint64_t full[K2P_NST], empty[K2P_NST], acc_full, acc_empty;
-  __shared__ uint32_t tmem_slot;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
+struct K2PShared {
+  uint64_t full[K2P_NST], empty[K2P_NST], acc_full, acc_empty;
+  uint32_t tmem_slot;
+};
+
+// TMA warp (both CTAs) and MMA warp (leader CTA)
+__device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
+                                         const CUtensorMap &map_thi, const CUtensorMap &map_tlo, const K2PArgs &P, int warp, uint32_t rank,
+                                         int nk, int tiles_yp, int tiles_x, int ntiles, int ncl, int cid) {
   const bool leader = rank == 0;
-
-  if (threadIdx.x == 0) {
-    for (int i = 0; i < K2P_NST; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-    mbar_init(&acc_full, 1);
-    mbar_init(&acc_empty, 2 * K2P_EPI_WARPS);
-    fence_barrier_init();
-  }
-  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_thi); prefetch_tmap(&map_tlo); }
-  if (warp == 1) tmem_alloc2(&tmem_slot, 512);
-  tcgen05_fence_before();
-  __syncthreads();
-  cluster_sync_all();                       // the peer's barriers are initialised before anything remote touches them
-  tcgen05_fence_after();
-  const uint32_t tmem = tmem_slot;
-
-  const int nk = P.n_pad / 64;
-  const int tiles_yp = (P.m_pad / 128 + 1) / 2, tiles_x = P.m_pad / 64;
-  const int ntiles = P.zc * tiles_yp * tiles_x;
-  const int ncl = gridDim.x >> 1, cid = blockIdx.x >> 1;
-
+  uint64_t *full = S.full, *empty = S.empty;
+  uint64_t &acc_full = S.acc_full, &acc_empty = S.acc_empty;
   if (warp == 0) {
     // ---------------- TMA: own 128 table rows (A) and 2 of the 4 chains of T^T (B half) ----------------
     if (elect_one()) {
@@ -220,8 +206,14 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
         }
       }
     }
-  } else if (warp >= 4) {
-    // ---------------- epilogue: butterfly + |E|^2, running sums over components ----------------
+  }
+}
+
+// sixteen epilogue warps: butterfly + |E|^2, running sums over the components, coalesced quadrant stores
+__device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint32_t tmem, const K2PArgs &P, int warp, int lane, uint32_t rank,
+                                             int tiles_yp, int tiles_x, int ntiles, int ncl, int cid) {
+  uint64_t &acc_full = S.acc_full, &acc_empty = S.acc_empty;
+  {
     const int q = warp & 3;                 // TMEM lane quarter
     const int e = (warp - 4) >> 2;          // 16-column slice of the 64 mx of the tile
     const int wi = warp - 4;
@@ -249,6 +241,11 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
           for (int ch = 0; ch < 8; ++ch)
             tmem_ld_32x32b_x4(tmem + ((uint32_t)(q * 32) << 16) + (ch >> 2) * 256 + (ch & 3) * 64 + e * 16 + i4 * 4, v[ch]);
           tmem_ld_wait();
+          if (i4 == 3) {                      // every TMEM read of this item is done: the MMAs of the next one may start
+            tcgen05_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(acc_empty_leader);
+          }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const float a0 = __uint_as_float(v[0][u]), a1 = __uint_as_float(v[1][u]), a2 = __uint_as_float(v[2][u]),
@@ -267,9 +264,6 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
             sum[3][i] = fmaf(w, re3 * re3 + im3 * im3, sum[3][i]);
           }
         }
-        tcgen05_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(acc_empty_leader);
       }
       // coalesced store of the four mirrored quadrants through the padded staging tile
       float *Ib = P.intensity + (size_t)(P.z0 + zl) * P.M * P.M;
@@ -299,6 +293,45 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
         }
       }
     }
+  }
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K2P_THREADS, 1)
+k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
+        const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo, const K2PArgs P) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
+  __shared__ K2PShared S;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < K2P_NST; ++i) { mbar_init(&S.full[i], 1); mbar_init(&S.empty[i], 1); }
+    mbar_init(&S.acc_full, 1);
+    mbar_init(&S.acc_empty, 2 * K2P_EPI_WARPS);
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_thi); prefetch_tmap(&map_tlo); }
+  if (warp == 1) tmem_alloc2(&S.tmem_slot, 512);
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();                       // the peer's barriers are initialised before anything remote touches them
+  tcgen05_fence_after();
+  const uint32_t tmem = S.tmem_slot;
+
+  const int nk = P.n_pad / 64;
+  const int tiles_yp = (P.m_pad / 128 + 1) / 2, tiles_x = P.m_pad / 64;
+  const int ntiles = P.zc * tiles_yp * tiles_x;
+  const int ncl = gridDim.x >> 1, cid = blockIdx.x >> 1;
+
+  // register budget: launch = 640 x 96; the four feeder warps drop to 24 registers, the sixteen epilogue warps take 112 (128 x 24 + 512 x 112 <= 640 x 96)
+  if (warp < 4) {
+    setmaxnreg_dec<24>();
+    k2p_feed(smem, S, tmem, map_xhi, map_xlo, map_thi, map_tlo, P, warp, rank, nk, tiles_yp, tiles_x, ntiles, ncl, cid);
+  } else {
+    setmaxnreg_inc<112>();
+    k2p_epilogue(staging, S, tmem, P, warp, lane, rank, tiles_yp, tiles_x, ntiles, ncl, cid);
   }
   tcgen05_fence_before();
   __syncthreads();
