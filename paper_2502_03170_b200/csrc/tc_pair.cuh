@@ -350,10 +350,19 @@ struct K1PArgs {
 
 constexpr int K1P_NST = 2;
 constexpr int K1P_PRODUCER_WARPS = 8;
-constexpr int K1P_THREADS = 32 * (2 + K1P_PRODUCER_WARPS + 4);
-constexpr int K1P_STAGING = 2 * TILE16K;                          // hi + lo tile of one chain: 128 mx x 64 qy
-constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + 2 * K1P_STAGING;
+constexpr int K1P_FEED_WARPS = 4;                                  // TMA, MMA, two idle: roles fill whole warpgroups (setmaxnreg)
+constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
+constexpr int K1P_STAGING = 2 * TILE16K;                          // hi tile + lo tile of one chain: 128 mx x 64 qy each
+constexpr int K1P_SC_KC = 4;                                      // k-chunks covered by the sin / cos cache (n_pad <= 256)
+constexpr int K1P_SINCOS = K1P_SC_KC * 4 * 256 * 16;              // 64 KB: 8 (cos, sin) pairs per producer thread and k-chunk
+constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + K1P_STAGING + K1P_SINCOS;
 constexpr int K1P_QY = 64;                                        // q_y per tile (32 generated by each CTA)
+
+struct K1PShared {
+  uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
+  uint32_t tmem_slot;
+};
+struct K1PGeom { int nk, tiles_j, tiles_m, ntiles, ncl, cid; };
 
 // Producer work item: one pipeline stage of one (plane, jt, c, g): this thread's 8 consecutive q_x of one q_y row.
 struct K1PIter {
@@ -361,77 +370,63 @@ struct K1PIter {
   int jt;               // decoded tile
   float zh, zl;
 };
-__device__ __forceinline__ void k1p_decode(K1PIter &it, const K1PArgs &P, int tiles_j, int tiles_m, int ntiles) {
-  if (it.t >= ntiles) return;
-  int r = it.t / tiles_m;
-  it.jt = r % tiles_j;
-  const float4 pl = __ldg(P.planes + P.z0 + r / tiles_j);
+__device__ __forceinline__ void k1p_decode(K1PIter &it, const K1PArgs &P, const K1PGeom &G) {
+  if (it.t >= G.ntiles) return;
+  const int r = it.t / G.tiles_m;
+  it.jt = r % G.tiles_j;
+  const float4 pl = __ldg(P.planes + P.z0 + r / G.tiles_j);
   it.zh = pl.x; it.zl = pl.y;
 }
-__device__ __forceinline__ void k1p_advance(K1PIter &it, const K1PArgs &P, int nk, int tiles_j, int tiles_m, int ntiles, int ncl) {
-  if (++it.kc < nk) return;
+__device__ __forceinline__ void k1p_advance(K1PIter &it, const K1PArgs &P, const K1PGeom &G) {
+  if (++it.kc < G.nk) return;
   it.kc = 0;
   if (++it.g < 2) return;
   it.g = 0;
   if (++it.c < P.C) return;
   it.c = 0;
-  it.t += ncl;
-  k1p_decode(it, P, tiles_j, tiles_m, ntiles);
+  it.t += G.ncl;
+  k1p_decode(it, P, G);
 }
-// loads for one item: 8 (kappa hi, lo) pairs and 8 base-pupil float4 (4 slots) of row `qy`, columns kc*64 + cg*8 + 0..7
-__device__ __forceinline__ void k1p_load(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&kt)[4], float4 (&bb)[8]) {
-  const size_t s = (size_t)(it.jt * K1P_QY + qyl) * P.n_pad + it.kc * 64 + cg * 8;
-  const float4 *k4 = reinterpret_cast<const float4 *>(P.ktp + s);
-  const float4 *b4 = P.bgrp + ((size_t)(it.g * P.C + it.c) * P.n_pad) * P.n_pad + s;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i);
+// sample index of this thread's first q_x of item `it`
+__device__ __forceinline__ size_t k1p_sample(const K1PIter &it, const K1PArgs &P, int qyl, int cg) {
+  return (size_t)(it.jt * K1P_QY + qyl) * P.n_pad + it.kc * 64 + cg * 8;
+}
+__device__ __forceinline__ void k1p_load_bb(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&bb)[8]) {
+  const float4 *b4 = P.bgrp + ((size_t)(it.g * P.C + it.c) * P.n_pad) * P.n_pad + k1p_sample(it, P, qyl, cg);
 #pragma unroll
   for (int i = 0; i < 8; ++i) bb[i] = __ldg(b4 + i);
 }
+__device__ __forceinline__ void k1p_load_kt(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&kt)[4]) {
+  const float4 *k4 = reinterpret_cast<const float4 *>(P.ktp + k1p_sample(it, P, qyl, cg));
+#pragma unroll
+  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i);
+}
+__device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+  return v;
+}
+__device__ __forceinline__ void st_shared_v4f(uint32_t saddr, float4 v) {
+  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K1P_THREADS, 1)
-k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
-        const __grid_constant__ CUtensorMap map_this, const __grid_constant__ CUtensorMap map_tlos, const K1PArgs P) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  __shared__ uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
-  __shared__ uint32_t tmem_slot;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
+// TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
+__device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
+                                         const K1PArgs &P, const K1PGeom &G, int warp, uint32_t rank) {
   const bool leader = rank == 0;
-
-  if (threadIdx.x == 0) {
-    for (int i = 0; i < K1P_NST; ++i) { mbar_init(&full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&acc_full[i], 1); mbar_init(&acc_empty[i], 8); }
-    fence_barrier_init();
-  }
-  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_this); prefetch_tmap(&map_tlos); }
-  if (warp == 1) tmem_alloc2(&tmem_slot, 512);
-  tcgen05_fence_before();
-  __syncthreads();
-  cluster_sync_all();
-  tcgen05_fence_after();
-  const uint32_t tmem = tmem_slot;
-
-  const int nk = P.n_pad / 64;
-  const int tiles_j = P.n_pad / K1P_QY, tiles_m = P.m_pad / 256;
-  const int ntiles = P.zc * tiles_j * tiles_m;                    // a tile = (plane, jt, mx pair-tile); c and g loop inside
-  const int ncl = gridDim.x >> 1, cid = blockIdx.x >> 1;
-
   if (warp == 0) {
-    // ---------------- TMA: cos / sin table rows of this CTA's 128 mx (A operand) ----------------
     if (elect_one()) {
       int st = 0, ph = 0;
       uint32_t full_leader[K1P_NST];
-      for (int i = 0; i < K1P_NST; ++i) full_leader[i] = mapa(smem_u32(&full[i]), 0);
-      for (int t = cid; t < ntiles; t += ncl) {
-        const int mt = t % tiles_m;
+      for (int i = 0; i < K1P_NST; ++i) full_leader[i] = mapa(smem_u32(&S.full[i]), 0);
+      for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+        const int mt = t % G.tiles_m;
         for (int cg = 0; cg < 2 * P.C; ++cg) {
           const int row = (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
-          for (int kc = 0; kc < nk; ++kc) {
-            mbar_wait(&empty[st], ph ^ 1);
+          for (int kc = 0; kc < G.nk; ++kc) {
+            mbar_wait(&S.empty[st], ph ^ 1);
             const uint32_t s = smem_u32(smem + st * P_STAGE);
-            if (leader) mbar_arrive_expect_tx(&full[st], 4 * TILE16K);
+            if (leader) mbar_arrive_expect_tx(&S.full[st], 4 * TILE16K);
             tma2_load_2d(s, &map_xhi, full_leader[st], kc * 64, row);
             tma2_load_2d(s + TILE16K, &map_xlo, full_leader[st], kc * 64, row);
             if (++st == K1P_NST) { st = 0; ph ^= 1; }
@@ -440,140 +435,212 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
       }
     }
   } else if (warp == 1) {
-    // ---------------- MMA issuer (leader CTA only) ----------------
     if (leader && elect_one()) {
       int st = 0, ph = 0, it = 0;
-      for (int t = cid; t < ntiles; t += ncl) {
+      for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
           const int g = cg & 1;
-          mbar_wait_cluster(&acc_empty[g], ((it >> 1) & 1) ^ 1);
+          mbar_wait_cluster(&S.acc_empty[g], ((it >> 1) & 1) ^ 1);
           tcgen05_fence_after();
           const uint32_t d = tmem + g * 256;
-          for (int kc = 0; kc < nk; ++kc) {
-            mbar_wait_cluster(&full[st], ph);
+          for (int kc = 0; kc < G.nk; ++kc) {
+            mbar_wait_cluster(&S.full[st], ph);
             tcgen05_fence_after();
             issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
-            umma2_commit(&empty[st]);
+            umma2_commit(&S.empty[st]);
             if (++st == K1P_NST) { st = 0; ph ^= 1; }
           }
-          umma2_commit(&acc_full[g]);
+          umma2_commit(&S.acc_full[g]);
         }
       }
     }
-  } else if (warp < 2 + K1P_PRODUCER_WARPS) {
-    // ---------------- pupil-field producers: this CTA's 32 q_y x 4 slots = 128 B-operand rows ----------------
-    const int tid = threadIdx.x - 64;
-    const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
-    const int qyl = (int)rank * 32 + ql;                           // q_y within the tile
-    // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
-    const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
-    const uint32_t full_leader0 = mapa(smem_u32(&full[0]), 0);
-    const uint32_t smem0 = smem_u32(smem);
-    int st = 0, ph = 0;
-    K1PIter cur{cid, 0, 0, 0, 0, 0.f, 0.f};
-    k1p_decode(cur, P, tiles_j, tiles_m, ntiles);
-    float4 kt[4], bb[8];
-    if (cur.t < ntiles) k1p_load(cur, P, qyl, cgp, kt, bb);
-    while (cur.t < ntiles) {
-      K1PIter nxt = cur;
-      k1p_advance(nxt, P, nk, tiles_j, tiles_m, ntiles, ncl);
-      float4 ktn[4], bbn[8];
+  }
+}
+
+// Eight producer warps: this CTA's 32 q_y x 4 slots = 128 B-operand rows per stage.  The defocus phasor of a sample is the
+// same for all 2 C (component, group) items of a tile: it is computed at the first item and parked in a per-thread
+// shared-memory cache; the base-pupil loads run two stages ahead of their use.
+__device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
+  const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
+  const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
+  const int qyl = (int)rank * 32 + ql;                           // q_y within the tile
+  // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
+  const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
+  const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
+  const uint32_t smem0 = smem_u32(smem);
+  const uint32_t sc0 = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // cache: [(kc*4 + j)][thread] float4
+  const bool cached = G.nk <= K1P_SC_KC;
+  int st = 0, ph = 0;
+  K1PIter cur{G.cid, 0, 0, 0, 0, 0.f, 0.f};
+  k1p_decode(cur, P, G);
+  K1PIter pre = cur;                                             // item whose base-pupil loads are issued next
+  float4 bb[3][8], kt[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) ktn[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int i = 0; i < 4; ++i) kt[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (cur.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[0]); k1p_load_kt(cur, P, qyl, cgp, kt); k1p_advance(pre, P, G); }
+  if (pre.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[1]); k1p_advance(pre, P, G); }
+  while (cur.t < G.ntiles) {
 #pragma unroll
-      for (int i = 0; i < 8; ++i) bbn[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (nxt.t < ntiles) k1p_load(nxt, P, qyl, cgp, ktn, bbn);   // prefetch: covers the L2 latency with this stage's math
-      uint32_t hi[4][4], lo[4][4];                                 // [slot][pair of q_x]
+    for (int u = 0; u < 3; ++u) {
+      if (cur.t < G.ntiles) {
+        if (pre.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[(u + 2) % 3]); k1p_advance(pre, P, G); }
+        // (cos, sin) of the 8 samples
+        float4 sc[4];
+        const bool first = !cached || (cur.c == 0 && cur.g == 0);
+        if (first) {
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {                                // two samples per iteration
-        float sn0, cs0, sn1, cs1;
-        {
-          const float t0 = kz_turns(make_float2(kt[i].x, kt[i].y), cur.zh, cur.zl);
-          const float t1 = kz_turns(make_float2(kt[i].z, kt[i].w), cur.zh, cur.zl);
-          sn0 = __sinf(6.283185307179586f * t0); cs0 = __cosf(6.283185307179586f * t0);
-          sn1 = __sinf(6.283185307179586f * t1); cs1 = __cosf(6.283185307179586f * t1);
+          for (int i = 0; i < 4; ++i) {
+            const float t0 = 6.283185307179586f * kz_turns(make_float2(kt[i].x, kt[i].y), cur.zh, cur.zl);
+            const float t1 = 6.283185307179586f * kz_turns(make_float2(kt[i].z, kt[i].w), cur.zh, cur.zl);
+            sc[i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
+            if (cached) st_shared_v4f(sc0 + (uint32_t)(cur.kc * 4 + i) * 4096u, sc[i]);
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) sc[i] = ld_shared_v4f(sc0 + (uint32_t)(cur.kc * 4 + i) * 4096u);
         }
-        const float4 b0 = bb[2 * i], b1 = bb[2 * i + 1];
-        split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
-        split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
-        split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
-        split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
-      }
-      mbar_wait(&empty[st], ph ^ 1);
-      const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
+        K1PIter nxt = cur;
+        k1p_advance(nxt, P, G);
+        if (nxt.t < G.ntiles && (!cached || (nxt.c == 0 && nxt.g == 0))) k1p_load_kt(nxt, P, qyl, cgp, kt);   // one stage ahead
+        uint32_t hi[4][4], lo[4][4];                               // [slot][pair of q_x]
 #pragma unroll
-      for (int s = 0; s < 4; ++s) {
-        st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
-        st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
-      }
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
-      if (++st == K1P_NST) { st = 0; ph ^= 1; }
-      cur = nxt;
+        for (int i = 0; i < 4; ++i) {
+          const float4 b0 = bb[u][2 * i], b1 = bb[u][2 * i + 1];
+          const float cs0 = sc[i].x, sn0 = sc[i].y, cs1 = sc[i].z, sn1 = sc[i].w;
+          split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
+          split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
+          split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
+          split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
+        }
+        mbar_wait(&S.empty[st], ph ^ 1);
+        const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) kt[i] = ktn[i];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) bb[i] = bbn[i];
-    }
-  } else {
-    // ---------------- epilogue: TMEM -> scale -> fp16 hi / lo -> swizzled staging -> TMA store of T^T ----------------
-    const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
-    const int row = q * 32 + lane;
-    const int et = threadIdx.x - 32 * (2 + K1P_PRODUCER_WARPS);   // 0..127
-    const uint32_t stg0 = smem_u32(smem + K1P_NST * P_STAGE);
-    const uint32_t acc_empty_leader = mapa(smem_u32(&acc_empty[0]), 0);
-    const uint32_t rbase = (uint32_t)row * 128u;
-    int it = 0, sbuf = 0;
-    for (int t = cid; t < ntiles; t += ncl) {
-      const int mt = t % tiles_m;
-      int r = t / tiles_m;
-      const int jt = r % tiles_j;
-      const int zl = r / tiles_j;
-      for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
-        const int g = cg & 1, c = cg >> 1;
-        mbar_wait(&acc_full[g], (it >> 1) & 1);
-        tcgen05_fence_after();
-#pragma unroll 1
         for (int s = 0; s < 4; ++s) {
-          // the staging buffer used two slots ago has been read by its TMA store
-          if (et == 0) bulk_wait_read<1>();
-          named_bar_sync(2, 128);
-          const uint32_t sh = stg0 + sbuf * K1P_STAGING + rbase, sl = sh + TILE16K;
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {            // q_y half h was generated by CTA h: columns h*128 + s*32 + 0..31
-            uint32_t v[32];
-            tmem_ld_32x32b_x32(tmem + ((uint32_t)(q * 32) << 16) + g * 256 + h * 128 + s * 32, v);
-            tmem_ld_wait();
-            uint32_t ph[16], pl[16];
-#pragma unroll
-            for (int e = 0; e < 16; ++e)
-              split_f16x2(__uint_as_float(v[2 * e]) * P.f1, __uint_as_float(v[2 * e + 1]) * P.f1, ph[e], pl[e]);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {          // 16-byte chunk h*4 + j of the 128-byte row
-              const uint32_t o = (((uint32_t)(h * 4 + j) ^ ((uint32_t)row & 7u)) << 4);
-              st_shared_v4(sh + o, ph[4 * j], ph[4 * j + 1], ph[4 * j + 2], ph[4 * j + 3]);
-              st_shared_v4(sl + o, pl[4 * j], pl[4 * j + 1], pl[4 * j + 2], pl[4 * j + 3]);
-            }
-          }
-          fence_proxy_async_smem();
-          named_bar_sync(2, 128);
-          if (et == 0) {
-            const int j = (s >> 1) * 4 + g * 2 + (s & 1);          // chain index of slot s in group g
-            const int chain = (zl * P.C + c) * 8 + j;
-            const int mx0 = mt * 256 + (int)rank * 128;
-            tma_store_3d(&map_this, stg0 + sbuf * K1P_STAGING, jt * K1P_QY, mx0, chain);
-            tma_store_3d(&map_tlos, stg0 + sbuf * K1P_STAGING + TILE16K, jt * K1P_QY, mx0, chain);
-            bulk_commit();
-          }
-          sbuf ^= 1;
+          st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
+          st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
         }
-        tcgen05_fence_before();
+        fence_proxy_async_smem();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + g * 8);
+        if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
+        if (++st == K1P_NST) { st = 0; ph ^= 1; }
+        cur = nxt;
       }
     }
-    if (et == 0) bulk_wait_all();
+  }
+}
+
+// Four epilogue warps: TMEM -> scale -> fp16 hi / lo -> swizzled staging tiles -> TMA store of T^T[chain][mx][qy].
+// The hi tile and the lo tile are separate 16 KB buffers, each stored by its own bulk group, so writing one overlaps the
+// TMA read of the other.
+__device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_this, const CUtensorMap &map_tlos,
+                                             const K1PArgs &P, const K1PGeom &G, int warp, int lane, uint32_t rank) {
+  const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
+  const int row = q * 32 + lane;
+  const int et = threadIdx.x - 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS);   // 0..127
+  const uint32_t stg_hi = smem_u32(smem + K1P_NST * P_STAGE) + (uint32_t)row * 128u, stg_lo = stg_hi + TILE16K;
+  const uint32_t stg0 = smem_u32(smem + K1P_NST * P_STAGE);
+  const uint32_t acc_empty_leader = mapa(smem_u32(&S.acc_empty[0]), 0);
+  const uint32_t swz = (uint32_t)row & 7u;
+  int it = 0;
+  for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+    const int mt = t % G.tiles_m;
+    const int r = t / G.tiles_m;
+    const int jt = r % G.tiles_j;
+    const int zl = r / G.tiles_j;
+    const int mx0 = mt * 256 + (int)rank * 128;
+    for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
+      const int g = cg & 1, c = cg >> 1;
+      mbar_wait(&S.acc_full[g], (it >> 1) & 1);
+      tcgen05_fence_after();
+#pragma unroll 1
+      for (int s = 0; s < 4; ++s) {
+        const int chain = (zl * P.C + c) * 8 + (s >> 1) * 4 + g * 2 + (s & 1);     // chain index of slot s in group g
+        uint32_t pl[2][16];
+        // the hi buffer was handed to the TMA store two bulk groups ago (hi, lo of the previous slot)
+        if (et == 0) bulk_wait_read<1>();
+        named_bar_sync(2, 128);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {            // q_y half h was generated by CTA h: columns h*128 + s*32 + 0..31
+          uint32_t v[32], ph[16];
+          tmem_ld_32x32b_x32(tmem + ((uint32_t)(q * 32) << 16) + g * 256 + h * 128 + s * 32, v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int e = 0; e < 16; ++e)
+            split_f16x2(__uint_as_float(v[2 * e]) * P.f1, __uint_as_float(v[2 * e + 1]) * P.f1, ph[e], pl[h][e]);
+#pragma unroll
+          for (int j = 0; j < 4; ++j)            // 16-byte chunk h*4 + j of the 128-byte row
+            st_shared_v4(stg_hi + ((((uint32_t)(h * 4 + j)) ^ swz) << 4), ph[4 * j], ph[4 * j + 1], ph[4 * j + 2], ph[4 * j + 3]);
+        }
+        if (s == 3) {                            // every TMEM read of this item is done: release the accumulator
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(acc_empty_leader + g * 8);
+        }
+        fence_proxy_async_smem();
+        named_bar_sync(2, 128);
+        if (et == 0) {
+          tma_store_3d(&map_this, stg0, jt * K1P_QY, mx0, chain);
+          bulk_commit();
+          bulk_wait_read<1>();                   // the lo buffer of the previous slot has been read
+        }
+        named_bar_sync(2, 128);
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            st_shared_v4(stg_lo + ((((uint32_t)(h * 4 + j)) ^ swz) << 4), pl[h][4 * j], pl[h][4 * j + 1], pl[h][4 * j + 2], pl[h][4 * j + 3]);
+        fence_proxy_async_smem();
+        named_bar_sync(2, 128);
+        if (et == 0) {
+          tma_store_3d(&map_tlos, stg0 + TILE16K, jt * K1P_QY, mx0, chain);
+          bulk_commit();
+        }
+      }
+    }
+  }
+  if (et == 0) bulk_wait_all();
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K1P_THREADS, 1)
+k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
+        const __grid_constant__ CUtensorMap map_this, const __grid_constant__ CUtensorMap map_tlos, const K1PArgs P) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ K1PShared S;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < K1P_NST; ++i) { mbar_init(&S.full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&S.empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo); prefetch_tmap(&map_this); prefetch_tmap(&map_tlos); }
+  if (warp == 1) tmem_alloc2(&S.tmem_slot, 512);
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tcgen05_fence_after();
+  const uint32_t tmem = S.tmem_slot;
+
+  K1PGeom G;
+  G.nk = P.n_pad / 64;
+  G.tiles_j = P.n_pad / K1P_QY;
+  G.tiles_m = P.m_pad / 256;
+  G.ntiles = P.zc * G.tiles_j * G.tiles_m;                        // a tile = (plane, jt, mx pair-tile); c and g loop inside
+  G.ncl = gridDim.x >> 1;
+  G.cid = blockIdx.x >> 1;
+
+  // register budget (launch: 512 x 128; setmaxnreg acts on whole warpgroups): feeders 24, producers 184, epilogue 104
+  if (warp < K1P_FEED_WARPS) {
+    setmaxnreg_dec<24>();
+    k1p_feed(smem, S, tmem, map_xhi, map_xlo, P, G, warp, rank);
+  } else if (warp < K1P_FEED_WARPS + K1P_PRODUCER_WARPS) {
+    setmaxnreg_inc<184>();
+    k1p_produce(smem, S, P, G, lane, rank);
+  } else {
+    setmaxnreg_dec<104>();
+    k1p_epilogue(smem, S, tmem, map_this, map_tlos, P, G, warp, lane, rank);
   }
   tcgen05_fence_before();
   __syncthreads();
