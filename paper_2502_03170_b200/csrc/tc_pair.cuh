@@ -190,12 +190,12 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
       int st = 0, ph = 0, item = 0;
       for (int t = cid; t < ntiles; t += ncl) {
         for (int c = 0; c < P.C; ++c, ++item) {
-          mbar_wait_cluster(&acc_empty, (item & 1) ^ 1);
+          mbar_wait(&acc_empty, (item & 1) ^ 1);
           tcgen05_fence_after();
           for (int a = 0; a < 2; ++a) {
             const uint32_t d = tmem + a * 256;
             for (int kc = 0; kc < nk; ++kc) {
-              mbar_wait_cluster(&full[st], ph);
+              mbar_wait(&full[st], ph);
               tcgen05_fence_after();
               issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
               umma2_commit(&empty[st]);
@@ -341,8 +341,8 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
 
 // ---- stage 1 ----------------------------------------------------------------------------------------------------------
 struct K1PArgs {
-  const float4 *bgrp;   // [2][C][n_pad][n_pad]  pre-scaled by s_Q
-  const float2 *ktp;    // [n_pad][n_pad]
+  const float4 *bgp;    // [2][C][jt][kc][half][8 samples][256 threads]  base pupil (4 slots), pre-scaled by s_Q
+  const float4 *ktq;    // [jt][kc][half][4 sample pairs][256 threads]      kappa / 2 pi (hi, lo) of two samples
   const float4 *planes; // [Z]
   int C, n_pad, m_pad, z0, zc;
   float f1;             // epilogue factor s_T / (s_Q s_X)
@@ -360,6 +360,7 @@ constexpr int K1P_QY = 64;                                        // q_y per til
 
 struct K1PShared {
   uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
+  uint64_t written[K1P_NST];    // producer warps -> fence warp: the B-operand rows of the stage are in shared memory
   uint32_t tmem_slot;
 };
 struct K1PGeom { int nk, tiles_j, tiles_m, ntiles, ncl, cid; };
@@ -387,19 +388,19 @@ __device__ __forceinline__ void k1p_advance(K1PIter &it, const K1PArgs &P, const
   it.t += G.ncl;
   k1p_decode(it, P, G);
 }
-// sample index of this thread's first q_x of item `it`
-__device__ __forceinline__ size_t k1p_sample(const K1PIter &it, const K1PArgs &P, int qyl, int cg) {
-  return (size_t)(it.jt * K1P_QY + qyl) * P.n_pad + it.kc * 64 + cg * 8;
+// block of item `it` in the producer-ordered tables (2048 samples per block); `th` = producer thread, `half` = CTA rank
+__device__ __forceinline__ size_t k1p_block(const K1PIter &it, const K1PGeom &G, int half) {
+  return ((size_t)(it.jt * G.nk + it.kc) * 2 + half) * 2048;
 }
-__device__ __forceinline__ void k1p_load_bb(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&bb)[8]) {
-  const float4 *b4 = P.bgrp + ((size_t)(it.g * P.C + it.c) * P.n_pad) * P.n_pad + k1p_sample(it, P, qyl, cg);
+__device__ __forceinline__ void k1p_load_bb(const K1PIter &it, const K1PArgs &P, const K1PGeom &G, int half, int th, float4 (&bb)[8]) {
+  const float4 *b4 = P.bgp + (size_t)(it.g * P.C + it.c) * P.n_pad * P.n_pad + k1p_block(it, G, half) + th;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) bb[i] = __ldg(b4 + i);
+  for (int i = 0; i < 8; ++i) bb[i] = __ldg(b4 + i * 256);
 }
-__device__ __forceinline__ void k1p_load_kt(const K1PIter &it, const K1PArgs &P, int qyl, int cg, float4 (&kt)[4]) {
-  const float4 *k4 = reinterpret_cast<const float4 *>(P.ktp + k1p_sample(it, P, qyl, cg));
+__device__ __forceinline__ void k1p_load_kt(const K1PIter &it, const K1PArgs &P, const K1PGeom &G, int half, int th, float4 (&kt)[4]) {
+  const float4 *k4 = P.ktq + k1p_block(it, G, half) / 2 + th;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i);
+  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i * 256);
 }
 __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
   float4 v;
@@ -440,17 +441,33 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
           const int g = cg & 1;
-          mbar_wait_cluster(&S.acc_empty[g], ((it >> 1) & 1) ^ 1);
+          mbar_wait(&S.acc_empty[g], ((it >> 1) & 1) ^ 1);
           tcgen05_fence_after();
           const uint32_t d = tmem + g * 256;
           for (int kc = 0; kc < G.nk; ++kc) {
-            mbar_wait_cluster(&S.full[st], ph);
+            mbar_wait(&S.full[st], ph);
             tcgen05_fence_after();
             issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
             umma2_commit(&S.empty[st]);
             if (++st == K1P_NST) { st = 0; ph ^= 1; }
           }
           umma2_commit(&S.acc_full[g]);
+        }
+      }
+    }
+  } else if (warp == 2) {
+    // Fence warp.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding load of the
+    // issuing thread: issued by the producers it would drain their base-pupil prefetch at every stage.  They hand the
+    // stage over through `written` instead, and this thread (no loads in flight) fences and arrives at the leader.
+    if (elect_one()) {
+      int st = 0, ph = 0;
+      const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
+      for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+        for (int i = 0; i < 2 * P.C * G.nk; ++i) {
+          mbar_wait(&S.written[st], ph);
+          fence_proxy_async_smem();
+          mbar_arrive_cluster(full_leader0 + st * 8);
+          if (++st == K1P_NST) { st = 0; ph ^= 1; }
         }
       }
     }
@@ -463,10 +480,8 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
 __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
   const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
   const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
-  const int qyl = (int)rank * 32 + ql;                           // q_y within the tile
   // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
   const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
-  const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
   const uint32_t smem0 = smem_u32(smem);
   const uint32_t sc0 = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // cache: [(kc*4 + j)][thread] float4
   const bool cached = G.nk <= K1P_SC_KC;
@@ -477,13 +492,13 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
   float4 bb[3][8], kt[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) kt[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (cur.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[0]); k1p_load_kt(cur, P, qyl, cgp, kt); k1p_advance(pre, P, G); }
-  if (pre.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[1]); k1p_advance(pre, P, G); }
+  if (cur.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[0]); k1p_load_kt(cur, P, G, (int)rank, tid, kt); k1p_advance(pre, P, G); }
+  if (pre.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[1]); k1p_advance(pre, P, G); }
   while (cur.t < G.ntiles) {
 #pragma unroll
     for (int u = 0; u < 3; ++u) {
       if (cur.t < G.ntiles) {
-        if (pre.t < G.ntiles) { k1p_load_bb(pre, P, qyl, cgp, bb[(u + 2) % 3]); k1p_advance(pre, P, G); }
+        if (pre.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[(u + 2) % 3]); k1p_advance(pre, P, G); }
         // (cos, sin) of the 8 samples
         float4 sc[4];
         const bool first = !cached || (cur.c == 0 && cur.g == 0);
@@ -501,7 +516,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
         }
         K1PIter nxt = cur;
         k1p_advance(nxt, P, G);
-        if (nxt.t < G.ntiles && (!cached || (nxt.c == 0 && nxt.g == 0))) k1p_load_kt(nxt, P, qyl, cgp, kt);   // one stage ahead
+        if (nxt.t < G.ntiles && (!cached || (nxt.c == 0 && nxt.g == 0))) k1p_load_kt(nxt, P, G, (int)rank, tid, kt);   // one stage ahead
         uint32_t hi[4][4], lo[4][4];                               // [slot][pair of q_x]
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -519,9 +534,8 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
           st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
         }
-        fence_proxy_async_smem();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
+        if (lane == 0) mbar_arrive(&S.written[st]);
         if (++st == K1P_NST) { st = 0; ph ^= 1; }
         cur = nxt;
       }
@@ -611,7 +625,11 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
   const uint32_t rank = cluster_ctarank();
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < K1P_NST; ++i) { mbar_init(&S.full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&S.empty[i], 1); }
+    for (int i = 0; i < K1P_NST; ++i) {
+      mbar_init(&S.full[i], 1 + 2);                       // the leader's expect_tx arrive + the fence warp of each CTA
+      mbar_init(&S.empty[i], 1);
+      mbar_init(&S.written[i], K1P_PRODUCER_WARPS);
+    }
     for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
     fence_barrier_init();
   }
