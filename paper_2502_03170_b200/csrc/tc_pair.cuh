@@ -476,7 +476,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
 
 // Eight producer warps: this CTA's 32 q_y x 4 slots = 128 B-operand rows per stage.  The defocus phasor of a sample is the
 // same for all 2 C (component, group) items of a tile: it is computed at the first item and parked in a per-thread
-// shared-memory cache; the base-pupil loads run two stages ahead of their use.
+// shared-memory cache; the base-pupil loads run one stage ahead of their use.
 __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
   const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
   const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
@@ -488,17 +488,17 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
   int st = 0, ph = 0;
   K1PIter cur{G.cid, 0, 0, 0, 0, 0.f, 0.f};
   k1p_decode(cur, P, G);
-  K1PIter pre = cur;                                             // item whose base-pupil loads are issued next
-  float4 bb[3][8], kt[4];
+  // ptxas tracks every global load of this loop with one scoreboard, so a wait for any of them waits for all that are in
+  // flight: the loads of the next stage are therefore issued right after the first use of this stage's values (not
+  // before), which gives them the rest of the iteration plus the wait for a free stage to land.
+  float4 bb[2][8], kt[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) kt[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (cur.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[0]); k1p_load_kt(cur, P, G, (int)rank, tid, kt); k1p_advance(pre, P, G); }
-  if (pre.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[1]); k1p_advance(pre, P, G); }
+  if (cur.t < G.ntiles) { k1p_load_bb(cur, P, G, (int)rank, tid, bb[0]); k1p_load_kt(cur, P, G, (int)rank, tid, kt); }
   while (cur.t < G.ntiles) {
 #pragma unroll
-    for (int u = 0; u < 3; ++u) {
+    for (int u = 0; u < 2; ++u) {
       if (cur.t < G.ntiles) {
-        if (pre.t < G.ntiles) { k1p_load_bb(pre, P, G, (int)rank, tid, bb[(u + 2) % 3]); k1p_advance(pre, P, G); }
         // (cos, sin) of the 8 samples
         float4 sc[4];
         const bool first = !cached || (cur.c == 0 && cur.g == 0);
@@ -514,9 +514,6 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
 #pragma unroll
           for (int i = 0; i < 4; ++i) sc[i] = ld_shared_v4f(sc0 + (uint32_t)(cur.kc * 4 + i) * 4096u);
         }
-        K1PIter nxt = cur;
-        k1p_advance(nxt, P, G);
-        if (nxt.t < G.ntiles && (!cached || (nxt.c == 0 && nxt.g == 0))) k1p_load_kt(nxt, P, G, (int)rank, tid, kt);   // one stage ahead
         uint32_t hi[4][4], lo[4][4];                               // [slot][pair of q_x]
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -526,6 +523,13 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
           split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
           split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
+        }
+        asm volatile("" ::: "memory");                             // keep the next stage's loads below this point
+        K1PIter nxt = cur;
+        k1p_advance(nxt, P, G);
+        if (nxt.t < G.ntiles) {
+          k1p_load_bb(nxt, P, G, (int)rank, tid, bb[u ^ 1]);
+          if (!cached || (nxt.c == 0 && nxt.g == 0)) k1p_load_kt(nxt, P, G, (int)rank, tid, kt);
         }
         mbar_wait(&S.empty[st], ph ^ 1);
         const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
