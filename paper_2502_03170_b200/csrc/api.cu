@@ -61,6 +61,7 @@ psf_status upload_static(psf_plan *p) {
   std::vector<float4> bfold((size_t)C * nn * 2);
   std::vector<float2> kt(nn);
   const double twopi = 6.283185307179586476925287;
+#pragma omp parallel for schedule(static)
   for (int qy = 0; qy < n; ++qy) {
     for (int qx = 0; qx < n; ++qx) {
       const int ry = N - 1 - qy, rx = N - 1 - qx;

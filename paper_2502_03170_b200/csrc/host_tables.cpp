@@ -186,7 +186,8 @@ void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const
   const size_t NN = (size_t)P0.N * P0.N;
   base = P0.base;
   if (!coeffs || K <= 0) return;
-  for (size_t i = 0; i < NN; ++i) {
+#pragma omp parallel for schedule(static)
+  for (long long i = 0; i < (long long)NN; ++i) {
     if (!P0.mask[i]) continue;
     double W = 0.0;
     for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];

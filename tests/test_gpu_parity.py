@@ -137,6 +137,20 @@ def test_shared_zernike_static_path_odd_sizes(psf, precision):
         assert plane_errors(I, ref).max() <= TOL, (path, seed)
 
 
+@pytest.mark.parametrize("seed,N,M,Z,pol", [(51, 300, 400, 3, W.POL_UNPOLARIZED),     # n = 150 (pad 192), m = 200 (pad 256)
+                                            (52, 130, 511, 2, W.POL_CIRC_L),          # odd M: self-mirror row and column
+                                            (53, 512, 258, 5, W.POL_X),               # m = 129 (pad 256): a nearly empty CTA
+                                            (54, 257, 1023, 1, W.POL_UNPOLARIZED)])   # m = 512: two pair tiles per plane
+def test_cta_pair_kernels_ragged_sizes(psf, seed, N, M, Z, pol):
+    """The cta_group::2 kernels (3xFP16 path, output half-size padded to whole pairs of 128 rows) on sizes that leave
+    padding in every tile dimension, against the separable fp64 oracle, every voxel."""
+    case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, per_plane=False, shifts=False, pol=pol)
+    I, path = gpu_stack(psf, case, "3xf16")
+    assert path == "tc3xf16"
+    ref = O.stack_T2(case)
+    assert plane_errors(I, ref).max() <= TOL, (path, seed)
+
+
 @pytest.mark.parametrize("precision", PRECISIONS)
 def test_field_output_matches_oracle_field(psf, precision):
     case = replace(W.config2(), z_um=np.linspace(-2.0, 2.0, 5), pupil_n=96, out_m=50)
