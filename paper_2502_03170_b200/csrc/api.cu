@@ -50,7 +50,8 @@ psf_status upload_static(psf_plan *p) {
     p->zb_first = p->noll_first;
     p->zb_K = Kneed;
   }
-  std::vector<cplx> base_z;
+  PhaseTimer tm;
+  std::vector<cplx> &base_z = p->h_base;
   apply_shared_zernike(hp, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis, base_z);
   const int N = d.pupil_n, n = (N + 1) / 2, C = hp.C;
   const size_t NN = (size_t)N * N, nn = (size_t)n * n;
@@ -58,8 +59,11 @@ psf_status upload_static(psf_plan *p) {
   P.C = C;
   for (int c = 0; c < 5; ++c) P.weight[c] = (float)hp.weight[c];
 
-  std::vector<float4> bfold((size_t)C * nn * 2);
-  std::vector<float2> kt(nn);
+  tm.mark("apply_shared_zernike");
+  std::vector<float4> &bfold = p->h_bfold;
+  std::vector<float2> &kt = p->h_kt;
+  bfold.resize((size_t)C * nn * 2);
+  kt.resize(nn);
   const double twopi = 6.283185307179586476925287;
 #pragma omp parallel for schedule(static)
   for (int qy = 0; qy < n; ++qy) {
@@ -85,9 +89,11 @@ psf_status upload_static(psf_plan *p) {
       }
     }
   }
+  tm.mark("fold");
   psf_status s;
   if ((s = upload(p, &p->d_bfold, &p->cap_bfold, bfold)) != PSF_OK) return s;
   if ((s = upload(p, &p->d_kt, &p->cap_kt, kt)) != PSF_OK) return s;
+  tm.mark("upload bfold, kt");
   P.bfold = (const float4 *)p->d_bfold;
   P.kt = (const float2 *)p->d_kt;
 
@@ -149,7 +155,9 @@ psf_status upload_static(psf_plan *p) {
   const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || prec == PSF_PREC_3XF16 || tc_eligible(p));
   p->path = want_tc ? (prec == PSF_PREC_3XTF32 ? 1 : 2) : 0;     // AUTO: the fp16 split (same accuracy, about twice as fast)
   if (!want_tc && small_eligible(p)) p->path = 3;                // whole path fused in one CTA per plane
+  tm.mark("planes, path");
   if (want_tc && (s = tc_setup(p, bfold, kt, p->phi, p->path == 2)) != PSF_OK) return s;
+  tm.mark("tc_setup");
   return PSF_OK;
 }
 

@@ -184,15 +184,20 @@ void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<
 void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
                           std::vector<cplx> &base) {
   const size_t NN = (size_t)P0.N * P0.N;
-  base = P0.base;
-  if (!coeffs || K <= 0) return;
+  base.resize(P0.base.size());
+  const bool zern = coeffs && K > 0;
 #pragma omp parallel for schedule(static)
   for (long long i = 0; i < (long long)NN; ++i) {
-    if (!P0.mask[i]) continue;
-    double W = 0.0;
-    for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];
-    const cplx e(std::cos(W), std::sin(W));
-    for (int c = 0; c < P0.C; ++c) base[(size_t)c * NN + i] *= e;
+    cplx e(1.0, 0.0);
+    if (zern && P0.mask[i]) {
+      double W = 0.0;
+      for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];
+      e = cplx(std::cos(W), std::sin(W));
+    }
+    for (int c = 0; c < P0.C; ++c) {
+      const cplx b = P0.base[(size_t)c * NN + i];
+      base[(size_t)c * NN + i] = cplx(b.real() * e.real() - b.imag() * e.imag(), b.real() * e.imag() + b.imag() * e.real());
+    }
   }
 }
 

@@ -2,6 +2,10 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cstdio>
+#include <cstdlib>
+#include <ctime>
+
 #include <string>
 #include <vector>
 
@@ -54,6 +58,9 @@ struct psf_plan {
   // host caches: static pupil without any Zernike term, and the Zernike basis of the last (noll_first, K)
   psf::HostPupil hp0;
   std::vector<double> zbasis;    // [K][N][N]
+  std::vector<psf::cplx> h_base; // static pupil times the shared Zernike phase (kept across refreshes)
+  std::vector<float4> h_bfold;
+  std::vector<float2> h_kt;
   int zb_first = 0, zb_K = 0;
   long long upload_bytes = 0;
   // profiling (psf_profile_enable)
@@ -73,6 +80,13 @@ struct psf_plan {
 };
 
 namespace psf {
+// PSF_TIMING=1: wall-clock phases of the host table refresh on stderr (development aid)
+struct PhaseTimer {
+  bool on; double t0;
+  static double now() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; }
+  PhaseTimer() : on(getenv("PSF_TIMING") != nullptr), t0(on ? now() : 0.0) {}
+  void mark(const char *what) { if (!on) return; const double t = now(); fprintf(stderr, "[psf timing] %-28s %8.3f ms\n", what, t - t0); t0 = t; }
+};
 // Marks the end of one kernel launch of `stage` for the profiler (no-op unless psf_profile_enable is on).
 inline void prof_mark(const psf_plan *p, cudaStream_t st, int stage) {
   psf_plan *q = const_cast<psf_plan *>(p);
