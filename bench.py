@@ -33,10 +33,10 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 # (profiles/*.md name the command); keyed by (path, workload, stage), in bytes PER PLANE of the captured launch (scaled to
 # the mean planes per launch below).  None where no capture exists yet.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1c_ncu_tc_cfg5.md: k2_tc<f16>, 146-plane launch: 1.676 GB read + 0.208 GB written
-    ("tc3xf16", "cfg5_large_stack", 1): (1.675852e9 + 0.208072e9) / 146,
-    # same capture, k1_tc<f16>: 0.018 GB read + 1.551 GB written
-    ("tc3xf16", "cfg5_large_stack", 0): (0.018017e9 + 1.551206e9) / 146,
+    # profiles/r1g_ncu_pair_cfg5.md: k2_pair, 256-plane launch: 2.705 GB read + 0.259 GB written
+    ("tc3xf16", "cfg5_large_stack", 1): (2.705373e9 + 0.259306e9) / 256,
+    # same capture, k1_pair: 0.155 GB read + 2.624 GB written
+    ("tc3xf16", "cfg5_large_stack", 0): (0.154841e9 + 2.624252e9) / 256,
 }
 
 
@@ -189,7 +189,7 @@ def blas_threads():
     return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
 
 
-ORACLE_PLANES = {1: 16, 2: 64, 3: 128, 4: 4096, 5: 128}    # about 10-30 s of CPU work each on the 16-core B200 host
+ORACLE_PLANES = {1: 16, 2: 64, 3: 128, 4: 4096, 5: 256}    # about 10-30 s of CPU work each on the 16-core B200 host
 
 
 def run_oracle_once(case, planes):
@@ -320,6 +320,8 @@ def run_ours(args):
                 "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
                 "algorithmic_tflops": flop_dom / launches_dom / (dur_ms * 1e-3) / 1e12, "peak_source": peak_note,
                 "stage_ms_per_step": [float(stage_ms[0]), float(stage_ms[1])]}
+    if bound == "tensor":      # both stages together against the same peak (context: the two kernels take about equal time)
+        roofline["step_frac"] = 3.0 * (f1 + f2) / (ms_per_step * 1e-3) / 1e12 / peak
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
