@@ -350,65 +350,33 @@ struct K1PArgs {
 
 constexpr int K1P_NST = 2;
 constexpr int K1P_PRODUCER_WARPS = 8;
-constexpr int K1P_FEED_WARPS = 4;                                  // TMA, MMA, two idle: roles fill whole warpgroups (setmaxnreg)
+constexpr int K1P_FEED_WARPS = 4;                                  // table TMA, MMA, fence, base-pupil copies: roles fill whole warpgroups (setmaxnreg)
 constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
 constexpr int K1P_STAGING = 2 * TILE16K;                          // hi tile + lo tile of one chain: 128 mx x 64 qy each
-constexpr int K1P_SC_KC = 4;                                      // k-chunks covered by the sin / cos cache (n_pad <= 256)
-constexpr int K1P_SINCOS = K1P_SC_KC * 4 * 256 * 16;              // 64 KB: 8 (cos, sin) pairs per producer thread and k-chunk
-constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + K1P_STAGING + K1P_SINCOS;
+constexpr int K1P_BB_SLOTS = 2;
+constexpr int K1P_BB_BYTES = 8 * 256 * 16;                        // one stage of base pupil for this CTA: 8 samples x 256 threads x float4
+constexpr int K1P_MAX_NK = 4;                                     // the producers keep the defocus phasors of a tile in registers: n_pad <= 256
+constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + K1P_STAGING + K1P_BB_SLOTS * K1P_BB_BYTES;
 constexpr int K1P_QY = 64;                                        // q_y per tile (32 generated by each CTA)
 
 struct K1PShared {
   uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
   uint64_t written[K1P_NST];    // producer warps -> fence warp: the B-operand rows of the stage are in shared memory
+  uint64_t bb_full[K1P_BB_SLOTS], bb_empty[K1P_BB_SLOTS];   // base-pupil ring: bulk copy -> producers -> free
   uint32_t tmem_slot;
 };
 struct K1PGeom { int nk, tiles_j, tiles_m, ntiles, ncl, cid; };
 
-// Producer work item: one pipeline stage of one (plane, jt, c, g): this thread's 8 consecutive q_x of one q_y row.
-struct K1PIter {
-  int t, c, g, kc;      // tile, component, x-parity group, k-chunk
-  int jt;               // decoded tile
-  float zh, zl;
-};
-__device__ __forceinline__ void k1p_decode(K1PIter &it, const K1PArgs &P, const K1PGeom &G) {
-  if (it.t >= G.ntiles) return;
-  const int r = it.t / G.tiles_m;
-  it.jt = r % G.tiles_j;
-  const float4 pl = __ldg(P.planes + P.z0 + r / G.tiles_j);
-  it.zh = pl.x; it.zl = pl.y;
-}
-__device__ __forceinline__ void k1p_advance(K1PIter &it, const K1PArgs &P, const K1PGeom &G) {
-  if (++it.kc < G.nk) return;
-  it.kc = 0;
-  if (++it.g < 2) return;
-  it.g = 0;
-  if (++it.c < P.C) return;
-  it.c = 0;
-  it.t += G.ncl;
-  k1p_decode(it, P, G);
-}
-// block of item `it` in the producer-ordered tables (2048 samples per block); `th` = producer thread, `half` = CTA rank
-__device__ __forceinline__ size_t k1p_block(const K1PIter &it, const K1PGeom &G, int half) {
-  return ((size_t)(it.jt * G.nk + it.kc) * 2 + half) * 2048;
-}
-__device__ __forceinline__ void k1p_load_bb(const K1PIter &it, const K1PArgs &P, const K1PGeom &G, int half, int th, float4 (&bb)[8]) {
-  const float4 *b4 = P.bgp + (size_t)(it.g * P.C + it.c) * P.n_pad * P.n_pad + k1p_block(it, G, half) + th;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) bb[i] = __ldg(b4 + i * 256);
-}
-__device__ __forceinline__ void k1p_load_kt(const K1PIter &it, const K1PArgs &P, const K1PGeom &G, int half, int th, float4 (&kt)[4]) {
-  const float4 *k4 = P.ktq + k1p_block(it, G, half) / 2 + th;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i * 256);
+// 1-D bulk copy global -> shared of this CTA, completion bytes on a local mbarrier
+__device__ __forceinline__ void bulk_load_1d(uint32_t smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_dst), "l"((uint64_t)gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
 }
 __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
   float4 v;
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
   return v;
-}
-__device__ __forceinline__ void st_shared_v4f(uint32_t saddr, float4 v) {
-  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
 // TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
@@ -471,77 +439,94 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         }
       }
     }
+  } else if (warp == 3) {
+    // Base-pupil copies: one 32 KB bulk copy per stage (the table is stored in the producers' read order, so a stage
+    // of this CTA is one contiguous block) into a two-slot ring.  The producers then only read shared memory: no
+    // global-load latency in their loop.
+    if (elect_one()) {
+      int bs = 0, bph = 0;
+      const uint32_t ring = smem_u32(smem + K1P_NST * P_STAGE + K1P_STAGING);
+      for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+        const int jt = (t / G.tiles_m) % G.tiles_j;
+        for (int cg = 0; cg < 2 * P.C; ++cg) {
+          const float4 *src = P.bgp + (size_t)((cg & 1) * P.C + (cg >> 1)) * P.n_pad * P.n_pad;
+          for (int kc = 0; kc < G.nk; ++kc) {
+            mbar_wait(&S.bb_empty[bs], bph ^ 1);
+            mbar_arrive_expect_tx(&S.bb_full[bs], K1P_BB_BYTES);
+            bulk_load_1d(ring + bs * K1P_BB_BYTES, src + ((size_t)(jt * G.nk + kc) * 2 + rank) * 2048, K1P_BB_BYTES, &S.bb_full[bs]);
+            if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
+          }
+        }
+      }
+    }
   }
 }
 
-// Eight producer warps: this CTA's 32 q_y x 4 slots = 128 B-operand rows per stage.  The defocus phasor of a sample is the
-// same for all 2 C (component, group) items of a tile: it is computed at the first item and parked in a per-thread
-// shared-memory cache; the base-pupil loads run one stage ahead of their use.
+// Eight producer warps: this CTA's 32 q_y x 4 slots = 128 B-operand rows per stage; a thread owns 8 consecutive q_x of one
+// q_y row.  The defocus phasor of a sample is the same for all 2 C (component, group) items of a tile: the thread
+// computes its 8 x nk phasors at the first item and keeps them in registers (the k-chunk loop is unrolled).  The base
+// pupil of the stage comes from the shared-memory ring filled by the copy warp.
 __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
   const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
   const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
   // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
   const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
   const uint32_t smem0 = smem_u32(smem);
-  const uint32_t sc0 = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // cache: [(kc*4 + j)][thread] float4
-  const bool cached = G.nk <= K1P_SC_KC;
-  int st = 0, ph = 0;
-  K1PIter cur{G.cid, 0, 0, 0, 0, 0.f, 0.f};
-  k1p_decode(cur, P, G);
-  // ptxas tracks every global load of this loop with one scoreboard, so a wait for any of them waits for all that are in
-  // flight: the loads of the next stage are therefore issued right after the first use of this stage's values (not
-  // before), which gives them the rest of the iteration plus the wait for a free stage to land.
-  float4 bb[2][8], kt[4];
+  const uint32_t ring = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // [slot][sample e][thread] float4
+  int st = 0, ph = 0, bs = 0, bph = 0;
+  float4 sc[K1P_MAX_NK][4];                                      // (cos, sin) of samples (2i, 2i+1) of k-chunk kc
+  float4 kt[4];
+  // kappa of (tile, kc): [jt][kc][half][4 sample pairs][256 threads] float4
+  auto load_kt = [&](int jt, int kc) {
+    const float4 *k4 = P.ktq + ((size_t)(jt * G.nk + kc) * 2 + rank) * 1024 + tid;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) kt[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (cur.t < G.ntiles) { k1p_load_bb(cur, P, G, (int)rank, tid, bb[0]); k1p_load_kt(cur, P, G, (int)rank, tid, kt); }
-  while (cur.t < G.ntiles) {
+    for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i * 256);
+  };
+  if (G.cid < G.ntiles) load_kt((G.cid / G.tiles_m) % G.tiles_j, 0);
+  for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+    const int r = t / G.tiles_m;
+    const int jt = r % G.tiles_j;
+    const float4 pl = __ldg(P.planes + P.z0 + r / G.tiles_j);
+    for (int cg = 0; cg < 2 * P.C; ++cg) {
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      if (cur.t < G.ntiles) {
-        // (cos, sin) of the 8 samples
-        float4 sc[4];
-        const bool first = !cached || (cur.c == 0 && cur.g == 0);
-        if (first) {
+      for (int kc = 0; kc < K1P_MAX_NK; ++kc) {
+        if (kc < G.nk) {
+          if (cg == 0) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float t0 = 6.283185307179586f * kz_turns(make_float2(kt[i].x, kt[i].y), pl.x, pl.y);
+              const float t1 = 6.283185307179586f * kz_turns(make_float2(kt[i].z, kt[i].w), pl.x, pl.y);
+              sc[kc][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
+            }
+            if (kc + 1 < G.nk) load_kt(jt, kc + 1);              // one stage ahead
+          }
+          if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+          mbar_wait(&S.bb_full[bs], bph);
+          uint32_t hi[4][4], lo[4][4];                             // [slot][pair of q_x]
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const float t0 = 6.283185307179586f * kz_turns(make_float2(kt[i].x, kt[i].y), cur.zh, cur.zl);
-            const float t1 = 6.283185307179586f * kz_turns(make_float2(kt[i].z, kt[i].w), cur.zh, cur.zl);
-            sc[i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
-            if (cached) st_shared_v4f(sc0 + (uint32_t)(cur.kc * 4 + i) * 4096u, sc[i]);
+            const float4 b0 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i) * 4096);
+            const float4 b1 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i + 1) * 4096);
+            const float cs0 = sc[kc][i].x, sn0 = sc[kc][i].y, cs1 = sc[kc][i].z, sn1 = sc[kc][i].w;
+            split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
+            split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
+            split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
+            split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
           }
-        } else {
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&S.bb_empty[bs]);             // the ring slot is in registers
+          if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
+          mbar_wait(&S.empty[st], ph ^ 1);
+          const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
 #pragma unroll
-          for (int i = 0; i < 4; ++i) sc[i] = ld_shared_v4f(sc0 + (uint32_t)(cur.kc * 4 + i) * 4096u);
+          for (int s = 0; s < 4; ++s) {
+            st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
+            st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&S.written[st]);
+          if (++st == K1P_NST) { st = 0; ph ^= 1; }
         }
-        uint32_t hi[4][4], lo[4][4];                               // [slot][pair of q_x]
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const float4 b0 = bb[u][2 * i], b1 = bb[u][2 * i + 1];
-          const float cs0 = sc[i].x, sn0 = sc[i].y, cs1 = sc[i].z, sn1 = sc[i].w;
-          split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
-          split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
-          split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
-          split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
-        }
-        asm volatile("" ::: "memory");                             // keep the next stage's loads below this point
-        K1PIter nxt = cur;
-        k1p_advance(nxt, P, G);
-        if (nxt.t < G.ntiles) {
-          k1p_load_bb(nxt, P, G, (int)rank, tid, bb[u ^ 1]);
-          if (!cached || (nxt.c == 0 && nxt.g == 0)) k1p_load_kt(nxt, P, G, (int)rank, tid, kt);
-        }
-        mbar_wait(&S.empty[st], ph ^ 1);
-        const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
-#pragma unroll
-        for (int s = 0; s < 4; ++s) {
-          st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
-          st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&S.written[st]);
-        if (++st == K1P_NST) { st = 0; ph ^= 1; }
-        cur = nxt;
       }
     }
   }
@@ -634,6 +619,7 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
       mbar_init(&S.empty[i], 1);
       mbar_init(&S.written[i], K1P_PRODUCER_WARPS);
     }
+    for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S.bb_full[i], 1); mbar_init(&S.bb_empty[i], K1P_PRODUCER_WARPS); }
     for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
     fence_barrier_init();
   }
