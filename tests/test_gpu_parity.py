@@ -203,3 +203,26 @@ def test_replan_zernike_and_shift_updates(psf):
     torch.cuda.synchronize()
     assert plane_errors(c, O.stack_T2(replace(base, zernike=None))).max() <= TOL
     plan.destroy()
+
+
+def test_cta_pair_kernels_replan_chunked_and_single_plane(psf, monkeypatch):
+    """Pair kernels: new shared Zernike coefficients after creation (the producer-ordered tables are rebuilt), a scratch
+    budget that forces several launch pairs per stack (z-chunks of unequal size), and a one-plane stack."""
+    import torch
+    monkeypatch.setenv("PSF_TC_SCRATCH_MB", "24")                      # 5.2 MB of T^T (hi or lo) per plane -> 4-plane chunks
+    base = W.small_random_case(71, pupil_n=512, out_m=512, n_planes=6, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
+    plan = psf.plan_from_case(base, precision="3xf16")
+    assert plan.path == "tc3xf16" and plan.launches_per_compute == 4
+    a = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(a, O.stack_T2(base)).max() <= TOL
+    other = replace(base, zernike=(0.2 * np.random.default_rng(72).standard_normal(9)).astype(np.float32), noll_first=4)
+    plan.set_zernike(other.zernike, other.noll_first)
+    b = plan.compute().cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
+    assert plane_errors(b, O.stack_T2(other)).max() <= TOL
+    plan.destroy()
+    monkeypatch.delenv("PSF_TC_SCRATCH_MB")
+    one = replace(base, z_um=base.z_um[:1])
+    I, path = gpu_stack(psf, one, "auto")
+    assert path == "tc3xf16"
+    assert plane_errors(I, O.stack_T2(one)).max() <= TOL
