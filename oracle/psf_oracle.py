@@ -28,6 +28,13 @@ itself (closed forms, the Bessel form, the Airy pattern, exact discrete symmetri
 pure-Python brute force).  The combined non-axisymmetric aberrated result (configs 2, 4, 5) is
 "parity unpinned" beyond the component pins (Zernike basis, tilt, L<->R relations): see DESIGN.md.
 
+Further correction factors, each a factor of the static pupil: the scalar model
+`case.model = "scalar"` (Eq. 3, e_inf = e_inc = 1, one component), the Gaussian envelope
+`case.envelope_s` (Eq. 20, a factor of amp(theta)), and the free phase mask `case.phase_mask`
+(W_0 of PAPER.md:176 Eq. 18, radians on the pupil grid, added to W).  Pins: Dawson-function closed form of the
+on-axis focus amplitude and the Bessel form (envelope), exact zeros of vortex / half-moon masks, a mask equal
+to a Zernike term (phase mask), Airy / sinc closed forms (scalar).
+
 Readings of the paper taken where it is silent/garbled are those of SURVEY.md §8(c) (G1, A1-A10, Z)
 and are listed in DESIGN.md.
 """
@@ -163,10 +170,16 @@ def zernike_noll(j: int, rho, cosphi, sinphi):
 # Pupil samples: everything that multiplies the Fourier kernel, per in-disc sample
 # --------------------------------------------------------------------------------------------
 
+def _model(case, model):
+    """`model` argument of the public functions: None -> the case's own model."""
+    return getattr(case, "model", "vectorial") if model is None else model
+
+
 class Pupil:
     """Per in-disc sample tables (fp64) for one case: the factors of Eq. 9/15 that do not depend on (x,y,z)."""
 
-    def __init__(self, case, model="vectorial", paraxial=False, jones=None):
+    def __init__(self, case, model=None, paraxial=False, jones=None):
+        model = _model(case, model)
         N = case.pupil_n
         self.N = N
         self.k = 2.0 * math.pi * case.n_immersion / case.wavelength_um   # k = 2 pi n / lambda, n = n_i (A3a)
@@ -191,6 +204,8 @@ class Pupil:
         amp = (np.sqrt(self.costh) if case.apodize else 1.0) / self.costh
         if paraxial:
             amp = amp * self.costh      # the extra s_z = cos(theta) of PAPER.md:253 (Airy benchmark)
+        if getattr(case, "envelope_s", 0.0) > 0.0:
+            amp = amp * np.exp(-sin2 / case.envelope_s ** 2)      # Gaussian envelope, Eq. 20
         self.amp = amp
         # far field
         if model == "vectorial":
@@ -204,6 +219,8 @@ class Pupil:
         W = np.zeros(len(px), dtype=np.complex128)
         if case.gibson_lanni:
             W = W + gibson_lanni_phase(case, self.sinth)
+        if getattr(case, "phase_mask", None) is not None:          # W_0 of PAPER.md:176 Eq. 18, sampled on the pupil grid
+            W = W + np.asarray(case.phase_mask, dtype=np.float64)[py, px]
         self.W_static = W
         self.case = case
         self._zbasis = None
@@ -233,6 +250,7 @@ class Pupil:
 
 def _pupils(case, model, paraxial):
     """One Pupil per incoherent input (unpolarised = x and y inputs, each weighted 1/2; A8)."""
+    model = _model(case, model)
     if case.pol == "unpolarized" and model == "vectorial":
         return [(0.5, Pupil(case, model, paraxial, jones=(1.0 + 0j, 0j))),
                 (0.5, Pupil(case, model, paraxial, jones=(0j, 1.0 + 0j)))]
@@ -243,7 +261,7 @@ def _pupils(case, model, paraxial):
 # T1: literal sum
 # --------------------------------------------------------------------------------------------
 
-def field_at(case, plane, x_um, y_um, model="vectorial", paraxial=False, jones=None, chunk=2048):
+def field_at(case, plane, x_um, y_um, model=None, paraxial=False, jones=None, chunk=2048):
     """T1: E_c at arbitrary points (x, y) of plane(s) `plane` -- the literal double sum.
 
     plane, x_um, y_um broadcast to a common 1-D shape V.  Returns complex [C, V].
@@ -268,7 +286,7 @@ def field_at(case, plane, x_um, y_um, model="vectorial", paraxial=False, jones=N
 
 def intensity_at(case, plane, x_um, y_um, **kw):
     """T1 intensity sum_c |E_c|^2 at points; unpolarised = 1/2 (I_x + I_y)."""
-    model = kw.get("model", "vectorial")
+    model = _model(case, kw.get("model"))
     if case.pol == "unpolarized" and model == "vectorial":
         ix = np.sum(np.abs(field_at(case, plane, x_um, y_um, jones=(1.0 + 0j, 0j), **kw)) ** 2, axis=0)
         iy = np.sum(np.abs(field_at(case, plane, x_um, y_um, jones=(0j, 1.0 + 0j), **kw)) ** 2, axis=0)
@@ -298,7 +316,7 @@ def voxel_intensity(case, b, iy, ix, **kw):
 # T2: the same finite sum, summed over p_x then p_y (two matrix products per plane and component)
 # --------------------------------------------------------------------------------------------
 
-def field_T2(case, planes=None, model="vectorial", paraxial=False, jones=None):
+def field_T2(case, planes=None, model=None, paraxial=False, jones=None):
     """T2: E[c, b, m_y, m_x] for the given planes (complex128)."""
     pup = Pupil(case, model, paraxial, jones)
     N, M = case.pupil_n, case.out_m
@@ -317,8 +335,9 @@ def field_T2(case, planes=None, model="vectorial", paraxial=False, jones=None):
     return pup.prefactor * E
 
 
-def stack_T2(case, planes=None, model="vectorial", paraxial=False):
+def stack_T2(case, planes=None, model=None, paraxial=False):
     """T2 intensity stack [len(planes), M, M] (float64)."""
+    model = _model(case, model)
     if case.pol == "unpolarized" and model == "vectorial":
         ix = np.sum(np.abs(field_T2(case, planes, model, paraxial, jones=(1.0 + 0j, 0j))) ** 2, axis=0)
         iy = np.sum(np.abs(field_T2(case, planes, model, paraxial, jones=(0j, 1.0 + 0j))) ** 2, axis=0)
@@ -339,13 +358,14 @@ def _simpson_weights(n_nodes: int, h: float) -> np.ndarray:
     return w * h / 3.0
 
 
-def bessel_integrals(case, r_um, z_um: float, model="vectorial", paraxial=False, n_nodes=4001):
+def bessel_integrals(case, r_um, z_um: float, model=None, paraxial=False, n_nodes=4001):
     """I_0, I_1, I_2 of PAPER.md:131-137 Eq. 12-14 (without e_inc) at radii r_um (1-D) and one defocus z,
     by composite Simpson over theta in [0, theta_max].  Scalar model: the single integral of Eq. 5.
 
     Axisymmetric corrections enter as a(theta) exp(i W(theta)) (Eq. 15, 209).
     """
     from scipy.special import jv
+    model = _model(case, model)
     r_um = np.atleast_1d(np.asarray(r_um, dtype=np.float64))
     k = 2.0 * math.pi * case.n_immersion / case.wavelength_um
     th_max = math.asin(case.NA / case.n_immersion)
@@ -355,6 +375,8 @@ def bessel_integrals(case, r_um, z_um: float, model="vectorial", paraxial=False,
     a = (np.sqrt(ct) if case.apodize else np.ones_like(ct)).astype(np.complex128)
     if paraxial:
         a = a * ct
+    if getattr(case, "envelope_s", 0.0) > 0.0:
+        a = a * np.exp(-(st / case.envelope_s) ** 2)                       # PAPER.md:194 Eq. 20
     if case.gibson_lanni:
         a = a * np.exp(1j * gibson_lanni_phase(case, st))
     a = a * np.exp(1j * k * float(z_um) * ct)                              # exp(i k z cos(theta))
@@ -367,14 +389,15 @@ def bessel_integrals(case, r_um, z_um: float, model="vectorial", paraxial=False,
     return I0, I1, I2
 
 
-def bessel_field(case, r_um, varphi, z_um: float, model="vectorial", paraxial=False, jones=None, n_nodes=4001):
+def bessel_field(case, r_um, varphi, z_um: float, model=None, paraxial=False, jones=None, n_nodes=4001):
     """E at cylindrical points (r, varphi) of the plane at defocus z from the Bessel integrals (Eq. 5 / Eq. 11).
 
     Valid for axisymmetric pupils only (no Zernike, no shifts).  f = 1 (A1).
     r_um, varphi broadcast to a common 1-D shape V.  Returns complex [C, V].
     """
-    if case.zernike is not None or case.shifts_um is not None:
+    if case.zernike is not None or case.shifts_um is not None or getattr(case, "phase_mask", None) is not None:
         raise ValueError("Bessel form needs an axisymmetric pupil")
+    model = _model(case, model)
     r_um, varphi = np.broadcast_arrays(np.atleast_1d(r_um).astype(float), np.atleast_1d(varphi).astype(float))
     k = 2.0 * math.pi * case.n_immersion / case.wavelength_um
     ru, inv = np.unique(np.round(r_um, 12), return_inverse=True)           # equal radii share their integrals
@@ -390,7 +413,7 @@ def bessel_field(case, r_um, varphi, z_um: float, model="vectorial", paraxial=Fa
     return (-1j * k / 2.0) * np.stack([Ex, Ey, Ez], axis=0)
 
 
-def bessel_stack(case, planes=None, model="vectorial", paraxial=False, n_nodes=4001):
+def bessel_stack(case, planes=None, model=None, paraxial=False, n_nodes=4001):
     """Bessel-form intensity on the output grid [len(planes), M, M]."""
     M = case.out_m
     xs = out_coords(M, case.pixel_um)
@@ -398,6 +421,7 @@ def bessel_stack(case, planes=None, model="vectorial", paraxial=False, n_nodes=4
     r = np.hypot(X, Y).ravel()
     vp = np.arctan2(Y, X).ravel()
     planes = range(case.n_planes) if planes is None else planes
+    model = _model(case, model)
     out = []
     for b in planes:
         z = float(case.z_um[b])

@@ -58,6 +58,10 @@ class PsfCase:
     # per-plane lateral emitter positions (config 4), float32 [Z, 2] = (x_b, y_b)
     shifts_um: Optional[np.ndarray] = None
     seed: Optional[int] = None
+    # remaining correction factors of the paper; all fold into the static pupil
+    model: str = "vectorial"              # "vectorial" (Eq. 9) or "scalar" (Eq. 3: e_inf = e_inc = 1)
+    envelope_s: float = 0.0               # s_env of the Gaussian envelope exp(-sin^2 theta / s_env^2) (Eq. 20); 0 = off
+    phase_mask: Optional[np.ndarray] = None   # W_0 of PAPER.md:176 Eq. 18: float32 [N, N] radians on the pupil grid (row = p_y)
 
     @property
     def n_planes(self) -> int:

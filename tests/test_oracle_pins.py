@@ -375,3 +375,69 @@ def test_single_c4_is_a_quadratic_pupil_phase():
     pup = O.Pupil(case)
     ph = pup.plane_phase(0).real
     assert np.allclose(ph, float(np.float32(c4)) * math.sqrt(3) * (2 * pup.rho ** 2 - 1), atol=1e-13)
+
+
+# ---- further correction factors --------------------------------------------------------
+
+def test_gaussian_envelope_on_axis_dawson_closed_form_and_bessel_form():
+    """PAPER.md:194 Eq. 20.  Scalar, no apodisation, at focus on axis:
+    E = -i k int_c^1 exp(-(1 - u^2)/s^2) du = -i k s [D(1/s) - exp(-(1 - c^2)/s^2) D(c/s)],  D = Dawson's integral."""
+    from scipy.special import dawsn
+    s = 0.6
+    case = _case(apodize=False, envelope_s=s)
+    k = 2 * math.pi * 1.518 / 0.6
+    c = math.sqrt(1 - (1.4 / 1.518) ** 2)
+    closed = -1j * k * s * (dawsn(1 / s) - math.exp(-(1 - c * c) / s ** 2) * dawsn(c / s))
+    Eb = O.bessel_field(case, 0.0, 0.0, 0.0, model="scalar")[0, 0]
+    assert abs(Eb - closed) < 1e-10 * k
+    Ec = O.field_at(replace(case, pupil_n=256), 0, 0.0, 0.0, model="scalar")[0, 0]
+    assert abs(Ec - closed) < 3e-3 * abs(closed)
+    # the envelope really is a factor of the amplitude: without it the focus amplitude is the plain k (1 - c)
+    E0 = O.field_at(replace(case, pupil_n=256, envelope_s=0.0), 0, 0.0, 0.0, model="scalar")[0, 0]
+    assert abs(abs(E0) - k * (1 - c)) < 3e-3 * k * (1 - c) and abs(Ec) < 0.5 * abs(E0)
+    # vectorial, apodised, off axis and defocused: Cartesian sum against the Bessel form (Eq. 11-14 with a(theta))
+    cv = _case(envelope_s=0.8, pupil_n=128, out_m=16, pixel_um=0.09, z_um=np.array([-0.4, 0.3]), pol=W.POL_CIRC_L)
+    Ic, Ib = O.stack_T2(cv), O.bessel_stack(cv, n_nodes=2001)
+    assert np.abs(Ic - Ib).max() / Ib.max() < 1e-2
+
+
+def test_phase_mask_vortex_half_moon_and_zernike_equivalence():
+    """W_0 of PAPER.md:176 Eq. 18 on the pupil grid."""
+    N = 24
+    a = (2 * np.arange(N) + 1 - N).astype(np.float64)
+    phi = np.arctan2(a[:, None], a[None, :])                       # row = p_y
+    base = _case(pupil_n=N, out_m=9, z_um=np.array([0.0, 0.35]), model="scalar")
+    # vortex ramp exp(i phi): the grid maps onto itself under a 90 degree turn, which multiplies the pupil by i, so the
+    # on-axis field is zero exactly (donut); the ring around it is bright
+    Iv = O.stack_T2(replace(base, phase_mask=phi.astype(np.float32)))
+    assert Iv[:, 4, 4].max() < 1e-9 * Iv.max() and Iv[0, 4, 6] > 0.05 * Iv.max()
+    # half-moon: W_0 = pi on the half pupil s_x > 0 flips the sign of that half -> E is odd in x: zero on the line x = 0
+    hm = np.where(a[None, :] > 0, np.pi, 0.0) * np.ones((N, 1))
+    Ih = O.stack_T2(replace(base, phase_mask=hm.astype(np.float64)))
+    assert Ih[:, :, 4].max() < 1e-24 * Ih.max()
+    assert np.abs(Ih - Ih[:, :, ::-1]).max() < 1e-12 * Ih.max()
+    # a mask equal to c Z_7 (coma) gives the field of the Zernike path (vectorial, every component)
+    vec = _case(pupil_n=N, out_m=7, z_um=np.array([0.2]), pol=W.POL_CIRC_R)
+    pup = O.Pupil(vec)
+    z7 = np.zeros((N, N))
+    z7[pup.py, pup.px] = O.zernike_noll(7, pup.rho, pup.cosphi, pup.sinphi)
+    c7 = float(np.float32(0.41))
+    Em = O.field_T2(replace(vec, phase_mask=c7 * z7))
+    Ez = O.field_T2(replace(vec, zernike=np.array([c7], dtype=np.float32), noll_first=7))
+    assert np.abs(Em - Ez).max() < 1e-12 * np.abs(Ez).max()
+    # and it adds to the Zernike phase rather than replacing it
+    Eb = O.field_T2(replace(vec, phase_mask=c7 * z7, zernike=np.array([c7], dtype=np.float32), noll_first=7))
+    E2 = O.field_T2(replace(vec, zernike=np.array([2 * c7], dtype=np.float32), noll_first=7))
+    assert np.abs(Eb - E2).max() < 1e-6 * np.abs(E2).max()
+
+
+def test_scalar_model_is_the_case_default_and_has_one_component():
+    """`case.model = "scalar"` selects PAPER.md:70 Eq. 3 in every entry point; T1 = T2; polarisation is ignored."""
+    case = _case(pupil_n=12, out_m=5, z_um=np.array([0.3]), model="scalar", pol=W.POL_CIRC_L)
+    E2 = O.field_T2(case)
+    assert E2.shape[0] == 1
+    xs = O.out_coords(5, case.pixel_um)
+    E1 = O.field_at(case, 0, xs[3], xs[1])[:, 0]
+    assert abs(E1[0] - E2[0, 0, 1, 3]) < 1e-12 * np.abs(E2).max()
+    assert np.abs(O.stack_T2(case) - O.stack_T2(replace(case, pol=W.POL_UNPOLARIZED))).max() == 0.0
+    assert np.abs(O.stack_T2(case) - O.intensity_T1(case)).max() < 1e-12 * O.stack_T2(case).max()
