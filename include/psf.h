@@ -62,8 +62,14 @@ typedef enum {
 enum {
   PSF_FLAG_APODIZE = 1,      /* a(s) = sqrt(cos theta), Eq. 19                                     */
   PSF_FLAG_GIBSON_LANNI = 2, /* W(s) of PAPER.md:154 Eq. 16                                                     */
-  PSF_FLAG_FRESNEL = 4       /* q_s, q_p of PAPER.md:102-107 Eq. 7-8: not built yet -> PSF_ERR_UNSUPPORTED      */
+  PSF_FLAG_FRESNEL = 4,      /* q_s, q_p of PAPER.md:102-107 Eq. 7-8: not built yet -> PSF_ERR_UNSUPPORTED      */
+  PSF_FLAG_GAUSSIAN_ENVELOPE = 8 /* a(s) *= exp(-sin^2 theta / envelope_s^2), Eq. 20              */
 };
+
+typedef enum {
+  PSF_MODEL_VECTORIAL = 0, /* PAPER.md:116 Eq. 9: three field components through the rotation matrix of Eq. 6   */
+  PSF_MODEL_SCALAR = 1     /* PAPER.md:70 Eq. 3: e_inf = e_inc = 1, one component; `pol` and `jones` are ignored */
+} psf_model;
 
 typedef enum {
   PSF_PREC_AUTO = 0,   /* the library picks per problem size: 3XF16 when the tensor tiles fill, FP32 otherwise  */
@@ -91,6 +97,8 @@ typedef struct {
   unsigned flags;                                   /* PSF_FLAG_*                                               */
   psf_precision precision;
   int device;                                       /* CUDA device ordinal                                      */
+  psf_model model;                                  /* vectorial (0) or scalar                                  */
+  double envelope_s;                                /* s_env > 0, read iff PSF_FLAG_GAUSSIAN_ENVELOPE           */
 } psf_plan_desc;
 
 /* Build a plan: validates `desc`, evaluates every z-independent factor of the integrand in fp64 on the host
@@ -105,13 +113,19 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out);
  * coeffs == NULL or n_coeffs == 0 clears the Zernike term.  coeffs is host memory, copied. */
 psf_status psf_set_zernike(psf_plan *plan, const float *coeffs, int noll_first, int n_coeffs, int per_plane);
 
+/* Free phase mask W_0 of PAPER.md:176 Eq. 18 (vortex ramp, half-moon, measured wavefront ...): w0_rad is host
+ * [N][N] radians on the pupil grid (row = p_y, sample (p_y, p_x) at s = s_max (2p + 1 - N)/N), added to the static
+ * phase of every plane; values outside the disc are ignored.  NULL clears.  Copied. */
+psf_status psf_set_phase_mask(psf_plan *plan, const float *w0_rad);
+
 /* Per-plane lateral emitter position (x_b, y_b): plane b becomes I(x - x_b, y - y_b; z_b), applied as the pupil
  * tilt phase -k (s_x x_b + s_y y_b).  xy_um is host [n_planes][2]; NULL clears. */
 psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
 
 /* Enqueue the whole stack on `cuda_stream`:
  *   intensity : device fp32 [n_planes][M][M], x fastest (required);
- *   field     : device complex64 (interleaved re, im) [3][n_planes][M][M] = (E_x, E_y, E_z), or NULL.
+ *   field     : device complex64 (interleaved re, im) [3][n_planes][M][M] = (E_x, E_y, E_z), or NULL
+ *               ([1][n_planes][M][M] for PSF_MODEL_SCALAR).
  * Asynchronous; results are valid once the stream has passed this point. */
 psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void *field);
 
@@ -142,7 +156,7 @@ psf_status psf_profile_read(psf_plan *plan, float *stage_ms, int *launches);
 long long psf_last_upload_bytes(const psf_plan *plan);
 
 /* Host-only diagnostic (no device needed): the plan-time static pupil in fp64, before folding and rounding.
- *   n_components : out, 3 (coherent input) or 5 (unpolarised: the distinct scalar pupils a, b, d, c_x, c_y);
+ *   n_components : out, 3 (coherent input), 5 (unpolarised: the distinct scalar pupils a, b, d, c_x, c_y) or 1 (scalar);
  *   weights      : out [5], intensity weight of each component;
  *   base         : out [n_components][N][N][2] (re, im) = prefactor * a / s_z * e_inf,c * exp(i W_static), 0 outside
  *                  the disc; W_static includes the shared Zernike term given here (coeffs may be NULL);

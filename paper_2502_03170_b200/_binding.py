@@ -14,10 +14,11 @@ PSF_OK, PSF_ERR_INVALID_ARG, PSF_ERR_UNSUPPORTED, PSF_ERR_ALLOC, PSF_ERR_CUDA, P
 STATUS_NAMES = {0: "PSF_OK", 1: "PSF_ERR_INVALID_ARG", 2: "PSF_ERR_UNSUPPORTED", 3: "PSF_ERR_ALLOC",
                 4: "PSF_ERR_CUDA", 5: "PSF_ERR_STATE"}
 POL = {"x": 0, "y": 1, "circ_l": 2, "circ_r": 3, "jones": 4, "unpolarized": 5}
-FLAG_APODIZE, FLAG_GIBSON_LANNI, FLAG_FRESNEL = 1, 2, 4
+FLAG_APODIZE, FLAG_GIBSON_LANNI, FLAG_FRESNEL, FLAG_GAUSSIAN_ENVELOPE = 1, 2, 4, 8
+MODEL = {"vectorial": 0, "scalar": 1}
 PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 
-EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_compute", "psf_plan_destroy",
+EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
            "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes"]
 
@@ -35,7 +36,8 @@ class psf_plan_desc(C.Structure):
                 ("n_immersion_design", C.c_double), ("t_immersion_design_um", C.c_double),
                 ("t_immersion_um", C.c_double), ("pupil_n", C.c_int), ("out_m", C.c_int), ("pixel_um", C.c_double),
                 ("n_planes", C.c_int), ("z_um", C.POINTER(C.c_double)), ("pol", C.c_int), ("jones", C.c_double * 4),
-                ("flags", C.c_uint), ("precision", C.c_int), ("device", C.c_int)]
+                ("flags", C.c_uint), ("precision", C.c_int), ("device", C.c_int),
+                ("model", C.c_int), ("envelope_s", C.c_double)]
 
 
 _lib = None
@@ -63,6 +65,8 @@ def load_library(build_if_missing: bool = True):
     lib.psf_set_zernike.restype = C.c_int
     lib.psf_set_shifts.argtypes = [P, C.POINTER(C.c_float)]
     lib.psf_set_shifts.restype = C.c_int
+    lib.psf_set_phase_mask.argtypes = [P, C.POINTER(C.c_float)]
+    lib.psf_set_phase_mask.restype = C.c_int
     lib.psf_compute.argtypes = [P, P, P, P]
     lib.psf_compute.restype = C.c_int
     lib.psf_plan_destroy.argtypes = [P]
@@ -108,7 +112,11 @@ def make_desc(case, device: int = 0, precision: str = "auto"):
     d.z_um = z.ctypes.data_as(C.POINTER(C.c_double))
     d.pol = POL[case.pol]
     d.jones = (C.c_double * 4)(*[float(v) for v in case.jones])
-    d.flags = (FLAG_APODIZE if case.apodize else 0) | (FLAG_GIBSON_LANNI if case.gibson_lanni else 0)
+    env = float(getattr(case, "envelope_s", 0.0) or 0.0)
+    d.flags = ((FLAG_APODIZE if case.apodize else 0) | (FLAG_GIBSON_LANNI if case.gibson_lanni else 0) |
+               (FLAG_GAUSSIAN_ENVELOPE if env > 0 else 0))
+    d.model = MODEL[getattr(case, "model", "vectorial")]
+    d.envelope_s = env
     d.precision = PREC[precision]
     d.device = int(device)
     return d, z
@@ -130,7 +138,8 @@ class PsfPlan:
             raise PsfError(st, self._lib.psf_last_error(None).decode())
         self.n_planes, self.out_m, self.pupil_n = desc.n_planes, desc.out_m, desc.pupil_n
         self.device = int(device)
-        self.unpolarized = case.pol == "unpolarized"
+        self.n_components = 1 if getattr(case, "model", "vectorial") == "scalar" else 3
+        self.unpolarized = case.pol == "unpolarized" and self.n_components == 3
 
     def _check(self, st):
         if st != PSF_OK:
@@ -145,6 +154,16 @@ class PsfPlan:
         if a.ndim == 2 and a.shape[0] != self.n_planes:
             raise ValueError("per-plane Zernike rows must match n_planes")
         self._check(self._lib.psf_set_zernike(self._h, _fptr(a), int(noll_first), int(a.shape[-1]), int(a.ndim == 2)))
+
+    def set_phase_mask(self, w0_rad):
+        """Free phase mask W_0: None or float32 [N, N] radians on the pupil grid (row = p_y)."""
+        if w0_rad is None:
+            self._check(self._lib.psf_set_phase_mask(self._h, None))
+            return
+        a = np.ascontiguousarray(np.asarray(w0_rad, dtype=np.float32))
+        if a.shape != (self.pupil_n, self.pupil_n):
+            raise ValueError("phase mask must be [pupil_n, pupil_n]")
+        self._check(self._lib.psf_set_phase_mask(self._h, _fptr(a)))
 
     def set_shifts(self, xy_um):
         if xy_um is None:
@@ -167,8 +186,8 @@ class PsfPlan:
         if intensity is None:
             intensity = torch.empty((Z, M, M), dtype=torch.float32, device=dev)
         if want_field and field is None:
-            field = torch.empty((3, Z, M, M), dtype=torch.complex64, device=dev)
-        for t, shape, dt in ((intensity, (Z, M, M), torch.float32), (field, (3, Z, M, M), torch.complex64)):
+            field = torch.empty((self.n_components, Z, M, M), dtype=torch.complex64, device=dev)
+        for t, shape, dt in ((intensity, (Z, M, M), torch.float32), (field, (self.n_components, Z, M, M), torch.complex64)):
             if t is not None and (tuple(t.shape) != shape or t.dtype != dt or not t.is_contiguous() or not t.is_cuda):
                 raise ValueError(f"output must be a contiguous CUDA tensor of shape {shape} and dtype {dt}")
         s = torch.cuda.current_stream(dev) if stream is None else stream
@@ -216,6 +235,8 @@ def plan_from_case(case, device: int = 0, precision: str = "auto") -> PsfPlan:
         plan.set_zernike(case.zernike, case.noll_first)
     if case.shifts_um is not None:
         plan.set_shifts(case.shifts_um)
+    if getattr(case, "phase_mask", None) is not None:
+        plan.set_phase_mask(case.phase_mask)
     return plan
 
 

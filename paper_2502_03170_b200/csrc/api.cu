@@ -52,7 +52,8 @@ psf_status upload_static(psf_plan *p) {
   }
   PhaseTimer tm;
   std::vector<cplx> &base_z = p->h_base;
-  apply_shared_zernike(hp, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis, base_z);
+  apply_shared_zernike(hp, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis,
+                       p->phase_mask.empty() ? nullptr : p->phase_mask.data(), base_z);
   const int N = d.pupil_n, n = (N + 1) / 2, C = hp.C;
   const size_t NN = (size_t)N * N, nn = (size_t)n * n;
   DevPlan &P = p->dp;
@@ -286,6 +287,19 @@ psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int
   return refresh(p);
 }
 
+psf_status psf_set_phase_mask(psf_plan *p, const float *w0_rad) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  const size_t NN = (size_t)p->desc.pupil_n * p->desc.pupil_n;
+  if (w0_rad)
+    for (size_t i = 0; i < NN; ++i)
+      if (!std::isfinite(w0_rad[i])) { p->err = "non-finite phase-mask value"; return PSF_ERR_INVALID_ARG; }
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  p->phase_mask.clear();
+  if (w0_rad) p->phase_mask.assign(w0_rad, w0_rad + NN);
+  return refresh(p);
+}
+
 psf_status psf_set_shifts(psf_plan *p, const float *xy_um) {
   if (!p) return PSF_ERR_INVALID_ARG;
   if (xy_um)
@@ -303,7 +317,7 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
   if (!p) return PSF_ERR_INVALID_ARG;
   if (!intensity) { p->err = "intensity is NULL"; return PSF_ERR_INVALID_ARG; }
   if (((uintptr_t)intensity & 15) || ((uintptr_t)field & 15)) { p->err = "output pointers must be 16-byte aligned"; return PSF_ERR_INVALID_ARG; }
-  if (field && p->desc.pol == PSF_POL_UNPOLARIZED) {
+  if (field && p->desc.pol == PSF_POL_UNPOLARIZED && p->desc.model == PSF_MODEL_VECTORIAL) {
     p->err = "field output is undefined for PSF_POL_UNPOLARIZED (two incoherent fields)";
     return PSF_ERR_UNSUPPORTED;
   }

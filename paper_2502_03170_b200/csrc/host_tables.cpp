@@ -29,7 +29,11 @@ psf_status validate_desc(const psf_plan_desc *d, std::string &err) {
     for (int i = 0; i < 4; ++i)
       if (!std::isfinite(d->jones[i])) return bad("jones holds a non-finite value");
   if ((int)d->precision < 0 || (int)d->precision > (int)PSF_PREC_3XF16) return bad("unknown precision");
-  if (d->flags & ~(unsigned)(PSF_FLAG_APODIZE | PSF_FLAG_GIBSON_LANNI | PSF_FLAG_FRESNEL)) return bad("unknown flag bit");
+  if (d->flags & ~(unsigned)(PSF_FLAG_APODIZE | PSF_FLAG_GIBSON_LANNI | PSF_FLAG_FRESNEL | PSF_FLAG_GAUSSIAN_ENVELOPE))
+    return bad("unknown flag bit");
+  if ((int)d->model != (int)PSF_MODEL_VECTORIAL && (int)d->model != (int)PSF_MODEL_SCALAR) return bad("unknown model");
+  if ((d->flags & PSF_FLAG_GAUSSIAN_ENVELOPE) && !(d->envelope_s > 0 && std::isfinite(d->envelope_s)))
+    return bad("envelope_s must be > 0 with PSF_FLAG_GAUSSIAN_ENVELOPE");
   if (d->flags & PSF_FLAG_FRESNEL) { err = "PSF_FLAG_FRESNEL is not built yet"; return PSF_ERR_UNSUPPORTED; }
   if (d->flags & PSF_FLAG_GIBSON_LANNI) {
     const double v[] = {d->particle_depth_um, d->n_glass, d->t_glass_um, d->n_glass_design, d->t_glass_design_um,
@@ -105,14 +109,15 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
   P.N = N;
   P.k = 2.0 * kPi * d.n_immersion / d.wavelength_um;
   P.s_max = d.NA / d.n_immersion;
-  const bool unpol = d.pol == PSF_POL_UNPOLARIZED;
-  P.C = unpol ? 5 : 3;
+  const bool scalar = d.model == PSF_MODEL_SCALAR;               // PAPER.md:70 Eq. 3: e_inf = e_inc = 1
+  const bool unpol = !scalar && d.pol == PSF_POL_UNPOLARIZED;
+  P.C = scalar ? 1 : (unpol ? 5 : 3);
   for (int c = 0; c < 5; ++c) P.weight[c] = 0.0;
   if (unpol) {   // I = 1/2 (|A|^2 + 2|B|^2 + |D|^2 + |C_x|^2 + |C_y|^2): the two inputs share the off-diagonal entry
     const double w[5] = {0.5, 1.0, 0.5, 0.5, 0.5};
     for (int c = 0; c < 5; ++c) P.weight[c] = w[c];
   } else {
-    P.weight[0] = P.weight[1] = P.weight[2] = 1.0;
+    for (int c = 0; c < P.C; ++c) P.weight[c] = 1.0;
   }
   cplx jx(1, 0), jy(0, 0);
   const double r2 = std::sqrt(0.5);
@@ -135,6 +140,7 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
   const cplx pref = cplx(0.0, -P.k / (2.0 * kPi)) * (P.s_max * du) * (P.s_max * du);   // -(i k / 2 pi) (s_max du)^2, f = 1
   const bool apod = (d.flags & PSF_FLAG_APODIZE) != 0;
   const bool gl = (d.flags & PSF_FLAG_GIBSON_LANNI) != 0;
+  const bool env = (d.flags & PSF_FLAG_GAUSSIAN_ENVELOPE) != 0;
   for (int py = 0; py < N; ++py) {
     for (int px = 0; px < N; ++px) {
       const long ax = 2L * px + 1 - N, ay = 2L * py + 1 - N;
@@ -149,7 +155,8 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
       P.rho[i] = st / P.s_max;
       P.cosphi[i] = cp;
       P.sinphi[i] = sp;
-      const double amp = (apod ? std::sqrt(ct) : 1.0) / ct;     // Eq. 19 x the 1/s_z of Eq. 9
+      double amp = (apod ? std::sqrt(ct) : 1.0) / ct;           // Eq. 19 x the 1/s_z of Eq. 9
+      if (env) amp *= std::exp(-(st * st) / (d.envelope_s * d.envelope_s));   // PAPER.md:194 Eq. 20
       cplx W(0, 0);
       if (gl) W += gibson_lanni_W(d, st);
       if (coeffs)
@@ -161,7 +168,9 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
       const double b = 0.5 * (-1.0 + ct) * s2;
       const double dd = 0.5 * ((1.0 + c2) + (1.0 - c2) * ct);
       const double cx = -cp * st, cy = -sp * st;
-      if (unpol) {
+      if (scalar) {
+        P.base[i] = stat;
+      } else if (unpol) {
         const double g[5] = {a, b, dd, cx, cy};
         for (int c = 0; c < 5; ++c) P.base[(size_t)c * NN + i] = stat * g[c];
       } else {
@@ -182,16 +191,17 @@ void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<
 }
 
 void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
-                          std::vector<cplx> &base) {
+                          const float *w0, std::vector<cplx> &base) {
   const size_t NN = (size_t)P0.N * P0.N;
   base.resize(P0.base.size());
   const bool zern = coeffs && K > 0;
 #pragma omp parallel for schedule(static)
   for (long long i = 0; i < (long long)NN; ++i) {
     cplx e(1.0, 0.0);
-    if (zern && P0.mask[i]) {
-      double W = 0.0;
-      for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];
+    if ((zern || w0) && P0.mask[i]) {
+      double W = w0 ? (double)w0[i] : 0.0;                     // free phase mask W_0 (Eq. 18)
+      if (zern)
+        for (int j = 0; j < K; ++j) W += (double)coeffs[j] * basis[(size_t)j * NN + i];
       e = cplx(std::cos(W), std::sin(W));
     }
     for (int c = 0; c < P0.C; ++c) {

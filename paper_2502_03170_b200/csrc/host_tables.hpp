@@ -14,7 +14,7 @@ typedef std::complex<double> cplx;
 
 struct HostPupil {
   int N = 0;                       // pupil grid
-  int C = 0;                       // scalar pupils pushed through the DFT stages: 3, or 5 for unpolarised
+  int C = 0;                       // scalar pupils pushed through the DFT stages: 3, 5 for unpolarised, 1 for the scalar model
   double weight[5] = {0, 0, 0, 0, 0};
   double k = 0;                    // 2 pi n_i / lambda
   double s_max = 0;                // NA / n_i
@@ -39,9 +39,10 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
 // Zernike basis values Z_{noll_first+j} at every in-disc sample: out[j][N][N] (0 outside the disc).
 void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<double> &out);
 
-// base[c][i] = P0.base[c][i] * exp(i sum_j coeffs[j] basis[j][i]): the shared Zernike term folded into the static pupil.
+// base[c][i] = P0.base[c][i] * exp(i (sum_j coeffs[j] basis[j][i] + w0[i])): the shared Zernike term and the free
+// phase mask w0 ([N][N] radians, may be null) folded into the static pupil.
 void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
-                          std::vector<cplx> &base);
+                          const float *w0, std::vector<cplx> &base);
 
 // Zoomed-DFT phase table: phi[mi][qi] = k s_max u_qi x_mi for mi < m = ceil(M/2), qi < n = ceil(N/2).
 void build_dft_phase(const psf_plan_desc &d, std::vector<double> &phi);

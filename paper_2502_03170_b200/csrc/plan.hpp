@@ -55,6 +55,7 @@ struct psf_plan {
   std::vector<float> zern_rows;  // [Z][K]
   int K_rows = 0;
   std::vector<float> shifts;     // [Z][2]
+  std::vector<float> phase_mask; // [N][N] radians (psf_set_phase_mask), empty = none
   // host caches: static pupil without any Zernike term, and the Zernike basis of the last (noll_first, K)
   psf::HostPupil hp0;
   std::vector<double> zbasis;    // [K][N][N]

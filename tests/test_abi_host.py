@@ -109,3 +109,30 @@ def test_host_tables_odd_grid_and_jones():
     base, kap, mask = _oracle_base(case)
     assert np.array_equal(t["mask"], mask)
     assert np.abs(t["base"] - base).max() < 1e-11 * np.abs(base).max()
+
+
+def test_host_tables_scalar_model_and_gaussian_envelope():
+    """PSF_MODEL_SCALAR (one pupil, polarisation ignored) and PSF_FLAG_GAUSSIAN_ENVELOPE against the oracle's pupil."""
+    case = replace(W.config3(), pupil_n=40, model="scalar", envelope_s=0.7, pol=W.POL_CIRC_L)
+    t = psf.host_tables(case)
+    base, kap, mask = _oracle_base(case)
+    assert t["n_components"] == 1 and base.shape[0] == 1 and t["weights"][0] == 1.0
+    assert np.abs(t["base"][:1] - base).max() < 1e-11 * np.abs(base).max()
+    vec = replace(W.config2(), pupil_n=33, envelope_s=0.45)
+    t = psf.host_tables(vec, vec.zernike, vec.noll_first)
+    base, _, _ = _oracle_base(vec)
+    assert np.abs(t["base"] - base).max() < 1e-11 * np.abs(base).max()
+    # the envelope changes the pupil (rim amplitude down by exp(-s_max^2 / s_env^2))
+    t0 = psf.host_tables(replace(vec, envelope_s=0.0), vec.zernike, vec.noll_first)
+    assert np.abs(t["base"]).max() < np.abs(t0["base"]).max()
+
+
+def test_model_and_envelope_validation():
+    lib = psf.load_library()
+    desc, keep = psf.make_desc(W.config1())
+    h = C.c_void_p()
+    desc.model = 7
+    assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 1 and b"model" in lib.psf_last_error(None)
+    desc.model = 0
+    desc.flags |= 8          # PSF_FLAG_GAUSSIAN_ENVELOPE with envelope_s = 0
+    assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 1 and b"envelope_s" in lib.psf_last_error(None)

@@ -226,3 +226,48 @@ def test_cta_pair_kernels_replan_chunked_and_single_plane(psf, monkeypatch):
     I, path = gpu_stack(psf, one, "auto")
     assert path == "tc3xf16"
     assert plane_errors(I, O.stack_T2(one)).max() <= TOL
+
+
+def _vortex(N):
+    a = (2 * np.arange(N) + 1 - N).astype(np.float64)
+    return np.arctan2(a[:, None], a[None, :]).astype(np.float32)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_scalar_model_gaussian_envelope_and_phase_mask(psf, precision):
+    """the scalar Cartesian model (Eq. 3), the Gaussian envelope (Eq. 20) and a free
+    phase mask W_0 (Eq. 18) all enter through the static pupil; every kernel path must still match the oracle."""
+    z = np.array([-0.6, 0.0, 0.45])
+    cases = [
+        # scalar + envelope + Gibson-Lanni, sizes that fill the tensor tiles
+        replace(W.config3(), pupil_n=200, out_m=260, z_um=z, model="scalar", envelope_s=0.7),
+        # vectorial, circular input, vortex mask (donut) + shared Zernike terms
+        replace(W.config2(), pupil_n=192, out_m=200, z_um=z, phase_mask=_vortex(192)),
+        # small grids (fused path): scalar with a half-moon mask; vectorial with envelope and per-plane rows
+        replace(W.config1(), pupil_n=40, out_m=33, z_um=z, model="scalar",
+                phase_mask=np.where(np.arange(40)[None, :] >= 20, np.float32(np.pi), np.float32(0)) * np.ones((40, 1), np.float32)),
+        replace(W.small_random_case(81, pupil_n=50, out_m=40, n_planes=3), envelope_s=0.5),
+    ]
+    for case in cases:
+        I, path = gpu_stack(psf, case, precision)
+        ref = O.stack_T2(case)
+        assert plane_errors(I, ref).max() <= TOL, (case.name, path)
+    # the donut really is dark on axis (odd grid -> a pixel on the axis)
+    donut = replace(W.config2(), pupil_n=96, out_m=65, z_um=np.array([0.0]), zernike=None, model="scalar", phase_mask=_vortex(96))
+    I, _ = gpu_stack(psf, donut, precision)
+    assert I[0, 32, 32] <= 1e-6 * I.max()
+
+
+def test_scalar_field_output_and_pair_kernels_with_mask(psf):
+    case = replace(W.config1(), pupil_n=70, out_m=45, z_um=np.array([-0.3, 0.2]), model="scalar", envelope_s=0.9)
+    (I, F), path = gpu_stack(psf, case, "fp32", want_field=True)
+    Eref = O.field_T2(case)
+    assert F.shape == Eref.shape == (1, 2, 45, 45)
+    assert np.abs(F - Eref).max() <= 2e-5 * np.abs(Eref).max()
+    # pair kernels (m_pad = 256): one scalar pupil, and five unpolarised pupils with a mask and an envelope
+    big = W.small_random_case(82, pupil_n=384, out_m=512, n_planes=2, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
+    for c in (replace(big, model="scalar", phase_mask=_vortex(384)),
+              replace(big, envelope_s=0.6, phase_mask=(0.5 * _vortex(384)).astype(np.float32))):
+        I, path = gpu_stack(psf, c, "auto")
+        assert path == "tc3xf16"
+        assert plane_errors(I, O.stack_T2(c)).max() <= TOL
