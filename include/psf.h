@@ -129,6 +129,16 @@ psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
  * Asynchronous; results are valid once the stream has passed this point. */
 psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void *field);
 
+/* Spherical (Bessel) parametrisation of the same integral, Eq. 11-14 (Eq. 5 for PSF_MODEL_SCALAR):
+ * three 1-D integrals over theta per (radius, plane) by composite Simpson with `n_nodes` (odd, >= 3) nodes, then Eq. 11
+ * with the plan's Jones vector.  Valid for axisymmetric pupils only: PSF_ERR_STATE while Zernike terms, shifts or a
+ * phase mask are set.  It is a different discretisation of the integral than psf_compute (quadrature in theta instead of
+ * the N x N pupil grid): the two agree to the quadrature error of the pupil grid, not to rounding.
+ *   psf_spherical_prepare : host tables for n_nodes, device scratch [n_planes][m (m + 1) / 2][3] complex64 (may allocate);
+ *   psf_compute_spherical : enqueue on `cuda_stream`; intensity is device fp32 [n_planes][M][M] as for psf_compute. */
+psf_status psf_spherical_prepare(psf_plan *plan, int n_nodes);
+psf_status psf_compute_spherical(psf_plan *plan, void *cuda_stream, float *intensity);
+
 psf_status psf_plan_destroy(psf_plan *plan);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /
@@ -147,7 +157,8 @@ psf_status psf_profile_enable(psf_plan *plan, int enable);
 
 /* After the caller has synchronised the stream of the last psf_compute: device time per stage of that call.
  *   stage_ms : host out [4], milliseconds summed over the launches of each stage
- *              (0 = stage-1 row DFT with the fused pupil producer, 1 = stage-2 column DFT + intensity, 2, 3 = unused);
+ *              (0 = stage-1 row DFT with the fused pupil producer, 1 = stage-2 column DFT + intensity,
+ *               2 = Bessel integrals, 3 = Eq. 11 combination of psf_compute_spherical);
  *   launches : host out [4], number of launches of each stage.
  * PSF_ERR_STATE if profiling is not enabled or no psf_compute ran since. */
 psf_status psf_profile_read(psf_plan *plan, float *stage_ms, int *launches);

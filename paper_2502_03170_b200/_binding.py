@@ -19,6 +19,7 @@ MODEL = {"vectorial": 0, "scalar": 1}
 PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
+           "psf_spherical_prepare", "psf_compute_spherical",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
            "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes"]
 
@@ -68,6 +69,10 @@ def load_library(build_if_missing: bool = True):
     lib.psf_set_phase_mask.argtypes = [P, C.POINTER(C.c_float)]
     lib.psf_set_phase_mask.restype = C.c_int
     lib.psf_compute.argtypes = [P, P, P, P]
+    lib.psf_spherical_prepare.argtypes = [P, C.c_int]
+    lib.psf_spherical_prepare.restype = C.c_int
+    lib.psf_compute_spherical.argtypes = [P, P, P]
+    lib.psf_compute_spherical.restype = C.c_int
     lib.psf_compute.restype = C.c_int
     lib.psf_plan_destroy.argtypes = [P]
     lib.psf_plan_destroy.restype = C.c_int
@@ -193,6 +198,21 @@ class PsfPlan:
         s = torch.cuda.current_stream(dev) if stream is None else stream
         self.compute_raw(s.cuda_stream, intensity.data_ptr(), field.data_ptr() if field is not None else 0)
         return (intensity, field) if field is not None else intensity
+
+    def compute_spherical(self, n_nodes: int = 2001, intensity=None, stream=None):
+        """Spherical (Bessel) parametrisation, axisymmetric pupils only; prepares its tables on first use or when
+        n_nodes changes."""
+        import torch
+        dev = torch.device("cuda", self.device)
+        if getattr(self, "_sph_nodes", None) != int(n_nodes):
+            self._check(self._lib.psf_spherical_prepare(self._h, int(n_nodes)))
+            self._sph_nodes = int(n_nodes)
+        Z, M = self.n_planes, self.out_m
+        if intensity is None:
+            intensity = torch.empty((Z, M, M), dtype=torch.float32, device=dev)
+        s = torch.cuda.current_stream(dev) if stream is None else stream
+        self._check(self._lib.psf_compute_spherical(self._h, C.c_void_p(s.cuda_stream), C.c_void_p(intensity.data_ptr())))
+        return intensity
 
     def profile_enable(self, enable: bool = True):
         self._check(self._lib.psf_profile_enable(self._h, int(bool(enable))))

@@ -207,6 +207,7 @@ void free_all(psf_plan *p) {
   for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
   p->prof_ev.clear();
   tc_free(p);
+  bessel_free(p);
 }
 
 }  // namespace
@@ -331,6 +332,40 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
   cudaError_t e = tc ? launch_tc(p, st, intensity)
                      : (p->path == 3 || small_eligible(p)) ? launch_small(p, st, intensity, (float2 *)field)
                                                             : launch_ffma(p, st, intensity, (float2 *)field);
+  if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  return PSF_OK;
+}
+
+// ---- spherical (Bessel) parametrisation: axisymmetric pupils only ---------------------------------------------------
+static bool axisymmetric(psf_plan *p) {
+  if (!p->zern_shared.empty() || p->K_rows > 0 || !p->shifts.empty() || !p->phase_mask.empty()) {
+    p->err = "the spherical parametrisation needs an axisymmetric pupil: clear Zernike terms, shifts and the phase mask";
+    return false;
+  }
+  return true;
+}
+
+psf_status psf_spherical_prepare(psf_plan *p, int n_nodes) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (n_nodes < 3 || !(n_nodes & 1) || n_nodes > (1 << 20)) { p->err = "n_nodes must be odd, >= 3 (composite Simpson)"; return PSF_ERR_INVALID_ARG; }
+  if (!axisymmetric(p)) return PSF_ERR_STATE;
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  return bessel_setup(p, n_nodes);
+}
+
+psf_status psf_compute_spherical(psf_plan *p, void *cuda_stream, float *intensity) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (!intensity || ((uintptr_t)intensity & 15)) { p->err = "intensity must be a 16-byte aligned device pointer"; return PSF_ERR_INVALID_ARG; }
+  if (!p->bessel) { p->err = "psf_spherical_prepare has not been called"; return PSF_ERR_STATE; }
+  if (!axisymmetric(p)) return PSF_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (p->prof) {
+    p->prof_n = 0;
+    p->prof_valid = true;
+    cudaEventRecord(p->prof_ev[0], st);
+  }
+  cudaError_t e = launch_bessel(p, st, intensity);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
 }

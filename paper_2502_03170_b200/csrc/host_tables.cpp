@@ -211,6 +211,31 @@ void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const
   }
 }
 
+void build_bessel_nodes(const psf_plan_desc &d, int n_nodes, BesselNodes &B) {
+  B.n = n_nodes;
+  B.k = 2.0 * kPi * d.n_immersion / d.wavelength_um;
+  const double th_max = std::asin(d.NA / d.n_immersion);
+  const double h = th_max / (n_nodes - 1);
+  const bool apod = (d.flags & PSF_FLAG_APODIZE) != 0;
+  const bool gl = (d.flags & PSF_FLAG_GIBSON_LANNI) != 0;
+  const bool env = (d.flags & PSF_FLAG_GAUSSIAN_ENVELOPE) != 0;
+  B.sinth.resize(n_nodes);
+  B.costh.resize(n_nodes);
+  B.A.resize(n_nodes);
+  for (int j = 0; j < n_nodes; ++j) {
+    const double th = (j == n_nodes - 1) ? th_max : j * h;
+    const double st = std::sin(th), ct = std::cos(th);
+    const double w = ((j == 0 || j == n_nodes - 1) ? 1.0 : ((j & 1) ? 4.0 : 2.0)) * h / 3.0;   // composite Simpson
+    double a = apod ? std::sqrt(ct) : 1.0;
+    if (env) a *= std::exp(-(st * st) / (d.envelope_s * d.envelope_s));
+    cplx e(1.0, 0.0);
+    if (gl) e = std::exp(cplx(0, 1) * gibson_lanni_W(d, st));
+    B.sinth[j] = st;
+    B.costh[j] = ct;
+    B.A[j] = w * a * st * e;
+  }
+}
+
 void build_dft_phase(const psf_plan_desc &d, std::vector<double> &phi) {
   const int N = d.pupil_n, M = d.out_m;
   const int n = (N + 1) / 2, m = (M + 1) / 2;

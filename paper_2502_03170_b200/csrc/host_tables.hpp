@@ -44,6 +44,17 @@ void build_zernike_basis(const HostPupil &P, int noll_first, int K, std::vector<
 void apply_shared_zernike(const HostPupil &P0, const float *coeffs, int K, const std::vector<double> &basis,
                           const float *w0, std::vector<cplx> &base);
 
+// Nodes of the spherical (Bessel) parametrisation, Eq. 12-14 (Eq. 5 for the scalar model): composite
+// Simpson over theta in [0, theta_max] with n (odd, >= 3) nodes.  A[j] = w_j a(theta_j) sin(theta_j) exp(i W_GL(theta_j))
+// with a = apodisation x Gaussian envelope (no 1/s_z here: d Omega = sin(theta) d theta d phi).
+struct BesselNodes {
+  int n = 0;
+  double k = 0;                    // 2 pi n_i / lambda
+  std::vector<double> sinth, costh;
+  std::vector<cplx> A;
+};
+void build_bessel_nodes(const psf_plan_desc &d, int n_nodes, BesselNodes &out);
+
 // Zoomed-DFT phase table: phi[mi][qi] = k s_max u_qi x_mi for mi < m = ceil(M/2), qi < n = ceil(N/2).
 void build_dft_phase(const psf_plan_desc &d, std::vector<double> &phi);
 

@@ -36,7 +36,8 @@ struct DevPlan {
   const float *cosT, *sinT;      // [m][n]        cos / sin of k s_max u_q x_mi
 };
 
-struct TcState;   // tcgen05 path (kernels_tc.cu)
+struct TcState;      // tcgen05 path (kernels_tc.cu)
+struct BesselState;  // spherical parametrisation (kernels_bessel.cu)
 
 }  // namespace psf
 
@@ -77,6 +78,7 @@ struct psf_plan {
   size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
   int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16, 3 = ffma_fused (small grids)
   psf::TcState *tc = nullptr;
+  psf::BesselState *bessel = nullptr;
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
 
@@ -108,4 +110,8 @@ psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::ve
 void tc_free(psf_plan *p);
 int tc_launches(const psf_plan *p);
 cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity);
+// kernels_bessel.cu
+psf_status bessel_setup(psf_plan *p, int n_nodes);
+void bessel_free(psf_plan *p);
+cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
 }  // namespace psf
