@@ -377,6 +377,30 @@ def run_ours(args):
                 sweep[name] = {"voxels_per_s": cs.voxels() / (ms * 1e-3), "planes_per_s": cs.n_planes / (ms * 1e-3),
                                "ms_per_step": ms, "path": r["path"], "launches": r["launches"]}
                 r["plan"].destroy()
+            # the spherical (Bessel) path on the two axisymmetric configs: ALU / SFU bound, context only
+            for name, c, nodes in (("cfg1_spherical", 1, 2001), ("cfg3_spherical", 3, 2001)):
+                cs = W.get_config(c)
+                plan = psf.plan_from_case(cs, device=local)
+                out = torch.empty((cs.n_planes, cs.out_m, cs.out_m), dtype=torch.float32, device=dev)
+                for _ in range(3):
+                    plan.compute_spherical(nodes, out)
+                torch.cuda.synchronize(dev)
+                ts = []
+                for i in range(min(args.steps, 10)):
+                    flush.fill_(float(i % 251))
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    plan.compute_spherical(nodes, out)
+                    b.record()
+                    torch.cuda.synchronize(dev)
+                    ts.append(a.elapsed_time(b))
+                ms = statistics.mean(ts)
+                m_half = (cs.out_m + 1) // 2
+                radii = m_half * (m_half + 1) // 2
+                sweep[name] = {"voxels_per_s": cs.voxels() / (ms * 1e-3), "ms_per_step": ms, "path": "spherical_bessel",
+                               "simpson_nodes": nodes, "launches": 2,
+                               "bessel_terms_per_s": radii * nodes * cs.n_planes / (ms * 1e-3)}
+                plan.destroy()
             line["workloads"] = sweep
     if rank == 0:
         print(json.dumps(line))
