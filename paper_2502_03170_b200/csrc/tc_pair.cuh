@@ -8,7 +8,8 @@
 //   k1_pair (stage 1):  D[mx, (half, slot, ql)] = X_g[mx, qx] * Q[(half, slot, ql), qx]^T      M = 256 mx, N = 256
 //       A = cos / sin table rows of the CTA's own 128 mx, by TMA;
 //       B = pupil field: CTA `half` generates slots (4 chains of the x-parity group) x 32 q_y = 128 rows straight into its
-//           swizzled shared memory (each pupil element is generated once per pair);
+//           swizzled shared memory (each pupil element is generated once per pair); the base pupil of a stage arrives by
+//           one bulk copy into a shared-memory ring, the defocus phasors of a tile live in registers;
 //       epilogue: one thread per mx row holds 64 consecutive q_y of a chain -> scale, fp16 hi / lo, 16-byte stores into a
 //           swizzled staging tile, TMA store into T^T[chain][mx][qy].
 //   k2_pair (stage 2):  D[my, (slot, mx)] = Y_a[my, qy] * T^T[(slot, mx), qy]^T                 M = 256 my, N = 4 x 64
@@ -51,16 +52,7 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
 }
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {   // acquire at cluster scope
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
+// (waits use the plain mbar_wait: an .acquire.cluster try_wait adds an L1 invalidate, CCTL.IVALL, to every successful wait)
 // TMA loads whose completion bytes are credited to an mbarrier of the pair's leader CTA (`bar_cluster` = mapa(bar, 0))
 __device__ __forceinline__ void tma2_load_2d(uint32_t smem_dst, const void *tmap, uint32_t bar_cluster, int x, int y) {
   asm volatile(
