@@ -102,6 +102,24 @@ def far_field_g(costh, sinth, cosphi, sinphi, px, py, q_s=1.0, q_p=1.0):
     return tuple(0.5 * (cx * px + cy * py) for cx, cy in zip(col_x, col_y))
 
 
+def fresnel_q(case, sinth):
+    """(q_s, q_p) of PAPER.md:102-107 Eq. 7-8 (reading G2: Eq. 7 is q_s, Eq. 8 is q_p): the product over the interfaces
+    immersion -> glass -> sample (focusing direction, reading A2) of
+        q_s^j = 2 n_j cos(theta_j) / (n_j cos(theta_j) + n_{j+1} cos(theta_{j+1}))
+        q_p^j = 2 n_j cos(theta_j) / (n_{j+1} cos(theta_j) + n_j cos(theta_{j+1}))
+    with Snell's law n_j sin(theta_j) = n_i sin(theta) and the principal complex root for cos(theta_j) past a
+    critical angle (the branch of A3b).  Complex arrays."""
+    n = (case.n_immersion, case.n_glass, case.n_sample)
+    a = case.n_immersion * np.asarray(sinth, dtype=np.float64)
+    cos = [_csqrt(1.0 - (a / nj) ** 2) for nj in n]
+    q_s = np.ones_like(cos[0])
+    q_p = np.ones_like(cos[0])
+    for j in range(len(n) - 1):
+        q_s = q_s * (2.0 * n[j] * cos[j] / (n[j] * cos[j] + n[j + 1] * cos[j + 1]))
+        q_p = q_p * (2.0 * n[j] * cos[j] / (n[j + 1] * cos[j] + n[j] * cos[j + 1]))
+    return q_s, q_p
+
+
 def _csqrt(v):
     """Principal complex square root of a real array: +i sqrt(|v|) for v < 0 (reading A3b)."""
     return np.sqrt(np.asarray(v, dtype=np.float64).astype(np.complex128))
@@ -210,7 +228,8 @@ class Pupil:
         # far field
         if model == "vectorial":
             pxj, pyj = jones_vector(case) if jones is None else jones
-            self.g = far_field_g(self.costh, self.sinth, self.cosphi, self.sinphi, pxj, pyj)
+            q_s, q_p = fresnel_q(case, self.sinth) if getattr(case, "fresnel", False) else (1.0, 1.0)
+            self.g = far_field_g(self.costh, self.sinth, self.cosphi, self.sinphi, pxj, pyj, q_s, q_p)
         elif model == "scalar":             # PAPER.md:63 e_inf = e_inc (= 1)
             self.g = (np.ones_like(self.costh, dtype=np.complex128),)
         else:
@@ -383,9 +402,12 @@ def bessel_integrals(case, r_um, z_um: float, model=None, paraxial=False, n_node
     arg = k * np.outer(r_um, st)                                           # k rho sin(theta)
     if model == "scalar":
         return (jv(0, arg) @ (w * a * st),)
-    I0 = jv(0, arg) @ (w * a * st * (ct + 1.0))                            # Eq. 12
-    I1 = jv(1, arg) @ (w * a * st * st)                                    # Eq. 13
-    I2 = jv(2, arg) @ (w * a * st * (ct - 1.0))                            # Eq. 14
+    # with Fresnel coefficients the phi integral of Eq. 6 gives (q_s + q_p cos), q_p sin, (q_p cos - q_s) in place of
+    # (1 + cos), sin, (cos - 1): footnote 3 applied to the entries of Eq. 6
+    q_s, q_p = fresnel_q(case, st) if getattr(case, "fresnel", False) else (1.0, 1.0)
+    I0 = jv(0, arg) @ (w * a * st * (q_s + q_p * ct))                      # Eq. 12
+    I1 = jv(1, arg) @ (w * a * st * (q_p * st))                            # Eq. 13
+    I2 = jv(2, arg) @ (w * a * st * (q_p * ct - q_s))                      # Eq. 14
     return I0, I1, I2
 
 

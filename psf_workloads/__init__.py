@@ -61,6 +61,7 @@ class PsfCase:
     # remaining correction factors of the paper; all fold into the static pupil
     model: str = "vectorial"              # "vectorial" (Eq. 9) or "scalar" (Eq. 3: e_inf = e_inc = 1)
     envelope_s: float = 0.0               # s_env of the Gaussian envelope exp(-sin^2 theta / s_env^2) (Eq. 20); 0 = off
+    fresnel: bool = False                 # q_s, q_p of PAPER.md:102-107 Eq. 7-8 over immersion -> glass -> sample (reading A2)
     phase_mask: Optional[np.ndarray] = None   # W_0 of PAPER.md:176 Eq. 18: float32 [N, N] radians on the pupil grid (row = p_y)
 
     @property

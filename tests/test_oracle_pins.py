@@ -441,3 +441,50 @@ def test_scalar_model_is_the_case_default_and_has_one_component():
     assert abs(E1[0] - E2[0, 0, 1, 3]) < 1e-12 * np.abs(E2).max()
     assert np.abs(O.stack_T2(case) - O.stack_T2(replace(case, pol=W.POL_UNPOLARIZED))).max() == 0.0
     assert np.abs(O.stack_T2(case) - O.intensity_T1(case)).max() < 1e-12 * O.stack_T2(case).max()
+
+
+def test_fresnel_coefficients_textbook_values_and_energy_balance():
+    """PAPER.md:102-107 Eq. 7-8 (readings G2, A2) against what the textbook fixes for a single interface: normal
+    incidence, Brewster's angle, and T + R = 1 with the reflection coefficients written out independently."""
+    n1, n2 = 1.518, 1.33
+    one = _case(n_immersion=n1, n_glass=n1, n_sample=n2, NA=1.2)          # glass = immersion: a single interface
+    qs0, qp0 = O.fresnel_q(one, np.array([0.0]))
+    assert abs(qs0[0] - 2 * n1 / (n1 + n2)) < 1e-15 and abs(qp0[0] - 2 * n1 / (n1 + n2)) < 1e-15
+    thB = math.atan(n2 / n1)                                               # Brewster: no p reflection, t_p = n1 / n2
+    _, qpB = O.fresnel_q(one, np.array([math.sin(thB)]))
+    assert abs(qpB[0] - n1 / n2) < 1e-14
+    th = np.linspace(0.0, math.asin(n2 / n1) * 0.999, 50)                  # below the critical angle
+    c1 = np.cos(th)
+    c2 = np.sqrt(1 - (n1 * np.sin(th) / n2) ** 2)
+    qs, qp = O.fresnel_q(one, np.sin(th))
+    Rs = ((n1 * c1 - n2 * c2) / (n1 * c1 + n2 * c2)) ** 2
+    Rp = ((n2 * c1 - n1 * c2) / (n2 * c1 + n1 * c2)) ** 2
+    T = n2 * c2 / (n1 * c1)
+    assert np.abs(T * np.abs(qs) ** 2 + Rs - 1).max() < 1e-13 and np.abs(T * np.abs(qp) ** 2 + Rp - 1).max() < 1e-13
+    # two interfaces multiply; matched indices transmit everything
+    two = _case(n_immersion=1.518, n_glass=1.46, n_sample=1.33, NA=1.2)
+    s = np.array([0.3, 0.7])
+    a = O.fresnel_q(_case(n_immersion=1.518, n_glass=1.518, n_sample=1.46, NA=1.2), s)
+    b = O.fresnel_q(_case(n_immersion=1.46, n_glass=1.46, n_sample=1.33, NA=1.2), s * 1.518 / 1.46)
+    qs2, qp2 = O.fresnel_q(two, s)
+    assert np.abs(qs2 - a[0] * b[0]).max() < 1e-15 and np.abs(qp2 - a[1] * b[1]).max() < 1e-15
+    m = O.fresnel_q(_case(n_glass=1.518), np.array([0.1, 0.9]))
+    assert np.abs(m[0] - 1).max() == 0 and np.abs(m[1] - 1).max() == 0
+    # past the critical angle the coefficients are complex with |q_s| <= 2 (total internal reflection: phase only in r)
+    qs_t, _ = O.fresnel_q(one, np.array([0.95]))
+    assert abs(qs_t[0].imag) > 0.1
+
+
+def test_fresnel_through_the_field_cartesian_equals_bessel_form():
+    """With Fresnel factors the phi integral of Eq. 6 gives (q_s + q_p cos), q_p sin, (q_p cos - q_s) in Eq. 12-14;
+    the discrete Cartesian sum with the complex q_s, q_p inside Eq. 6 must agree with that Bessel form (axisymmetric
+    case with index mismatch, supercritical rim included)."""
+    case = replace(W.config3(), pupil_n=512, out_m=18, pixel_um=0.1, z_um=np.array([-2.6, -2.0]), fresnel=True, n_glass=1.46,
+                   pol=W.POL_CIRC_R)
+    Ib = O.bessel_stack(case, n_nodes=4001)
+    Ic = O.stack_T2(case)
+    err = np.abs(Ic - Ib).max() / Ib.max()
+    coarse = np.abs(O.stack_T2(replace(case, pupil_n=128)) - Ib).max() / Ib.max()
+    assert err < 2e-3 and coarse > 5 * err                  # quadrature error of the pupil grid, falling with N
+    I0 = O.stack_T2(replace(case, fresnel=False))
+    assert np.abs(Ic - I0).max() / I0.max() > 5e-2          # the coefficients do change the PSF
