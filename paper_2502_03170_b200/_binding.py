@@ -119,7 +119,7 @@ def make_desc(case, device: int = 0, precision: str = "auto"):
     d.jones = (C.c_double * 4)(*[float(v) for v in case.jones])
     env = float(getattr(case, "envelope_s", 0.0) or 0.0)
     d.flags = ((FLAG_APODIZE if case.apodize else 0) | (FLAG_GIBSON_LANNI if case.gibson_lanni else 0) |
-               (FLAG_GAUSSIAN_ENVELOPE if env > 0 else 0))
+               (FLAG_GAUSSIAN_ENVELOPE if env > 0 else 0) | (FLAG_FRESNEL if getattr(case, "fresnel", False) else 0))
     d.model = MODEL[getattr(case, "model", "vectorial")]
     d.envelope_s = env
     d.precision = PREC[precision]

@@ -34,7 +34,8 @@ psf_status validate_desc(const psf_plan_desc *d, std::string &err) {
   if ((int)d->model != (int)PSF_MODEL_VECTORIAL && (int)d->model != (int)PSF_MODEL_SCALAR) return bad("unknown model");
   if ((d->flags & PSF_FLAG_GAUSSIAN_ENVELOPE) && !(d->envelope_s > 0 && std::isfinite(d->envelope_s)))
     return bad("envelope_s must be > 0 with PSF_FLAG_GAUSSIAN_ENVELOPE");
-  if (d->flags & PSF_FLAG_FRESNEL) { err = "PSF_FLAG_FRESNEL is not built yet"; return PSF_ERR_UNSUPPORTED; }
+  if ((d->flags & PSF_FLAG_FRESNEL) && !(d->n_glass > 0 && std::isfinite(d->n_glass)))
+    return bad("n_glass must be > 0 with PSF_FLAG_FRESNEL (interfaces immersion -> glass -> sample)");
   if (d->flags & PSF_FLAG_GIBSON_LANNI) {
     const double v[] = {d->particle_depth_um, d->n_glass, d->t_glass_um, d->n_glass_design, d->t_glass_design_um,
                         d->t_immersion_design_um};
@@ -87,6 +88,21 @@ double zernike_noll(int j, double rho, double cosphi, double sinphi) {
 
 // principal square root of a real number as a complex one: +i sqrt(|v|) for v < 0 (evanescent branch, A3b)
 static cplx csqrt_real(double v) { return v >= 0 ? cplx(std::sqrt(v), 0.0) : cplx(0.0, std::sqrt(-v)); }
+
+// q_s, q_p of PAPER.md:102-107 Eq. 7-8 (readings G2, A2): product over the interfaces immersion -> glass -> sample,
+// Snell's law n_j sin(theta_j) = n_i sin(theta), principal complex root for cos(theta_j) past a critical angle
+static void fresnel_q(const psf_plan_desc &d, double sinth, cplx &qs, cplx &qp) {
+  const double n[3] = {d.n_immersion, d.n_glass, d.n_sample};
+  const double a = d.n_immersion * sinth;
+  cplx c[3];
+  for (int j = 0; j < 3; ++j) c[j] = csqrt_real(1.0 - (a / n[j]) * (a / n[j]));
+  qs = cplx(1, 0);
+  qp = cplx(1, 0);
+  for (int j = 0; j < 2; ++j) {
+    qs *= 2.0 * n[j] * c[j] / (n[j] * c[j] + n[j + 1] * c[j + 1]);
+    qp *= 2.0 * n[j] * c[j] / (n[j + 1] * c[j] + n[j] * c[j + 1]);
+  }
+}
 
 static cplx gibson_lanni_W(const psf_plan_desc &d, double sinth) {
   const double k0 = 2.0 * kPi / d.wavelength_um;
@@ -141,6 +157,7 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
   const bool apod = (d.flags & PSF_FLAG_APODIZE) != 0;
   const bool gl = (d.flags & PSF_FLAG_GIBSON_LANNI) != 0;
   const bool env = (d.flags & PSF_FLAG_GAUSSIAN_ENVELOPE) != 0;
+  const bool fres = (d.flags & PSF_FLAG_FRESNEL) != 0;
   for (int py = 0; py < N; ++py) {
     for (int px = 0; px < N; ++px) {
       const long ax = 2L * px + 1 - N, ay = 2L * py + 1 - N;
@@ -162,16 +179,18 @@ void build_host_pupil(const psf_plan_desc &d, const float *coeffs, int noll_firs
       if (coeffs)
         for (int j = 0; j < n_coeffs; ++j) W += (double)coeffs[j] * zernike_noll(noll_first + j, P.rho[i], cp, sp);
       const cplx stat = pref * amp * std::exp(cplx(0, 1) * W);
-      // PAPER.md:93-97 Eq. 6 with q_s = q_p = 1 (Fresnel off)
+      // PAPER.md:93-97 Eq. 6; q_s = q_p = 1 unless PSF_FLAG_FRESNEL
+      cplx qs(1, 0), qp(1, 0);
+      if (fres) fresnel_q(d, st, qs, qp);
       const double c2 = cp * cp - sp * sp, s2 = 2.0 * sp * cp;
-      const double a = 0.5 * ((1.0 - c2) + (1.0 + c2) * ct);
-      const double b = 0.5 * (-1.0 + ct) * s2;
-      const double dd = 0.5 * ((1.0 + c2) + (1.0 - c2) * ct);
-      const double cx = -cp * st, cy = -sp * st;
+      const cplx a = 0.5 * (qs * (1.0 - c2) + qp * ((1.0 + c2) * ct));
+      const cplx b = 0.5 * (-qs + qp * ct) * s2;
+      const cplx dd = 0.5 * (qs * (1.0 + c2) + qp * ((1.0 - c2) * ct));
+      const cplx cx = -qp * (cp * st), cy = -qp * (sp * st);
       if (scalar) {
         P.base[i] = stat;
       } else if (unpol) {
-        const double g[5] = {a, b, dd, cx, cy};
+        const cplx g[5] = {a, b, dd, cx, cy};
         for (int c = 0; c < 5; ++c) P.base[(size_t)c * NN + i] = stat * g[c];
       } else {
         P.base[0 * NN + i] = stat * (a * jx + b * jy);

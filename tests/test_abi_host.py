@@ -60,9 +60,9 @@ def test_non_finite_z_and_null_out_are_rejected():
     desc, keep = psf.make_desc(W.config1())
     assert lib.psf_plan_create(C.byref(desc), None) == 1
     assert b"NULL" in lib.psf_last_error(None)
-    desc.flags = 4   # PSF_FLAG_FRESNEL
+    desc.flags = 64  # unknown flag bit
     h = C.c_void_p()
-    assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 2 and not h.value
+    assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 1 and not h.value
 
 
 def _oracle_base(case, jones=None):
@@ -136,3 +136,20 @@ def test_model_and_envelope_validation():
     desc.model = 0
     desc.flags |= 8          # PSF_FLAG_GAUSSIAN_ENVELOPE with envelope_s = 0
     assert lib.psf_plan_create(C.byref(desc), C.byref(h)) == 1 and b"envelope_s" in lib.psf_last_error(None)
+
+
+def test_host_tables_fresnel_coefficients():
+    """PSF_FLAG_FRESNEL: complex q_s, q_p inside Eq. 6 (coherent and unpolarised pupils), supercritical rim included."""
+    case = replace(W.config3(), pupil_n=36, fresnel=True, n_glass=1.46, pol=W.POL_CIRC_L)
+    t = psf.host_tables(case)
+    base, _, _ = _oracle_base(case)
+    assert np.abs(t["base"] - base).max() < 1e-11 * np.abs(base).max()
+    t0 = psf.host_tables(replace(case, fresnel=False))
+    assert np.abs(t["base"] - t0["base"]).max() > 1e-2 * np.abs(base).max()
+    un = replace(case, pol=W.POL_UNPOLARIZED)
+    t = psf.host_tables(un)
+    bx, _, _ = _oracle_base(un, jones=(1.0 + 0j, 0j))
+    by, _, _ = _oracle_base(un, jones=(0j, 1.0 + 0j))
+    a, b, d, cx, cy = t["base"]
+    for got, want in ((a, bx[0]), (b, bx[1]), (cx, bx[2]), (b, by[0]), (d, by[1]), (cy, by[2])):
+        assert np.abs(got - want).max() < 1e-11 * np.abs(bx).max()

@@ -302,3 +302,26 @@ def test_spherical_bessel_path_matches_oracle_bessel_form(psf):
         plan.compute_spherical(101)
     assert e.value.status == 5
     plan.destroy()
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_fresnel_coefficients_every_path(psf, precision):
+    """PSF_FLAG_FRESNEL (Eq. 7-8): complex q_s, q_p in the static pupil, supercritical rim included."""
+    z = np.array([-2.5, -2.0, 0.4])
+    cases = [
+        replace(W.config3(), pupil_n=160, out_m=200, z_um=z, fresnel=True, n_glass=1.46, pol=W.POL_CIRC_L),
+        replace(W.config3(), pupil_n=44, out_m=30, z_um=z, fresnel=True, n_glass=1.46, pol=W.POL_UNPOLARIZED),
+        replace(W.small_random_case(91, pupil_n=60, out_m=37, n_planes=3), fresnel=True),
+    ]
+    for case in cases:
+        I, path = gpu_stack(psf, case, precision)
+        assert plane_errors(I, O.stack_T2(case)).max() <= TOL, (case.name, path)
+    if precision == "auto":     # pair kernels, and the refusal of the spherical path
+        big = replace(W.config3(), pupil_n=320, out_m=512, z_um=z, fresnel=True, n_glass=1.46, pol=W.POL_UNPOLARIZED)
+        I, path = gpu_stack(psf, big, precision)
+        assert path == "tc3xf16" and plane_errors(I, O.stack_T2(big)).max() <= TOL
+        plan = psf.plan_from_case(cases[0])
+        with pytest.raises(psf.PsfError) as e:
+            plan.compute_spherical(101)
+        assert e.value.status == 2
+        plan.destroy()
