@@ -455,3 +455,45 @@ def bessel_stack(case, planes=None, model=None, paraxial=False, n_nodes=4001):
             I = np.sum(np.abs(bessel_field(case, r, vp, z, model, paraxial, None, n_nodes)) ** 2, axis=0)
         out.append(I.reshape(M, M))
     return np.stack(out, axis=0)
+
+
+# --------------------------------------------------------------------------------------------
+# Adjoint: gradients of a linear functional of the intensity
+# --------------------------------------------------------------------------------------------
+
+def grad_T2(case, G, planes=None, model=None):
+    """Gradients of L = sum_{b,y,x} G[b,y,x] I[b,y,x] with respect to the per-plane pupil phase parameters, by the
+    adjoint of the finite sum of `field_T2` (the paper's motivation for a differentiable PSF).
+
+    With Q_c[p] = amp g_c exp(i phi_b[p]) the pupil of plane b and phi_b = W + k cos(theta) z_b + sum_j c_bj Z_j - ...,
+        dI/dphi[p] = sum_c 2 Re( conj(E_c) i Q_c[p] A(x, p) ),   A(x, p) = prefactor exp(i k (s_x x + s_y y)),
+        dL/dphi_b[p] = -2 sum_c Im( Q_c[p] B_c[p] ),   B_c[p] = sum_x G conj(E_c(x)) A(x, p)   (the back-projection),
+        dL/dz_b = sum_p k cos(theta_p) dL/dphi_b[p],     dL/dc_bj = sum_p Z_j[p] dL/dphi_b[p].
+    Unpolarised light: the two incoherent inputs, each with weight 1/2.
+    Returns (dL_dz [len(planes)], dL_dc [len(planes), K] or None without Zernike terms).  A shared coefficient's
+    gradient is the sum of its column over the planes."""
+    model = _model(case, model)
+    planes = list(range(case.n_planes)) if planes is None else list(planes)
+    G = np.asarray(G, dtype=np.float64)
+    N, M = case.pupil_n, case.out_m
+    K = 0 if case.zernike is None else case.zernike.shape[-1]
+    dz = np.zeros(len(planes))
+    dc = np.zeros((len(planes), K)) if K else None
+    for wgt, pup in _pupils(case, model, False):
+        xs = out_coords(M, case.pixel_um)
+        Ax = np.exp(1j * pup.k * pup.s_max * np.outer(xs, pup.u))          # [m, p]
+        for ib, b in enumerate(planes):
+            e = np.exp(1j * pup.plane_phase(int(b)))
+            S = np.zeros(len(pup.px))
+            for g in pup.g:
+                Qd = pup.amp * g * e                                         # in-disc samples
+                P = np.zeros((N, N), dtype=np.complex128)
+                P[pup.py, pup.px] = Qd
+                E = pup.prefactor * (Ax @ (P @ Ax.T))                        # [m_y, m_x]
+                H = wgt * G[ib] * np.conj(E)
+                B = pup.prefactor * (Ax.T @ H @ Ax)                          # [p_y, p_x] = sum_x H A(x, p)
+                S += -2.0 * np.imag(Qd * B[pup.py, pup.px])
+            dz[ib] += np.sum(pup.k * pup.costh * S)
+            if K:
+                dc[ib] += pup.zernike_basis() @ S
+    return dz, dc

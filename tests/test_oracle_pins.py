@@ -488,3 +488,33 @@ def test_fresnel_through_the_field_cartesian_equals_bessel_form():
     assert err < 2e-3 and coarse > 5 * err                  # quadrature error of the pupil grid, falling with N
     I0 = O.stack_T2(replace(case, fresnel=False))
     assert np.abs(Ic - I0).max() / I0.max() > 5e-2          # the coefficients do change the PSF
+
+
+@pytest.mark.parametrize("pol", [W.POL_JONES, W.POL_UNPOLARIZED])
+def test_adjoint_gradients_match_finite_differences_of_the_forward_sum(pol):
+    """`grad_T2` (adjoint formula) against central differences of the pinned forward sum `stack_T2`: per-plane Zernike
+    rows, shared coefficients (column sums) and the defocus of every plane; every option on (Gibson-Lanni with the
+    evanescent rim, shifts, complex Jones vector / unpolarised)."""
+    rng = np.random.default_rng(5)
+    case = replace(W.small_random_case(101, pupil_n=14, out_m=11, n_planes=3, pol=pol), envelope_s=0.9)
+    G = rng.standard_normal((3, 11, 11))
+    L = lambda c: float(np.sum(G * O.stack_T2(c)))
+    dz, dc = O.grad_T2(case, G)
+    h = 1e-6
+    for b in range(3):
+        zp, zm = case.z_um.copy(), case.z_um.copy()
+        zp[b] += h; zm[b] -= h
+        fd = (L(replace(case, z_um=zp)) - L(replace(case, z_um=zm))) / (2 * h)
+        assert abs(fd - dz[b]) < 1e-6 * np.abs(dz).max()
+        for j in (0, 3, 5):
+            cp, cm = case.zernike.astype(np.float64), case.zernike.astype(np.float64)
+            cp[b, j] += h; cm[b, j] -= h
+            fd = (L(replace(case, zernike=cp)) - L(replace(case, zernike=cm))) / (2 * h)
+            assert abs(fd - dc[b, j]) < 1e-6 * np.abs(dc).max()
+    # shared coefficients: the gradient is the column sum over the planes
+    sh = replace(case, zernike=case.zernike[0].astype(np.float64), shifts_um=None)
+    _, dcs = O.grad_T2(sh, G)
+    cp, cm = sh.zernike.copy(), sh.zernike.copy()
+    cp[2] += h; cm[2] -= h
+    fd = (L(replace(sh, zernike=cp)) - L(replace(sh, zernike=cm))) / (2 * h)
+    assert abs(fd - dcs[:, 2].sum()) < 1e-6 * np.abs(dcs.sum(0)).max()
