@@ -142,6 +142,16 @@ psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void
 psf_status psf_spherical_prepare(psf_plan *plan, int n_nodes);
 psf_status psf_compute_spherical(psf_plan *plan, void *cuda_stream, float *intensity);
 
+/* Adjoint of psf_compute (the paper's differentiable-PSF use): for L = sum dL_dI[b][y][x] *
+ * I[b][y][x] the gradients with respect to the plane parameters the pupil phase depends on,
+ *   dL_dz : device fp64 [n_planes]            dL / d z_b (per micrometre);
+ *   dL_dc : device fp64 [n_planes][K] or NULL  dL / d c_bj for the K Zernike terms currently set (radians^-1); row b is
+ *           the contribution of plane b: for shared coefficients the gradient is the column sum over the planes.
+ * dL_dI is device fp32 [n_planes][M][M].  All polarisations incl. PSF_POL_UNPOLARIZED, both models, every correction
+ * factor.  The first call (and the first call after any psf_set_*) builds device copies of the unfolded tables and
+ * allocates scratch, so it may allocate and synchronise; later calls only enqueue on `cuda_stream`. */
+psf_status psf_gradients(psf_plan *plan, void *cuda_stream, const float *dL_dI, double *dL_dz, double *dL_dc);
+
 psf_status psf_plan_destroy(psf_plan *plan);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

@@ -19,7 +19,7 @@ MODEL = {"vectorial": 0, "scalar": 1}
 PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
-           "psf_spherical_prepare", "psf_compute_spherical",
+           "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
            "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes"]
 
@@ -69,6 +69,8 @@ def load_library(build_if_missing: bool = True):
     lib.psf_set_phase_mask.argtypes = [P, C.POINTER(C.c_float)]
     lib.psf_set_phase_mask.restype = C.c_int
     lib.psf_compute.argtypes = [P, P, P, P]
+    lib.psf_gradients.argtypes = [P, P, P, P, P]
+    lib.psf_gradients.restype = C.c_int
     lib.psf_spherical_prepare.argtypes = [P, C.c_int]
     lib.psf_spherical_prepare.restype = C.c_int
     lib.psf_compute_spherical.argtypes = [P, P, P]
@@ -213,6 +215,21 @@ class PsfPlan:
         s = torch.cuda.current_stream(dev) if stream is None else stream
         self._check(self._lib.psf_compute_spherical(self._h, C.c_void_p(s.cuda_stream), C.c_void_p(intensity.data_ptr())))
         return intensity
+
+    def gradients(self, dL_dI, n_terms: int = 0, stream=None):
+        """Adjoint: dL_dI is a CUDA float32 tensor [Z, M, M]; returns (dL_dz [Z], dL_dc [Z, n_terms] or None), float64
+        CUDA tensors.  n_terms = number of Zernike terms currently set (0: defocus gradients only)."""
+        import torch
+        dev = torch.device("cuda", self.device)
+        Z, M = self.n_planes, self.out_m
+        if tuple(dL_dI.shape) != (Z, M, M) or dL_dI.dtype != torch.float32 or not dL_dI.is_contiguous() or not dL_dI.is_cuda:
+            raise ValueError("dL_dI must be a contiguous CUDA float32 tensor [n_planes, M, M]")
+        dz = torch.empty((Z,), dtype=torch.float64, device=dev)
+        dc = torch.empty((Z, n_terms), dtype=torch.float64, device=dev) if n_terms > 0 else None
+        s = torch.cuda.current_stream(dev) if stream is None else stream
+        self._check(self._lib.psf_gradients(self._h, C.c_void_p(s.cuda_stream), C.c_void_p(dL_dI.data_ptr()),
+                                            C.c_void_p(dz.data_ptr()), C.c_void_p(dc.data_ptr()) if dc is not None else None))
+        return dz, dc
 
     def profile_enable(self, enable: bool = True):
         self._check(self._lib.psf_profile_enable(self._h, int(bool(enable))))

@@ -194,6 +194,7 @@ psf_status alloc_scratch(psf_plan *p) {
 
 psf_status refresh(psf_plan *p) {
   p->upload_bytes = 0;
+  ++p->table_version;
   psf_status s = upload_static(p);
   if (s != PSF_OK) return s;
   return alloc_scratch(p);     // C is fixed per plan, but keep the scratch consistent with it
@@ -208,6 +209,7 @@ void free_all(psf_plan *p) {
   p->prof_ev.clear();
   tc_free(p);
   bessel_free(p);
+  grad_free(p);
 }
 
 }  // namespace
@@ -370,6 +372,20 @@ psf_status psf_compute_spherical(psf_plan *p, void *cuda_stream, float *intensit
     cudaEventRecord(p->prof_ev[0], st);
   }
   cudaError_t e = launch_bessel(p, st, intensity);
+  if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  return PSF_OK;
+}
+
+// ---- adjoint ---------------------------------------------------------------------------------------------------------
+psf_status psf_gradients(psf_plan *p, void *cuda_stream, const float *dL_dI, double *dL_dz, double *dL_dc) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  if (!dL_dI || !dL_dz) { p->err = "dL_dI and dL_dz must be device pointers"; return PSF_ERR_INVALID_ARG; }
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  psf_status s = grad_setup(p);               // first call, or the tables changed: (re)build the adjoint's copies
+  if (s != PSF_OK) return s;
+  if (dL_dc && grad_terms(p) == 0) { p->err = "dL_dc asked for, but no Zernike terms are set"; return PSF_ERR_STATE; }
+  e = launch_grad(p, (cudaStream_t)cuda_stream, dL_dI, dL_dz, dL_dc);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
 }

@@ -38,6 +38,7 @@ struct DevPlan {
 
 struct TcState;      // tcgen05 path (kernels_tc.cu)
 struct BesselState;  // spherical parametrisation (kernels_bessel.cu)
+struct GradState;    // adjoint / gradients (kernels_grad.cu)
 
 }  // namespace psf
 
@@ -79,6 +80,8 @@ struct psf_plan {
   int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16, 3 = ffma_fused (small grids)
   psf::TcState *tc = nullptr;
   psf::BesselState *bessel = nullptr;
+  psf::GradState *grad = nullptr;
+  long long table_version = 0;   // bumped by every table refresh (psf_set_*): derived copies check it
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
 
@@ -114,4 +117,9 @@ cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity);
 psf_status bessel_setup(psf_plan *p, int n_nodes);
 void bessel_free(psf_plan *p);
 cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
+// kernels_grad.cu
+psf_status grad_setup(psf_plan *p);
+void grad_free(psf_plan *p);
+int grad_terms(const psf_plan *p);
+cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, double *dL_dz, double *dL_dc);
 }  // namespace psf

@@ -325,3 +325,41 @@ def test_fresnel_coefficients_every_path(psf, precision):
             plan.compute_spherical(101)
         assert e.value.status == 2
         plan.destroy()
+
+
+GRAD_TOL = 2e-4     # of the largest gradient component (fp32 products and sums over N^2 pupil samples)
+
+
+def test_adjoint_gradients_match_oracle(psf):
+    """psf_gradients against the oracle's adjoint (itself pinned by finite differences of the
+    forward sum): per-plane rows with shifts and a Jones vector, shared coefficients with unpolarised light, the scalar
+    model with a phase mask, and defocus-only gradients without any Zernike term."""
+    import torch
+    rng = np.random.default_rng(9)
+    cases = [
+        W.small_random_case(111, pupil_n=30, out_m=24, n_planes=3),
+        replace(W.small_random_case(112, pupil_n=64, out_m=48, n_planes=4, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED),
+                fresnel=True, envelope_s=0.8),
+        replace(W.small_random_case(113, pupil_n=41, out_m=33, n_planes=2, per_plane=False, shifts=False), model="scalar",
+                phase_mask=_vortex(41)),
+        replace(W.config3(), pupil_n=96, out_m=70, z_um=np.array([-2.7, -2.2, -1.5])),
+    ]
+    for case in cases:
+        G = rng.standard_normal((case.n_planes, case.out_m, case.out_m)).astype(np.float32)
+        dz_ref, dc_ref = O.grad_T2(case, G.astype(np.float64))
+        plan = psf.plan_from_case(case)
+        K = 0 if case.zernike is None else case.zernike.shape[-1]
+        dz, dc = plan.gradients(torch.from_numpy(G).cuda(), K)
+        torch.cuda.synchronize()
+        assert np.abs(dz.cpu().numpy() - dz_ref).max() <= GRAD_TOL * np.abs(dz_ref).max(), case.name
+        if K:
+            assert np.abs(dc.cpu().numpy() - dc_ref).max() <= GRAD_TOL * np.abs(dc_ref).max(), case.name
+        # a second call after new coefficients uses refreshed tables
+        if K and not case.per_plane_zernike:
+            other = replace(case, zernike=(case.zernike * 0.5).astype(np.float32))
+            plan.set_zernike(other.zernike, other.noll_first)
+            dz2, dc2 = plan.gradients(torch.from_numpy(G).cuda(), K)
+            r2, c2 = O.grad_T2(other, G.astype(np.float64))
+            assert np.abs(dc2.cpu().numpy() - c2).max() <= GRAD_TOL * np.abs(c2).max()
+            assert np.abs(dz2.cpu().numpy() - r2).max() <= GRAD_TOL * np.abs(r2).max()
+        plan.destroy()
