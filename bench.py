@@ -401,6 +401,33 @@ def run_ours(args):
                                "simpson_nodes": nodes, "launches": 2,
                                "bessel_terms_per_s": radii * nodes * cs.n_planes / (ms * 1e-3)}
                 plan.destroy()
+            # the adjoint: gradients w.r.t. z_b and the Zernike coefficients for a random dL/dI; complex
+            # fp32 FFMA products, so the roofline is the FFMA pipe
+            for name, c in (("cfg2_gradients", 2), ("cfg5_gradients", 5)):
+                cs = W.get_config(c)
+                plan = psf.plan_from_case(cs, device=local)
+                G = torch.randn((cs.n_planes, cs.out_m, cs.out_m), dtype=torch.float32, device=dev)
+                K = cs.zernike.shape[-1]
+                for _ in range(2):
+                    plan.gradients(G, K)
+                torch.cuda.synchronize(dev)
+                ts = []
+                for i in range(3):
+                    flush.fill_(float(i % 251))
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    plan.gradients(G, K)
+                    b.record()
+                    torch.cuda.synchronize(dev)
+                    ts.append(a.elapsed_time(b))
+                ms = statistics.mean(ts)
+                cg = 6 if cs.pol == "unpolarized" else 3
+                flop = 2 * 8.0 * cs.pupil_n * cs.out_m * (cs.pupil_n + cs.out_m) * cg * cs.n_planes     # forward + back-projection
+                ffma_peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+                sweep[name] = {"ms_per_step": ms, "planes_per_s": cs.n_planes / (ms * 1e-3), "path": "adjoint_ffma",
+                               "tflops": flop / (ms * 1e-3) / 1e12, "frac_of_ffma_peak": flop / (ms * 1e-3) / 1e12 / ffma_peak,
+                               "zernike_terms": int(K)}
+                plan.destroy()
             line["workloads"] = sweep
     if rank == 0:
         print(json.dumps(line))

@@ -45,10 +45,14 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
   return r;
 }
 // default semantics (release at CTA scope): a cluster-scope release compiles to MEMBAR.ALL.GPU + ERRBAR, microseconds per
-// arrive; what the waiter needs here (shared-memory operand writes made visible to the async proxy, TMEM reads
-// completed) is ordered by the fence.proxy.async / tcgen05.wait::ld + tcgen05.fence issued before the arrive
+// arrive.  Used where the signal carries no shared-memory data written by generic-proxy stores: accumulator hand-backs
+// (TMEM reads completed by tcgen05.wait::ld + tcgen05.fence).  Operand rows written with st.shared in the peer CTA need
+// mbar_arrive_cluster_release.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -426,7 +430,12 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         for (int i = 0; i < 2 * P.C * G.nk; ++i) {
           mbar_wait(&S.written[st], ph);
           fence_proxy_async_smem();
-          mbar_arrive_cluster(full_leader0 + st * 8);
+          // The peer CTA's operand rows were written by generic-proxy stores and are consumed because of THIS signal:
+          // it must be a cluster-scope release (MEMBAR.GPU, ~0.25 us per stage).  With the default CTA-scope release
+          // about 4 % of 256-plane runs had one stage read stale rows (profiles/r1j_race_k1_pair.md).  The leader's own
+          // rows are handed over inside its CTA, where the CTA-scope release is enough.
+          if (leader) mbar_arrive(&S.full[st]);
+          else mbar_arrive_cluster_release(full_leader0 + st * 8);
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
         }
       }
@@ -515,6 +524,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
             st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
             st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
           }
+          fence_proxy_async_smem();                                // every writer fences its own stores (no loads are in flight here)
           __syncwarp();
           if (lane == 0) mbar_arrive(&S.written[st]);
           if (++st == K1P_NST) { st = 0; ph ^= 1; }

@@ -327,7 +327,7 @@ def test_fresnel_coefficients_every_path(psf, precision):
         plan.destroy()
 
 
-GRAD_TOL = 2e-4     # of the largest gradient component (fp32 products and sums over N^2 pupil samples)
+GRAD_TOL = 2e-5     # of the largest gradient component: the intensity bar carried over (measured ~1e-6: fp32 products, fp64 sums)
 
 
 def test_adjoint_gradients_match_oracle(psf):
@@ -363,3 +363,23 @@ def test_adjoint_gradients_match_oracle(psf):
             assert np.abs(dc2.cpu().numpy() - c2).max() <= GRAD_TOL * np.abs(c2).max()
             assert np.abs(dz2.cpu().numpy() - r2).max() <= GRAD_TOL * np.abs(r2).max()
         plan.destroy()
+
+
+def test_pair_kernels_are_deterministic_under_repetition(psf):
+    """The pair kernels sum in a fixed order: repeated psf_compute calls on one plan are bit-identical.  Guards the
+    cross-CTA hand-off of generic-proxy operand writes in k1_pair (profiles/r1j_race_k1_pair.md): with a CTA-scope
+    release about 4 % of config-5 calls had one plane computed from stale rows."""
+    import torch
+    plan = psf.plan_from_case(W.config5())
+    ref = plan.compute().clone()
+    torch.cuda.synchronize()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    out = torch.empty_like(ref)
+    bad = 0
+    for it in range(200):
+        if it & 1:
+            flush.fill_(it % 251)            # every other call starts from a cold L2
+        plan.compute(out)
+        bad += int(not torch.equal(out, ref))
+    plan.destroy()
+    assert bad == 0
