@@ -375,6 +375,27 @@ __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
   return v;
 }
 
+// Fence threads of the peer (non-leader) CTA, one per stage buffer.  The peer's operand rows were written by generic-proxy
+// stores and are consumed by the pair's UMMA because of THIS signal, which crosses to the leader CTA: it must be a
+// cluster-scope release (MEMBAR.GPU).  With the default CTA-scope release about 4 % of 256-plane runs had one stage read
+// stale rows (profiles/r1j_race_k1_pair.md).  The barrier takes a fraction of a microsecond, so two threads (the fence
+// warp and the peer's idle MMA warp) take alternate stages and their barriers overlap.
+__device__ __forceinline__ void k1p_fence_peer(K1PShared &S, const K1PArgs &P, const K1PGeom &G, int buf) {
+  static_assert(K1P_NST == 2, "one fence thread per stage buffer");
+  if (!elect_one()) return;
+  const uint32_t full_leader = mapa(smem_u32(&S.full[buf]), 0);
+  int ph = 0;
+  for (int t = G.cid; t < G.ntiles; t += G.ncl) {
+    const int uses = 2 * P.C * G.nk;               // stage uses of this tile: even, so use i lands in buffer i & 1
+    for (int i = buf; i < uses; i += 2) {
+      mbar_wait(&S.written[buf], ph);
+      fence_proxy_async_smem();
+      mbar_arrive_cluster_release(full_leader);
+      ph ^= 1;
+    }
+  }
+}
+
 // TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
 __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
                                          const K1PArgs &P, const K1PGeom &G, int warp, uint32_t rank) {
@@ -399,8 +420,10 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         }
       }
     }
+  } else if (warp == 1 && !leader) {
+    k1p_fence_peer(S, P, G, 1);       // the peer CTA issues no UMMA: its warp 1 is the second fence thread (stage buffer 1)
   } else if (warp == 1) {
-    if (leader && elect_one()) {
+    if (elect_one()) {
       int st = 0, ph = 0, it = 0;
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
@@ -419,23 +442,19 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         }
       }
     }
+  } else if (warp == 2 && !leader) {
+    k1p_fence_peer(S, P, G, 0);
   } else if (warp == 2) {
-    // Fence warp.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding load of the
-    // issuing thread: issued by the producers it would drain their base-pupil prefetch at every stage.  They hand the
-    // stage over through `written` instead, and this thread (no loads in flight) fences and arrives at the leader.
+    // Fence warp of the leader.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding
+    // load of the issuing thread, so the producers hand the stage over through `written` and this thread (no loads in
+    // flight) fences and arrives.  Inside the leader's CTA the default CTA-scope release is enough.
     if (elect_one()) {
       int st = 0, ph = 0;
-      const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int i = 0; i < 2 * P.C * G.nk; ++i) {
           mbar_wait(&S.written[st], ph);
           fence_proxy_async_smem();
-          // The peer CTA's operand rows were written by generic-proxy stores and are consumed because of THIS signal:
-          // it must be a cluster-scope release (MEMBAR.GPU, ~0.25 us per stage).  With the default CTA-scope release
-          // about 4 % of 256-plane runs had one stage read stale rows (profiles/r1j_race_k1_pair.md).  The leader's own
-          // rows are handed over inside its CTA, where the CTA-scope release is enough.
-          if (leader) mbar_arrive(&S.full[st]);
-          else mbar_arrive_cluster_release(full_leader0 + st * 8);
+          mbar_arrive(&S.full[st]);
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
         }
       }
