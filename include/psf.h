@@ -44,8 +44,7 @@ typedef enum {
   PSF_OK = 0,
   PSF_ERR_INVALID_ARG = 1, /* NA<=0, NA>=n_immersion, lambda<=0, N<2, M<1, pixel<=0, n_planes<1, non-finite z,
                               noll_first<1, null pointers, misaligned outputs                                 */
-  PSF_ERR_UNSUPPORTED = 2, /* field output with PSF_POL_UNPOLARIZED, spherical path with PSF_FLAG_FRESNEL, device
-                              without sm_100                                                                   */
+  PSF_ERR_UNSUPPORTED = 2, /* field output with PSF_POL_UNPOLARIZED, device without sm_100                            */
   PSF_ERR_ALLOC = 3,       /* host or device allocation failed                                                 */
   PSF_ERR_CUDA = 4,        /* any CUDA runtime failure (message via psf_last_error)                            */
   PSF_ERR_STATE = 5        /* call order violated (e.g. shifts given for another n_planes)                     */
@@ -64,8 +63,7 @@ enum {
   PSF_FLAG_APODIZE = 1,      /* a(s) = sqrt(cos theta), Eq. 19                                     */
   PSF_FLAG_GIBSON_LANNI = 2, /* W(s) of PAPER.md:154 Eq. 16                                                     */
   PSF_FLAG_FRESNEL = 4,      /* q_s, q_p of PAPER.md:102-107 Eq. 7-8 over immersion -> glass (n_glass) -> sample,
-                                complex past a critical angle; ignored by PSF_MODEL_SCALAR; psf_spherical_prepare
-                                returns PSF_ERR_UNSUPPORTED with it                                                  */
+                                complex past a critical angle; ignored by PSF_MODEL_SCALAR                       */
   PSF_FLAG_GAUSSIAN_ENVELOPE = 8 /* a(s) *= exp(-sin^2 theta / envelope_s^2), Eq. 20              */
 };
 

@@ -351,10 +351,6 @@ psf_status psf_spherical_prepare(psf_plan *p, int n_nodes) {
   if (!p) return PSF_ERR_INVALID_ARG;
   if (n_nodes < 3 || !(n_nodes & 1) || n_nodes > (1 << 20)) { p->err = "n_nodes must be odd, >= 3 (composite Simpson)"; return PSF_ERR_INVALID_ARG; }
   if (!axisymmetric(p)) return PSF_ERR_STATE;
-  if ((p->desc.flags & PSF_FLAG_FRESNEL) && p->desc.model == PSF_MODEL_VECTORIAL) {
-    p->err = "the spherical path does not carry Fresnel coefficients yet";
-    return PSF_ERR_UNSUPPORTED;
-  }
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return bessel_setup(p, n_nodes);

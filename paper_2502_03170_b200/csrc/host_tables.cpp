@@ -241,6 +241,8 @@ void build_bessel_nodes(const psf_plan_desc &d, int n_nodes, BesselNodes &B) {
   B.sinth.resize(n_nodes);
   B.costh.resize(n_nodes);
   B.A.resize(n_nodes);
+  for (int n = 0; n < 3; ++n) B.F[n].resize(n_nodes);
+  const bool fres = (d.flags & PSF_FLAG_FRESNEL) != 0 && d.model == PSF_MODEL_VECTORIAL;
   for (int j = 0; j < n_nodes; ++j) {
     const double th = (j == n_nodes - 1) ? th_max : j * h;
     const double st = std::sin(th), ct = std::cos(th);
@@ -252,6 +254,11 @@ void build_bessel_nodes(const psf_plan_desc &d, int n_nodes, BesselNodes &B) {
     B.sinth[j] = st;
     B.costh[j] = ct;
     B.A[j] = w * a * st * e;
+    cplx qs(1, 0), qp(1, 0);
+    if (fres) fresnel_q(d, st, qs, qp);      // the phi integral of Eq. 6 with q_s, q_p kept (footnote 3 of the paper)
+    B.F[0][j] = qs + qp * ct;
+    B.F[1][j] = qp * st;
+    B.F[2][j] = qp * ct - qs;
   }
 }
 

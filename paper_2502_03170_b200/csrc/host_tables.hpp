@@ -52,6 +52,7 @@ struct BesselNodes {
   double k = 0;                    // 2 pi n_i / lambda
   std::vector<double> sinth, costh;
   std::vector<cplx> A;
+  std::vector<cplx> F[3];          // theta factors of Eq. 12-14: (q_s + q_p cos), q_p sin, (q_p cos - q_s); q = 1 without Fresnel
 };
 void build_bessel_nodes(const psf_plan_desc &d, int n_nodes, BesselNodes &out);
 

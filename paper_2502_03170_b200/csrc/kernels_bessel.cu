@@ -2,7 +2,8 @@
 // model): for axisymmetric pupils the phi integral is done in closed form and the field needs three 1-D integrals over
 // theta per (radius, plane),
 //     I_n(rho, z) = sum_j A_j f_n(theta_j) J_n(k rho sin theta_j) exp(i k z cos theta_j),     n = 0, 1, 2,
-//     f_0 = cos theta + 1,  f_1 = sin theta,  f_2 = cos theta - 1,   A_j = Simpson weight x a(theta_j) x sin theta_j x exp(i W_j)
+//     f_0 = q_s + q_p cos theta,  f_1 = q_p sin theta,  f_2 = q_p cos theta - q_s  (q_s = q_p = 1 without PSF_FLAG_FRESNEL),
+//     A_j = Simpson weight x a(theta_j) x sin theta_j x exp(i W_j)
 // (SURVEY.md §8(f) NEXT-2).  The Bessel values do not depend on the plane and the plane phasors do not depend on the
 // radius, so a thread owns one radius, evaluates J_0, J_1 (and J_2 by recurrence) once per node and feeds them to the
 // accumulators of ZC planes whose phasors sit in shared memory.  ALU / SFU bound; no tensor cores (the contraction
@@ -19,7 +20,8 @@ namespace psf {
 
 struct BesselState {
   int n_nodes = 0, R = 0;
-  void *d_nodes = nullptr;   // float4 [n]: (sin theta, cos theta, A.re, A.im)
+  void *d_nodes = nullptr;   // float  [n]: sin theta
+  void *d_af = nullptr;      // float2 [3][n]: A_j f_n(theta_j), f_n = (q_s + q_p cos), q_p sin, (q_p cos - q_s)  (scalar: A_j)
   void *d_kt = nullptr;      // float2 [n]: k cos theta / 2 pi in turns per um (hi, lo)
   void *d_kr = nullptr;      // float  [R]: k rho of the distinct radii of the folded output grid
   void *d_int = nullptr;     // float2 [Z][R][3]
@@ -36,14 +38,14 @@ constexpr int BT = 128;       // threads = radii per CTA
 
 template <bool SCALAR>
 __global__ void __launch_bounds__(BT)
-k_bessel_integrals(const float4 *__restrict__ nodes, const float2 *__restrict__ kt, const float *__restrict__ kr,
-                   const float4 *__restrict__ planes, float2 *__restrict__ out, int n_nodes, int R, int Z) {
-  __shared__ float2 Bs[BN][BZ];       // A_j exp(i k z cos theta_j) of the chunk
-  __shared__ float4 Ns[BN];           // (sin theta, f_0, f_2, unused); f_1 = sin theta
+k_bessel_integrals(const float *__restrict__ sinth, const float2 *__restrict__ af, const float2 *__restrict__ kt,
+                   const float *__restrict__ kr, const float4 *__restrict__ planes, float2 *__restrict__ out, int n_nodes, int R, int Z) {
+  constexpr int NI = SCALAR ? 1 : 3;
+  __shared__ float2 Bs[NI][BN][BZ];   // A_j f_n(theta_j) exp(i k z cos theta_j) of the chunk
+  __shared__ float Ss[BN];            // sin theta_j
   const int r = blockIdx.x * BT + threadIdx.x;
   const int z0 = blockIdx.y * BZ;
   const float x_r = r < R ? __ldg(kr + r) : 0.f;
-  constexpr int NI = SCALAR ? 1 : 3;
   float2 acc[NI][BZ];
 #pragma unroll
   for (int n = 0; n < NI; ++n)
@@ -55,26 +57,19 @@ k_bessel_integrals(const float4 *__restrict__ nodes, const float2 *__restrict__ 
     for (int i = threadIdx.x; i < BN * BZ; i += BT) {
       const int jl = i / BZ, zl = i % BZ;
       const int j = j0 + jl, z = z0 + zl;
-      float2 b = make_float2(0.f, 0.f);
-      if (j < n_nodes && z < Z) {
-        const float4 nd = __ldg(nodes + j);
+      float sn = 0.f, cs = 0.f;
+      const bool ok = j < n_nodes && z < Z;
+      if (ok) {
         const float4 pl = __ldg(planes + z);
-        const float t = kz_turns(__ldg(kt + j), pl.x, pl.y);
-        float sn, cs;
-        sincospif(2.0f * t, &sn, &cs);
-        b = make_float2(nd.z * cs - nd.w * sn, nd.z * sn + nd.w * cs);
+        sincospif(2.0f * kz_turns(__ldg(kt + j), pl.x, pl.y), &sn, &cs);
       }
-      Bs[jl][zl] = b;
-    }
-    if (threadIdx.x < BN) {
-      const int j = j0 + threadIdx.x;
-      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (j < n_nodes) {
-        const float4 nd = __ldg(nodes + j);
-        v = make_float4(nd.x, nd.y + 1.0f, nd.y - 1.0f, 0.f);
+#pragma unroll
+      for (int n = 0; n < NI; ++n) {
+        const float2 a = ok ? __ldg(af + (size_t)n * n_nodes + j) : make_float2(0.f, 0.f);
+        Bs[n][jl][zl] = make_float2(a.x * cs - a.y * sn, a.x * sn + a.y * cs);
       }
-      Ns[threadIdx.x] = v;
     }
+    if (threadIdx.x < BN) Ss[threadIdx.x] = (j0 + threadIdx.x < n_nodes) ? __ldg(sinth + j0 + threadIdx.x) : 0.f;
     __syncthreads();
     // two-level accumulation: the chunk's partial sums are added to the running totals once per chunk
     float2 part[NI][BZ];
@@ -84,28 +79,22 @@ k_bessel_integrals(const float4 *__restrict__ nodes, const float2 *__restrict__ 
       for (int z = 0; z < BZ; ++z) part[n][z] = make_float2(0.f, 0.f);
 #pragma unroll 2
     for (int jl = 0; jl < BN; ++jl) {
-      const float4 nd = Ns[jl];
-      const float x = x_r * nd.x;
-      const float J0 = j0f(x);
+      const float x = x_r * Ss[jl];
       float w[NI];
-      if (SCALAR) {
-        w[0] = J0;
-      } else {
+      w[0] = j0f(x);
+      if (!SCALAR) {
         const float J1 = j1f(x);
-        const float J2 = x > 1e-3f ? fmaf(2.0f / x, J1, -J0) : 0.125f * x * x;   // recurrence; series below 1e-3
-        w[0] = J0 * nd.y;
-        w[1 % NI] = J1 * nd.x;
-        w[2 % NI] = J2 * nd.z;
+        w[1 % NI] = J1;
+        w[2 % NI] = x > 1e-3f ? fmaf(2.0f / x, J1, -w[0]) : 0.125f * x * x;   // recurrence; series below 1e-3
       }
 #pragma unroll
-      for (int z = 0; z < BZ; ++z) {
-        const float2 b = Bs[jl][z];
+      for (int n = 0; n < NI; ++n)
 #pragma unroll
-        for (int n = 0; n < NI; ++n) {
+        for (int z = 0; z < BZ; ++z) {
+          const float2 b = Bs[n][jl][z];
           part[n][z].x = fmaf(w[n], b.x, part[n][z].x);
           part[n][z].y = fmaf(w[n], b.y, part[n][z].y);
         }
-      }
     }
 #pragma unroll
     for (int n = 0; n < NI; ++n)
@@ -177,7 +166,7 @@ __global__ void k_bessel_combine(const CombineArgs P) {
 void bessel_free(psf_plan *p) {
   BesselState *b = p->bessel;
   if (!b) return;
-  void *bufs[] = {b->d_nodes, b->d_kt, b->d_kr, b->d_int};
+  void *bufs[] = {b->d_nodes, b->d_af, b->d_kt, b->d_kr, b->d_int};
   for (void *q : bufs)
     if (q) cudaFree(q);
   delete b;
@@ -209,11 +198,15 @@ psf_status bessel_setup(psf_plan *p, int n_nodes) {
     default: break;
   }
   for (int i = 0; i < 4; ++i) b->jones[i] = (float)j[i];
-  std::vector<float4> nodes(n_nodes);
-  std::vector<float2> kt(n_nodes);
+  std::vector<float> nodes(n_nodes);
+  std::vector<float2> kt(n_nodes), af((size_t)3 * n_nodes);
   const double twopi = 6.283185307179586476925287;
   for (int i = 0; i < n_nodes; ++i) {
-    nodes[i] = make_float4((float)B.sinth[i], (float)B.costh[i], (float)B.A[i].real(), (float)B.A[i].imag());
+    nodes[i] = (float)B.sinth[i];
+    for (int n = 0; n < 3; ++n) {
+      const cplx v = b->scalar ? B.A[i] : B.A[i] * B.F[n][i];
+      af[(size_t)n * n_nodes + i] = make_float2((float)v.real(), (float)v.imag());
+    }
     const double t = B.k * B.costh[i] / twopi;
     const float hi = (float)t;
     kt[i] = make_float2(hi, (float)(t - (double)hi));
@@ -227,7 +220,7 @@ psf_status bessel_setup(psf_plan *p, int n_nodes) {
   auto up = [&](void **dst, const void *src, size_t bytes) {
     return cudaMalloc(dst, bytes) == cudaSuccess && cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
-  if (!up(&b->d_nodes, nodes.data(), nodes.size() * sizeof(float4)) || !up(&b->d_kt, kt.data(), kt.size() * sizeof(float2)) ||
+  if (!up(&b->d_nodes, nodes.data(), nodes.size() * sizeof(float)) || !up(&b->d_af, af.data(), af.size() * sizeof(float2)) || !up(&b->d_kt, kt.data(), kt.size() * sizeof(float2)) ||
       !up(&b->d_kr, kr.data(), kr.size() * sizeof(float)) ||
       cudaMalloc(&b->d_int, (size_t)d.n_planes * b->R * 3 * sizeof(float2)) != cudaSuccess) {
     p->err = "spherical path: device allocation / upload failed";
@@ -242,11 +235,11 @@ cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity) 
   const DevPlan &D = p->dp;
   dim3 g1((b->R + BT - 1) / BT, (D.Z + BZ - 1) / BZ);
   if (b->scalar)
-    k_bessel_integrals<true><<<g1, BT, 0, st>>>((const float4 *)b->d_nodes, (const float2 *)b->d_kt, (const float *)b->d_kr,
-                                                D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
+    k_bessel_integrals<true><<<g1, BT, 0, st>>>((const float *)b->d_nodes, (const float2 *)b->d_af, (const float2 *)b->d_kt,
+                                                (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
   else
-    k_bessel_integrals<false><<<g1, BT, 0, st>>>((const float4 *)b->d_nodes, (const float2 *)b->d_kt, (const float *)b->d_kr,
-                                                 D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
+    k_bessel_integrals<false><<<g1, BT, 0, st>>>((const float *)b->d_nodes, (const float2 *)b->d_af, (const float2 *)b->d_kt,
+                                                 (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
   prof_mark(p, st, 2);
   CombineArgs a;
   a.ints = (const float2 *)b->d_int; a.intensity = intensity; a.M = D.M; a.m = D.m; a.R = b->R; a.Z = D.Z;
