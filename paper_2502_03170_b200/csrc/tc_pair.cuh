@@ -45,14 +45,10 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
   return r;
 }
 // default semantics (release at CTA scope): a cluster-scope release compiles to MEMBAR.ALL.GPU + ERRBAR, microseconds per
-// arrive.  Used where the signal carries no shared-memory data written by generic-proxy stores: accumulator hand-backs
-// (TMEM reads completed by tcgen05.wait::ld + tcgen05.fence).  Operand rows written with st.shared in the peer CTA need
-// mbar_arrive_cluster_release.
+// arrive, and is not needed: accumulator hand-backs carry no memory data (TMEM reads completed by tcgen05.wait::ld +
+// tcgen05.fence), and the stage-1 operand rows are fenced for the async proxy inside their own CTA before the signal.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -112,16 +108,18 @@ constexpr int TILE16K = 128 * 128;                       // 128 rows x one 128-b
 constexpr int P_STAGE = 4 * TILE16K;                     // A hi, A lo, B-half hi, B-half lo = 64 KB per CTA
 constexpr uint32_t P_IDESC = umma_idesc_f16(256, 256);
 
-// one stage = 64 contraction indices: D += A_lo B_hi + A_hi B_lo + A_hi B_hi, four K = 16 steps
-__device__ __forceinline__ void issue_stage_mmas2(uint32_t sbase, uint32_t d_tmem, bool first) {
+// one K = 16 step of a stage: D += A_lo B_hi + A_hi B_lo + A_hi B_hi
+__device__ __forceinline__ void issue_kstep2(uint32_t sbase, uint32_t d_tmem, int k, bool zero) {
   const uint32_t ah = sbase, al = sbase + TILE16K, bh = sbase + 2 * TILE16K, bl = sbase + 3 * TILE16K;
+  const uint32_t o = k * 32;
+  umma2_f16(d_tmem, umma_desc_sw128(al + o), umma_desc_sw128(bh + o), P_IDESC, zero ? 0u : 1u);
+  umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bl + o), P_IDESC, 1u);
+  umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bh + o), P_IDESC, 1u);
+}
+// one stage = 64 contraction indices = four K = 16 steps
+__device__ __forceinline__ void issue_stage_mmas2(uint32_t sbase, uint32_t d_tmem, bool first) {
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    const uint32_t o = k * 32;
-    umma2_f16(d_tmem, umma_desc_sw128(al + o), umma_desc_sw128(bh + o), P_IDESC, (first && k == 0) ? 0u : 1u);
-    umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bl + o), P_IDESC, 1u);
-    umma2_f16(d_tmem, umma_desc_sw128(ah + o), umma_desc_sw128(bh + o), P_IDESC, 1u);
-  }
+  for (int k = 0; k < 4; ++k) issue_kstep2(sbase, d_tmem, k, first && k == 0);
 }
 
 // ---- stage 2 ----------------------------------------------------------------------------------------------------------
@@ -345,6 +343,7 @@ struct K1PArgs {
 };
 
 constexpr int K1P_NST = 2;
+constexpr int K1P_DEFER = 1;                                      // K = 16 steps of the next stage issued before a stage buffer is released
 constexpr int K1P_PRODUCER_WARPS = 8;
 constexpr int K1P_FEED_WARPS = 4;                                  // table TMA, MMA, fence, base-pupil copies: roles fill whole warpgroups (setmaxnreg)
 constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
@@ -375,27 +374,6 @@ __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
   return v;
 }
 
-// Fence threads of the peer (non-leader) CTA, one per stage buffer.  The peer's operand rows were written by generic-proxy
-// stores and are consumed by the pair's UMMA because of THIS signal, which crosses to the leader CTA: it must be a
-// cluster-scope release (MEMBAR.GPU).  With the default CTA-scope release about 4 % of 256-plane runs had one stage read
-// stale rows (profiles/r1j_race_k1_pair.md).  The barrier takes a fraction of a microsecond, so two threads (the fence
-// warp and the peer's idle MMA warp) take alternate stages and their barriers overlap.
-__device__ __forceinline__ void k1p_fence_peer(K1PShared &S, const K1PArgs &P, const K1PGeom &G, int buf) {
-  static_assert(K1P_NST == 2, "one fence thread per stage buffer");
-  if (!elect_one()) return;
-  const uint32_t full_leader = mapa(smem_u32(&S.full[buf]), 0);
-  int ph = 0;
-  for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-    const int uses = 2 * P.C * G.nk;               // stage uses of this tile: even, so use i lands in buffer i & 1
-    for (int i = buf; i < uses; i += 2) {
-      mbar_wait(&S.written[buf], ph);
-      fence_proxy_async_smem();
-      mbar_arrive_cluster_release(full_leader);
-      ph ^= 1;
-    }
-  }
-}
-
 // TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
 __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
                                          const K1PArgs &P, const K1PGeom &G, int warp, uint32_t rank) {
@@ -420,11 +398,9 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         }
       }
     }
-  } else if (warp == 1 && !leader) {
-    k1p_fence_peer(S, P, G, 1);       // the peer CTA issues no UMMA: its warp 1 is the second fence thread (stage buffer 1)
   } else if (warp == 1) {
-    if (elect_one()) {
-      int st = 0, ph = 0, it = 0;
+    if (leader && elect_one()) {
+      int st = 0, ph = 0, it = 0, pending = -1;
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
           const int g = cg & 1;
@@ -434,27 +410,37 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
           for (int kc = 0; kc < G.nk; ++kc) {
             mbar_wait(&S.full[st], ph);
             tcgen05_fence_after();
-            issue_stage_mmas2(smem_u32(smem + st * P_STAGE), d, kc == 0);
-            umma2_commit(&S.empty[st]);
+            const uint32_t sb = smem_u32(smem + st * P_STAGE);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              issue_kstep2(sb, d, k, kc == 0 && k == 0);
+              // Deferred release (profiles/r1j_race_k1_pair.md): the commit tracks the UMMAs of the issuing (leader) CTA; in
+              // the peer, whose tensor core can trail by a little, producers with their rows ready in registers
+              // overwrote the operand tile while it was still being read.  The previous stage's buffer is therefore
+              // released only after K1P_DEFER K-steps of this stage have been issued behind it: the commit then also
+              // waits for those, which gives the peer that much tensor time of slack.
+              if (k == K1P_DEFER - 1 && pending >= 0) { umma2_commit(&S.empty[pending]); pending = -1; }
+            }
+            pending = st;
             if (++st == K1P_NST) { st = 0; ph ^= 1; }
           }
           umma2_commit(&S.acc_full[g]);
         }
       }
+      if (pending >= 0) umma2_commit(&S.empty[pending]);
     }
-  } else if (warp == 2 && !leader) {
-    k1p_fence_peer(S, P, G, 0);
   } else if (warp == 2) {
-    // Fence warp of the leader.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding
-    // load of the issuing thread, so the producers hand the stage over through `written` and this thread (no loads in
-    // flight) fences and arrives.  Inside the leader's CTA the default CTA-scope release is enough.
+    // Fence warp.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding load of the
+    // issuing thread, so the hand-over of a stage goes through `written` to this thread (no loads in flight), which
+    // fences and arrives at the leader's `full` barrier.
     if (elect_one()) {
       int st = 0, ph = 0;
+      const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int i = 0; i < 2 * P.C * G.nk; ++i) {
           mbar_wait(&S.written[st], ph);
           fence_proxy_async_smem();
-          mbar_arrive(&S.full[st]);
+          mbar_arrive_cluster(full_leader0 + st * 8);
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
         }
       }
