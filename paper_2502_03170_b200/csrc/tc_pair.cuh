@@ -345,7 +345,7 @@ struct K1PArgs {
 constexpr int K1P_NST = 2;
 constexpr int K1P_DEFER = 1;                                      // K = 16 steps of the next stage issued before a stage buffer is released
 constexpr int K1P_PRODUCER_WARPS = 8;
-constexpr int K1P_FEED_WARPS = 4;                                  // table TMA, MMA, fence, base-pupil copies: roles fill whole warpgroups (setmaxnreg)
+constexpr int K1P_FEED_WARPS = 4;                                  // table TMA, MMA, idle, base-pupil copies: roles fill whole warpgroups (setmaxnreg)
 constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
 constexpr int K1P_STAGING = 2 * TILE16K;                          // hi tile + lo tile of one chain: 128 mx x 64 qy each
 constexpr int K1P_BB_SLOTS = 2;
@@ -356,7 +356,6 @@ constexpr int K1P_QY = 64;                                        // q_y per til
 
 struct K1PShared {
   uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
-  uint64_t written[K1P_NST];    // producer warps -> fence warp: the B-operand rows of the stage are in shared memory
   uint64_t bb_full[K1P_BB_SLOTS], bb_empty[K1P_BB_SLOTS];   // base-pupil ring: bulk copy -> producers -> free
   uint32_t tmem_slot;
 };
@@ -429,22 +428,6 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
       }
       if (pending >= 0) umma2_commit(&S.empty[pending]);
     }
-  } else if (warp == 2) {
-    // Fence warp.  fence.proxy.async carries a CTA-wide memory barrier that waits for every outstanding load of the
-    // issuing thread, so the hand-over of a stage goes through `written` to this thread (no loads in flight), which
-    // fences and arrives at the leader's `full` barrier.
-    if (elect_one()) {
-      int st = 0, ph = 0;
-      const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
-      for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-        for (int i = 0; i < 2 * P.C * G.nk; ++i) {
-          mbar_wait(&S.written[st], ph);
-          fence_proxy_async_smem();
-          mbar_arrive_cluster(full_leader0 + st * 8);
-          if (++st == K1P_NST) { st = 0; ph ^= 1; }
-        }
-      }
-    }
   } else if (warp == 3) {
     // Base-pupil copies: one 32 KB bulk copy per stage (the table is stored in the producers' read order, so a stage
     // of this CTA is one contiguous block) into a two-slot ring.  The producers then only read shared memory: no
@@ -478,6 +461,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
   // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
   const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
   const uint32_t smem0 = smem_u32(smem);
+  const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
   const uint32_t ring = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // [slot][sample e][thread] float4
   int st = 0, ph = 0, bs = 0, bph = 0;
   float4 sc[K1P_MAX_NK][4];                                      // (cos, sin) of samples (2i, 2i+1) of k-chunk kc
@@ -504,9 +488,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
               const float t1 = 6.283185307179586f * kz_turns(make_float2(kt[i].z, kt[i].w), pl.x, pl.y);
               sc[kc][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
             }
-            if (kc + 1 < G.nk) load_kt(jt, kc + 1);              // one stage ahead
           }
-          if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
           mbar_wait(&S.bb_full[bs], bph);
           uint32_t hi[4][4], lo[4][4];                             // [slot][pair of q_x]
 #pragma unroll
@@ -529,10 +511,14 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
             st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
             st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
           }
-          fence_proxy_async_smem();                                // every writer fences its own stores (no loads are in flight here)
+          fence_proxy_async_smem();                                // every writer fences its own stores; no load is in flight here
           __syncwarp();
-          if (lane == 0) mbar_arrive(&S.written[st]);
+          if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
+          // kappa of the stage that computes phasors next (one stage ahead), issued after the fence so that the fence's
+          // memory barrier never waits for it
+          if (cg == 0 && kc + 1 < G.nk) load_kt(jt, kc + 1);
+          if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
         }
       }
     }
@@ -622,9 +608,8 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < K1P_NST; ++i) {
-      mbar_init(&S.full[i], 1 + 2);                       // the leader's expect_tx arrive + the fence warp of each CTA
+      mbar_init(&S.full[i], 1 + 2 * K1P_PRODUCER_WARPS);  // the leader's expect_tx arrive + every producer warp of the pair
       mbar_init(&S.empty[i], 1);
-      mbar_init(&S.written[i], K1P_PRODUCER_WARPS);
     }
     for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S.bb_full[i], 1); mbar_init(&S.bb_empty[i], K1P_PRODUCER_WARPS); }
     for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
