@@ -39,7 +39,8 @@ constexpr int BT = 128;       // threads = radii per CTA
 template <bool SCALAR>
 __global__ void __launch_bounds__(BT)
 k_bessel_integrals(const float *__restrict__ sinth, const float2 *__restrict__ af, const float2 *__restrict__ kt,
-                   const float *__restrict__ kr, const float4 *__restrict__ planes, float2 *__restrict__ out, int n_nodes, int R, int Z) {
+                   const float *__restrict__ kr, const float4 *__restrict__ planes, float2 *__restrict__ out, int n_nodes, int R, int Z,
+                   int chunks_per_split) {
   constexpr int NI = SCALAR ? 1 : 3;
   __shared__ float2 Bs[NI][BN][BZ];   // A_j f_n(theta_j) exp(i k z cos theta_j) of the chunk
   __shared__ float Ss[BN];            // sin theta_j
@@ -52,7 +53,10 @@ k_bessel_integrals(const float *__restrict__ sinth, const float2 *__restrict__ a
 #pragma unroll
     for (int z = 0; z < BZ; ++z) acc[n][z] = make_float2(0.f, 0.f);
 
-  for (int j0 = 0; j0 < n_nodes; j0 += BN) {
+  // small grids: the node range is split over gridDim.z CTAs whose partial sums meet in `out` by atomic adds
+  const int j_begin = blockIdx.z * chunks_per_split * BN;
+  const int j_end = min(n_nodes, j_begin + chunks_per_split * BN);
+  for (int j0 = j_begin; j0 < j_end; j0 += BN) {
     __syncthreads();
     for (int i = threadIdx.x; i < BN * BZ; i += BT) {
       const int jl = i / BZ, zl = i % BZ;
@@ -106,8 +110,13 @@ k_bessel_integrals(const float *__restrict__ sinth, const float2 *__restrict__ a
     for (int z = 0; z < BZ; ++z)
       if (z0 + z < Z) {
         float2 *o = out + ((size_t)(z0 + z) * R + r) * 3;
+        if (gridDim.z == 1) {
 #pragma unroll
-        for (int n = 0; n < NI; ++n) o[n] = acc[n][z];
+          for (int n = 0; n < NI; ++n) o[n] = acc[n][z];
+        } else {
+#pragma unroll
+          for (int n = 0; n < NI; ++n) { atomicAdd(&o[n].x, acc[n][z].x); atomicAdd(&o[n].y, acc[n][z].y); }
+        }
       }
   }
 }
@@ -234,12 +243,20 @@ cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity) 
   const BesselState *b = p->bessel;
   const DevPlan &D = p->dp;
   dim3 g1((b->R + BT - 1) / BT, (D.Z + BZ - 1) / BZ);
+  // fewer CTAs than two per SM: split the Simpson nodes across gridDim.z (partial sums by atomic adds into a zeroed scratch)
+  const int chunks = (b->n_nodes + BN - 1) / BN;
+  int split = (2 * p->sm_count + (int)(g1.x * g1.y) - 1) / (int)(g1.x * g1.y);
+  if (split > chunks) split = chunks;
+  if (split < 1) split = 1;
+  const int per = (chunks + split - 1) / split;
+  g1.z = (chunks + per - 1) / per;
+  if (g1.z > 1) cudaMemsetAsync(b->d_int, 0, (size_t)D.Z * b->R * 3 * sizeof(float2), st);
   if (b->scalar)
     k_bessel_integrals<true><<<g1, BT, 0, st>>>((const float *)b->d_nodes, (const float2 *)b->d_af, (const float2 *)b->d_kt,
-                                                (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
+                                                (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z, per);
   else
     k_bessel_integrals<false><<<g1, BT, 0, st>>>((const float *)b->d_nodes, (const float2 *)b->d_af, (const float2 *)b->d_kt,
-                                                 (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z);
+                                                 (const float *)b->d_kr, D.planes, (float2 *)b->d_int, b->n_nodes, b->R, D.Z, per);
   prof_mark(p, st, 2);
   CombineArgs a;
   a.ints = (const float2 *)b->d_int; a.intensity = intensity; a.M = D.M; a.m = D.m; a.R = b->R; a.Z = D.Z;
