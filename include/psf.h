@@ -127,7 +127,9 @@ psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
  *   intensity : device fp32 [n_planes][M][M], x fastest (required);
  *   field     : device complex64 (interleaved re, im) [3][n_planes][M][M] = (E_x, E_y, E_z), or NULL
  *               ([1][n_planes][M][M] for PSF_MODEL_SCALAR).
- * Asynchronous; results are valid once the stream has passed this point. */
+ * Asynchronous; results are valid once the stream has passed this point.  One exception to "only enqueues": on a plan
+ * that runs on the tensor cores, the first call with field != NULL after a table refresh first uploads the tables of
+ * the FFMA kernels that write the field (a synchronous copy). */
 psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void *field);
 
 /* Spherical (Bessel) parametrisation of the same integral, Eq. 11-14 (Eq. 5 for PSF_MODEL_SCALAR):

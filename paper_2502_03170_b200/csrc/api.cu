@@ -40,6 +40,17 @@ psf_status upload(psf_plan *p, void **dptr, size_t *cap, const std::vector<T> &h
 // (hi, lo) float pair of a double
 inline void split2(double v, float &hi, float &lo) { hi = (float)v; lo = (float)(v - (double)hi); }
 
+// Device copies of the folded base pupil and kappa table of the FFMA kernels, from the plan's host copies.
+psf_status upload_ffma_tables(psf_plan *p) {
+  psf_status s;
+  if ((s = upload(p, &p->d_bfold, &p->cap_bfold, p->h_bfold)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_kt, &p->cap_kt, p->h_kt)) != PSF_OK) return s;
+  p->dp.bfold = (const float4 *)p->d_bfold;
+  p->dp.kt = (const float2 *)p->d_kt;
+  p->ffma_stale = false;
+  return PSF_OK;
+}
+
 // Folds the static pupil about both axes into the four parity classes and uploads every static table.
 psf_status upload_static(psf_plan *p) {
   const psf_plan_desc &d = p->desc;
@@ -92,11 +103,13 @@ psf_status upload_static(psf_plan *p) {
   }
   tm.mark("fold");
   psf_status s;
-  if ((s = upload(p, &p->d_bfold, &p->cap_bfold, bfold)) != PSF_OK) return s;
-  if ((s = upload(p, &p->d_kt, &p->cap_kt, kt)) != PSF_OK) return s;
+  // The folded tables feed the FFMA kernels.  A plan on the tensor path needs them only for a field output, so their
+  // upload (10 MB at N = 512) is left to the first such psf_compute after a refresh.
+  const bool tensor_path = d.precision != PSF_PREC_FP32 && !P.per_plane &&
+                           (d.precision == PSF_PREC_3XTF32 || d.precision == PSF_PREC_3XF16 || tc_eligible(p));
+  p->ffma_stale = tensor_path;
+  if (!tensor_path && (s = upload_ffma_tables(p)) != PSF_OK) return s;
   tm.mark("upload bfold, kt");
-  P.bfold = (const float4 *)p->d_bfold;
-  P.kt = (const float2 *)p->d_kt;
 
   if (P.per_plane) {
     std::vector<float2> bunf((size_t)C * NN);
@@ -331,6 +344,11 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool tc = (p->path == 1 || p->path == 2) && !field;
+  if (!tc && p->ffma_stale) {                  // first field output of a tensor-path plan since the last table refresh
+    if (cudaSetDevice(p->device) != cudaSuccess) { p->err = "cudaSetDevice failed"; return PSF_ERR_CUDA; }
+    const psf_status us = upload_ffma_tables(p);
+    if (us != PSF_OK) return us;
+  }
   cudaError_t e = tc ? launch_tc(p, st, intensity)
                      : (p->path == 3 || small_eligible(p)) ? launch_small(p, st, intensity, (float2 *)field)
                                                             : launch_ffma(p, st, intensity, (float2 *)field);

@@ -81,6 +81,7 @@ struct psf_plan {
   psf::TcState *tc = nullptr;
   psf::BesselState *bessel = nullptr;
   psf::GradState *grad = nullptr;
+  bool ffma_stale = false;       // tensor-path plan: the FFMA tables on the device are older than the host copies
   long long table_version = 0;   // bumped by every table refresh (psf_set_*): derived copies check it
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
