@@ -44,6 +44,7 @@ def plane_errors(I_gpu, I_ref):
 
 
 PRECISIONS = ["fp32", "auto", "3xtf32", "3xf16"]
+_ORACLE_CACHE = {}
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
@@ -95,14 +96,15 @@ def test_config4_all_emitters(psf, precision):
 
 @pytest.mark.parametrize("precision", PRECISIONS)
 def test_config5_sampled_planes_and_voxels(psf, precision):
-    """Full BASELINE size in the launch configuration bench.py times; the oracle covers 6 full planes (T2) and
-    4096 seeded voxels over all 256 planes (T1)."""
+    """Full BASELINE size in the launch configuration bench.py times; the oracle covers every voxel of all 256 planes
+    (T2, computed once for the module) and 4096 seeded voxels by the literal sum (T1)."""
     case = W.config5()
     I, path = gpu_stack(psf, case, precision)
-    planes = [0, 37, 101, 128, 200, 255]
-    ref = O.stack_T2(case, planes)
-    rel = plane_errors(I[planes], ref)
-    assert rel.max() <= TOL, (path, rel)
+    if "cfg5" not in _ORACLE_CACHE:
+        _ORACLE_CACHE["cfg5"] = O.stack_T2(case)
+    ref = _ORACLE_CACHE["cfg5"]
+    rel = plane_errors(I, ref)
+    assert rel.max() <= TOL, (path, rel.max(), int(rel.argmax()))
     rng = np.random.default_rng(5)
     b = rng.integers(0, 256, 4096)
     iy, ix = rng.integers(0, 512, 4096), rng.integers(0, 512, 4096)
