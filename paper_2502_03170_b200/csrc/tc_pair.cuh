@@ -350,7 +350,7 @@ constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
 constexpr int K1P_STAGING = 2 * TILE16K;                          // hi tile + lo tile of one chain: 128 mx x 64 qy each
 constexpr int K1P_BB_SLOTS = 2;
 constexpr int K1P_BB_BYTES = 8 * 256 * 16;                        // one stage of base pupil for this CTA: 8 samples x 256 threads x float4
-constexpr int K1P_MAX_NK = 4;                                     // the producers keep the defocus phasors of a tile in registers: n_pad <= 256
+constexpr int K1P_MAX_NK = 4;                                     // k-chunks whose defocus phasors the producers keep in registers per tile (n_pad <= 256)
 constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + K1P_STAGING + K1P_BB_SLOTS * K1P_BB_BYTES;
 constexpr int K1P_QY = 64;                                        // q_y per tile (32 generated by each CTA)
 
@@ -464,7 +464,8 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
   const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
   const uint32_t ring = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // [slot][sample e][thread] float4
   int st = 0, ph = 0, bs = 0, bph = 0;
-  float4 sc[K1P_MAX_NK][4];                                      // (cos, sin) of samples (2i, 2i+1) of k-chunk kc
+  float4 sc[K1P_MAX_NK][4];                                      // (cos, sin) of samples (2i, 2i+1) of k-chunk kc (mod 4)
+  const bool cached = G.nk <= K1P_MAX_NK;                        // larger pupils recompute the phasors at every stage
   float4 kt[4];
   // kappa of (tile, kc): [jt][kc][half][4 sample pairs][256 threads] float4
   auto load_kt = [&](int jt, int kc) {
@@ -478,15 +479,17 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
     const int jt = r % G.tiles_j;
     const float4 pl = __ldg(P.planes + P.z0 + r / G.tiles_j);
     for (int cg = 0; cg < 2 * P.C; ++cg) {
+     for (int kcb = 0; kcb < G.nk; kcb += K1P_MAX_NK) {
 #pragma unroll
-      for (int kc = 0; kc < K1P_MAX_NK; ++kc) {
+      for (int k4 = 0; k4 < K1P_MAX_NK; ++k4) {
+        const int kc = kcb + k4;
         if (kc < G.nk) {
-          if (cg == 0) {
+          if (cg == 0 || !cached) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const float t0 = 6.283185307179586f * kz_turns(make_float2(kt[i].x, kt[i].y), pl.x, pl.y);
               const float t1 = 6.283185307179586f * kz_turns(make_float2(kt[i].z, kt[i].w), pl.x, pl.y);
-              sc[kc][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
+              sc[k4][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
             }
           }
           mbar_wait(&S.bb_full[bs], bph);
@@ -495,7 +498,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           for (int i = 0; i < 4; ++i) {
             const float4 b0 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i) * 4096);
             const float4 b1 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i + 1) * 4096);
-            const float cs0 = sc[kc][i].x, sn0 = sc[kc][i].y, cs1 = sc[kc][i].z, sn1 = sc[kc][i].w;
+            const float cs0 = sc[k4][i].x, sn0 = sc[k4][i].y, cs1 = sc[k4][i].z, sn1 = sc[k4][i].w;
             split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
             split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
             split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
@@ -517,10 +520,19 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
           // kappa of the stage that computes phasors next (one stage ahead), issued after the fence so that the fence's
           // memory barrier never waits for it
-          if (cg == 0 && kc + 1 < G.nk) load_kt(jt, kc + 1);
-          if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+          if (cached) {
+            if (cg == 0 && kc + 1 < G.nk) load_kt(jt, kc + 1);
+            if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+          } else if (kc + 1 < G.nk) {
+            load_kt(jt, kc + 1);
+          } else if (cg + 1 < 2 * P.C) {
+            load_kt(jt, 0);
+          } else if (t + G.ncl < G.ntiles) {
+            load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+          }
         }
       }
+     }
     }
   }
 }

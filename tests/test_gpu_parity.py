@@ -143,7 +143,7 @@ def test_shared_zernike_static_path_odd_sizes(psf, precision):
                                             (52, 130, 511, 2, W.POL_CIRC_L),          # odd M: self-mirror row and column
                                             (53, 512, 258, 5, W.POL_X),               # m = 129 (pad 256): a nearly empty CTA
                                             (54, 257, 1023, 1, W.POL_UNPOLARIZED),    # m = 512: two pair tiles per plane
-                                            (55, 640, 512, 2, W.POL_UNPOLARIZED)])    # n_pad = 320 > 256: stage 1 on single-CTA tiles, stage 2 on pairs
+                                            (55, 640, 512, 2, W.POL_UNPOLARIZED)])    # n_pad = 320 > 256: stage-1 producers recompute the phasors per stage
 def test_cta_pair_kernels_ragged_sizes(psf, seed, N, M, Z, pol):
     """The cta_group::2 kernels (3xFP16 path, output half-size padded to whole pairs of 128 rows) on sizes that leave
     padding in every tile dimension, against the separable fp64 oracle, every voxel."""
