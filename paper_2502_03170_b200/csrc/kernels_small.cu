@@ -5,7 +5,9 @@
 //
 //   phase 0 : per folded pupil sample, the plane's phasors exp(2 pi i t) at its four mirror images
 //             (defocus kappa z, per-plane Zernike row, tilt); the Zernike basis is stored folded and sorted by
-//             parity, so the four mirror phases cost K loads + K FMAs, not 4K; phasors go to shared memory.
+//             parity, so the four mirror phases cost K loads + K FMAs, not 4K; in per-plane mode the phasors stay in
+//             the registers of the thread that made them (it is the only reader), which leaves 54 KB of shared memory
+//             per CTA and four CTAs per SM.
 //   per scalar pupil c:
 //     Q       : base pupil x phasor at the four mirrors, folded into the 8 real chains   -> Qs[qy][qx][8]
 //     stage 1 : T_j[qy, mx] = sum_qx Q_j[qy, qx] X_j[mx, qx]   (thread tile 8 chains x 4 mx)   -> Ts[qy][half][mx][4]
@@ -22,12 +24,12 @@ constexpr int SM_THREADS = 128;
 constexpr int NQ = 32;                 // folded pupil samples per axis held by a CTA
 constexpr int QS_ROW = NQ * 8 + 4;     // floats per q_y row of Qs (+4 shifts consecutive rows by one 16-byte bank group)
 
-template <int MQ>
+template <int MQ, bool PER_PLANE>
 struct SmallSmem {
   float Qs[NQ][QS_ROW];                // [qy][qx][8 chains]
   float Ts[NQ][2 * MQ * 4 + 4];        // [qy][chains 0-3 | 4-7][mx][4]
+  float2 Ph0[PER_PLANE ? 2 : NQ * NQ]; // static mode: one phasor per sample, kept here (small code: tiny stacks start cold)
   float Xc[NQ][MQ], Xs[NQ][MQ];        // cos / sin of k s_max u_q x_m, [q][m]; serves both stages (square grids)
-  float2 Ph[4][NQ * NQ];               // phasors (cos, sin) per mirror image [ymirror * 2 + xmirror][qy * 32 + qx]
 };
 
 __device__ __forceinline__ void sincos_turns(float t, float &sn, float &cs) {
@@ -38,9 +40,9 @@ __device__ __forceinline__ void sincos_turns(float t, float &sn, float &cs) {
 }
 
 template <int MQ, bool PER_PLANE, bool FIELD>
-__global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__restrict__ I, float2 *__restrict__ field) {
+__global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const DevPlan P, float *__restrict__ I, float2 *__restrict__ field) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  SmallSmem<MQ> &S = *reinterpret_cast<SmallSmem<MQ> *>(smem_raw);
+  SmallSmem<MQ, PER_PLANE> &S = *reinterpret_cast<SmallSmem<MQ, PER_PLANE> *>(smem_raw);
   const int tid = threadIdx.x;
   const int b = blockIdx.x;
   const int n = P.n, m = P.m, N = P.N, M = P.M;
@@ -54,7 +56,10 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
 
   // ---- phase 0: phasors -------------------------------------------------------------------------------------------
   const float4 pl = __ldg(P.planes + b);
-#pragma unroll 2
+  // phasors (cos, sin) of this thread's 8 samples at their (up to) four mirror images, kept in registers: a thread reads
+  // back only the phasors it wrote, and without the 32 KB they took in shared memory more CTAs fit an SM
+  float2 phr[PER_PLANE ? (NQ * NQ) / SM_THREADS : 1][PER_PLANE ? 4 : 1];
+#pragma unroll (PER_PLANE ? 8 : 2)
   for (int r = 0; r < (NQ * NQ) / SM_THREADS; ++r) {
     const int f = tid + SM_THREADS * r;
     const int qy = f >> 5, qx = f & 31;
@@ -90,8 +95,12 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
         sincos_turns(t0, ph[0].y, ph[0].x);
       }
     }
-    S.Ph[0][f] = ph[0];
-    if (PER_PLANE) { S.Ph[1][f] = ph[1]; S.Ph[2][f] = ph[2]; S.Ph[3][f] = ph[3]; }
+    if (PER_PLANE) {
+      phr[PER_PLANE ? r : 0][0] = ph[0];
+      phr[PER_PLANE ? r : 0][1 % (PER_PLANE ? 4 : 1)] = ph[1]; phr[PER_PLANE ? r : 0][2 % (PER_PLANE ? 4 : 1)] = ph[2]; phr[PER_PLANE ? r : 0][3 % (PER_PLANE ? 4 : 1)] = ph[3];
+    } else {
+      S.Ph0[PER_PLANE ? 0 : f] = ph[0];
+    }
   }
 
   constexpr int PASS1 = MQ / 16;                 // stage-1 passes over m_x groups of 4 (4 groups per pass)
@@ -107,7 +116,7 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
   for (int c = 0; c < P.C; ++c) {
     __syncthreads();                             // Qs / Ts of the previous component are free (and the tables are in)
     // ---- Q: base pupil x phasor, folded (a thread reads back only the phasors it wrote) ----
-#pragma unroll 2
+#pragma unroll (PER_PLANE ? 8 : 2)
     for (int r = 0; r < (NQ * NQ) / SM_THREADS; ++r) {
       const int f = tid + SM_THREADS * r;
       const int qy = f >> 5, qx = f & 31;
@@ -122,7 +131,7 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
 #pragma unroll
             for (int bb = 0; bb < 2; ++bb) {
               const float2 bu = __ldg(B + (size_t)(a ? ry : qy) * N + (bb ? rx : qx));
-              const float2 e = S.Ph[a * 2 + bb][f];
+              const float2 e = phr[PER_PLANE ? r : 0][(a * 2 + bb) % (PER_PLANE ? 4 : 1)];
               v[a][bb] = make_float2(bu.x * e.x - bu.y * e.y, bu.x * e.y + bu.y * e.x);
             }
           if (rx == qx) { v[0][1] = make_float2(0.f, 0.f); v[1][1] = make_float2(0.f, 0.f); }   // odd N: self-mirror column
@@ -139,7 +148,7 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
         } else {
           const size_t s = ((size_t)c * n * n + (size_t)qy * n + qx) * 2;
           const float4 b0 = __ldg(P.bfold + s), b1 = __ldg(P.bfold + s + 1);
-          const float2 e = S.Ph[0][f];
+          const float2 e = S.Ph0[PER_PLANE ? 0 : f];
           o[0] = b0.x * e.x - b0.y * e.y;  o[1] = b0.x * e.y + b0.y * e.x;
           o[2] = b0.z * e.x - b0.w * e.y;  o[3] = b0.z * e.y + b0.w * e.x;
           o[4] = b1.x * e.x - b1.y * e.y;  o[5] = b1.x * e.y + b1.y * e.x;
@@ -284,7 +293,7 @@ __global__ void __launch_bounds__(SM_THREADS) k_small(const DevPlan P, float *__
 template <int MQ, bool PP, bool FIELD>
 cudaError_t launch_one(const DevPlan &P, cudaStream_t st, float *intensity, float2 *field) {
   static bool attr_set = false;
-  const int bytes = (int)sizeof(SmallSmem<MQ>);
+  const int bytes = (int)sizeof(SmallSmem<MQ, PP>);
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_small<MQ, PP, FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e != cudaSuccess) return e;
