@@ -33,10 +33,10 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 # (profiles/*.md name the command); keyed by (path, workload, stage), in bytes PER PLANE of the captured launch (scaled to
 # the mean planes per launch below).  None where no capture exists yet.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1l_ncu_pair_cfg5.md: k2_pair, 256-plane launch: 2.705 GB read + 0.260 GB written
-    ("tc3xf16", "cfg5_large_stack", 1): (2.705396e9 + 0.260451e9) / 256,
-    # same capture, k1_pair: 0.156 GB read + 2.624 GB written
-    ("tc3xf16", "cfg5_large_stack", 0): (0.155723e9 + 2.623920e9) / 256,
+    # profiles/r1m_ncu_pair_cfg5.md: k2_pair, 256-plane launch: 2.705 GB read + 0.261 GB written
+    ("tc3xf16", "cfg5_large_stack", 1): (2.705340e9 + 0.260985e9) / 256,
+    # same capture, k1_pair: 0.156 GB read + 2.626 GB written
+    ("tc3xf16", "cfg5_large_stack", 0): (0.155747e9 + 2.625637e9) / 256,
 }
 
 
