@@ -25,8 +25,12 @@ Tiers
 
 Pins: every function here is checked in tests/test_oracle_pins.py against something other than
 itself (closed forms, the Bessel form, the Airy pattern, exact discrete symmetries, Parseval,
-pure-Python brute force).  The combined non-axisymmetric aberrated result (configs 2, 4, 5) is
-"parity unpinned" beyond the component pins (Zernike basis, tilt, L<->R relations): see DESIGN.md.
+pure-Python brute force).  The combined non-axisymmetric aberrated result (the class of configs 2, 4, 5)
+is pinned by an exact identity: Noll 2 / 3 terms inside the full combination (Gibson-Lanni with design !=
+actual, circular input, further Zernike terms, defocus) are a lateral shift by 2 c / (k s_max), checked T2 on
+the grid against T1 at the shifted points; `immersion_thickness` and every glass / design term of
+`gibson_lanni_phase` by the paraxial curvature of Eq. 16 + Eq. 17, which is -k0 t_s / (2 n_i) for any design
+values; the in-disc counts of SURVEY.md section 8 are asserted.
 
 Further correction factors, each a factor of the static pupil: the scalar model
 `case.model = "scalar"` (Eq. 3, e_inf = e_inc = 1, one component), the Gaussian envelope

@@ -86,12 +86,13 @@ def test_config4_all_emitters(psf, precision):
     ref = O.stack_T2(case.with_planes(idx))
     rel = plane_errors(I[idx], ref)
     assert rel.max() <= TOL, (path, rel.max())
-    rng = np.random.default_rng(4)                 # ... and 4096 random voxels over all emitters through T1
-    b = rng.integers(0, 4096, 4096)
+    rng = np.random.default_rng(4)                 # ... and 4096 random voxels of those emitters through T1
     iy, ix = rng.integers(0, 32, 4096), rng.integers(0, 32, 4096)
+    b = idx[rng.integers(0, len(idx), 4096)]       # (their oracle plane peaks are known from T2 above)
     v1 = O.voxel_intensity(case, b, iy, ix)
-    peaks = I.reshape(4096, -1).max(axis=1)[b]
-    assert (np.abs(I[b, iy, ix] - v1) / peaks).max() <= 1.5 * TOL
+    peak_of = np.zeros(4096)
+    peak_of[idx] = ref.reshape(len(idx), -1).max(axis=1)
+    assert (np.abs(I[b, iy, ix] - v1) / peak_of[b]).max() <= TOL
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
@@ -109,8 +110,8 @@ def test_config5_sampled_planes_and_voxels(psf, precision):
     b = rng.integers(0, 256, 4096)
     iy, ix = rng.integers(0, 512, 4096), rng.integers(0, 512, 4096)
     v1 = O.voxel_intensity(case, b, iy, ix)
-    peaks = I.reshape(256, -1).max(axis=1)[b]       # plane peaks of the GPU stack (within 2e-5 of the oracle's on the checked planes)
-    assert (np.abs(I[b, iy, ix] - v1) / peaks).max() <= 1.5 * TOL
+    peaks = ref.reshape(256, -1).max(axis=1)[b]     # plane peaks of the oracle stack
+    assert (np.abs(I[b, iy, ix] - v1) / peaks).max() <= TOL
     # property valid at any size: unpolarised intensity is symmetric under (x,y) -> (-x,-y) only without Zernike;
     # with it, check positivity and finiteness of every voxel instead
     assert np.isfinite(I).all() and (I >= 0).all()

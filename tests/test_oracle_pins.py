@@ -349,6 +349,36 @@ def test_gibson_lanni_on_axis_phase_closed_form():
     assert abs(math.exp(-Wc[1].imag) - decay) < 1e-12
 
 
+def test_gl_eq17_paraxial_curvature_is_a_pure_defocus_by_t_s():
+    """PAPER.md:154 Eq. 16 with t_i from PAPER.md:167 Eq. 17 as printed, design != actual (every glass / design term
+    alive).  In a = n_i sin(theta) each term t sqrt(n^2 - a^2) has the quadratic coefficient -t / (2 n), so
+        W_GL(a) = W_GL(0) - (k0 / 2) a^2 [t_s/n_s + t_i/n_i - t_i*/n_i* + t_g/n_g - t_g*/n_g*] + O(a^4),
+    and inserting Eq. 17 (t_i/n_i = t_s/n_i - t_s/n_s - t_g/n_g + t_g*/n_g* + t_i*/n_i*) the bracket collapses to
+    t_s / n_i for ANY design values: the paraxial curvature of a defocus by t_s in the immersion medium.  A sign slip or
+    a swapped index in any glass / design term of Eq. 16 or Eq. 17 changes the bracket by ~t_g/n_g = 100 um against
+    t_s/n_i = 1 um.  The coefficient is taken by Richardson-extrapolated second differences (even function of a: the
+    h^2 and h^4 error terms are cancelled); the bar 1e-8 is the rounding of W ~ 1e2 rad in the differences."""
+    for case in (W.small_random_case(3), replace(W.small_random_case(4), n_glass=1.47, t_glass_um=163.0,
+                                                 t_immersion_design_um=140.0, n_immersion_design=1.52, particle_depth_um=3.1)):
+        assert (case.n_glass, case.t_glass_um) != (case.n_glass_design, case.t_glass_design_um)
+        assert case.n_immersion_design != case.n_immersion and case.t_immersion_um is None
+        k0 = 2 * math.pi / case.wavelength_um
+        n_i = case.n_immersion
+
+        def w(a):
+            v = O.gibson_lanni_phase(case, np.array([a / n_i]))[0]
+            assert v.imag == 0.0
+            return v.real
+
+        w0 = w(0.0)
+        d = lambda h: (w(h) - w0) / (h * h)
+        h = 0.05
+        r2a, r2b = (4 * d(h / 2) - d(h)) / 3, (4 * d(h / 4) - d(h / 2)) / 3
+        c2 = (16 * r2b - r2a) / 15
+        want = -0.5 * k0 * case.particle_depth_um / n_i
+        assert abs(c2 / want - 1.0) < 1e-8, (c2, want)
+
+
 # ---- tilt (A9) and Zernike defocus ---------------------------------------------------------------------------------
 
 def test_tilt_is_an_exact_pixel_shift():
@@ -366,6 +396,47 @@ def test_tilt_is_an_exact_pixel_shift():
     # and a whole-pixel shift is an index shift (up to the fp32 rounding of the shift itself)
     I0 = O.stack_T2(base)[0]
     assert np.abs(got[:-3, 2:] - I0[3:, :-2]).max() < 1e-5 * I0.max()
+
+
+def test_noll2_noll3_are_exact_lateral_shifts_of_the_combined_aberrated_field():
+    """PAPER.md:176 Eq. 18 inside PAPER.md:116 Eq. 9.  Noll 2 and 3 are Z_2 = 2 rho cos(phi) = 2 s_x / s_max and
+    Z_3 = 2 s_y / s_max, linear in the pupil coordinates, so c_2 Z_2 + c_3 Z_3 adds to the Fourier kernel
+    k (s_x x + s_y y) exactly a lateral shift: with them the field at (x, y) is the field without them at
+    (x + 2 c_2 / (k s_max), y + 2 c_3 / (k s_max)).  Checked through the whole combined path -- Gibson-Lanni with
+    design != actual, circular input, two more Zernike terms, defocus -- by comparing T2 on the grid (zernike_noll ->
+    plane_phase -> matmul sums) with the literal sum T1 at the shifted points without the two terms: this pins the
+    non-axisymmetric aberrated combination (the class of configs 2, 4, 5) against something other than itself."""
+    base = W.small_random_case(5, pupil_n=22, out_m=13, n_planes=2, pol=W.POL_CIRC_L, per_plane=False, shifts=False)
+    c = np.array([0.45, -0.3, 0.25, -0.2], dtype=np.float32)            # Noll 2, 3, 4, 5
+    with_tilt = replace(base, zernike=c, noll_first=2)
+    c0 = c.copy()
+    c0[:2] = 0.0
+    without = replace(base, zernike=c0, noll_first=2)
+    pup = O.Pupil(base)
+    dx, dy = 2.0 * float(c[0]) / (pup.k * pup.s_max), 2.0 * float(c[1]) / (pup.k * pup.s_max)
+    xs = O.out_coords(13, base.pixel_um)
+    Y, X = np.meshgrid(xs, xs, indexing="ij")
+    got = O.stack_T2(with_tilt)
+    for b in range(2):
+        want = O.intensity_at(without, b, (X + dx).ravel(), (Y + dy).ravel()).reshape(13, 13)
+        assert np.abs(got[b] - want).max() < 1e-12 * want.max()
+    # the shift is real: about 0.3 and 0.2 pixels here, and the unshifted stack differs at the 10 % level
+    assert abs(dx) > 0.2 * base.pixel_um and np.abs(got - O.stack_T2(without)).max() > 0.05 * got.max()
+    # per-plane rows take the same route (config 4's mode): row b shifts plane b only
+    rows = np.stack([c, c0]).astype(np.float32)
+    per = O.stack_T2(replace(base, zernike=rows, noll_first=2))
+    assert np.abs(per[0] - got[0]).max() < 1e-12 * got.max()
+    assert np.abs(per[1] - O.stack_T2(without)[1]).max() < 1e-12 * got.max()
+
+
+def test_in_disc_sample_counts():
+    """in-disc samples of the midpoint grid (integer rim test) for the config sizes."""
+    for N, count in ((64, 3228), (128, 12892), (256, 51468), (512, 205892)):
+        assert int(O.disc_mask(N).sum()) == count
+    # and by plain integer brute force on a small grid
+    N = 10
+    cnt = sum(1 for py in range(N) for px in range(N) if (2 * px + 1 - N) ** 2 + (2 * py + 1 - N) ** 2 <= N * N)
+    assert int(O.disc_mask(N).sum()) == cnt
 
 
 def test_single_c4_is_a_quadratic_pupil_phase():
