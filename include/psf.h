@@ -27,8 +27,15 @@
  *   - every call returns a psf_status; nothing throws or aborts across the ABI; on error outputs are
  *     unspecified and *out is NULL; the message is available from psf_last_error();
  *   - psf_plan_create / psf_set_* may allocate device memory and synchronise; psf_compute only enqueues
- *     kernels on `cuda_stream`: it never allocates, never synchronises and never touches host memory;
- *   - a plan is not thread-safe; distinct plans are independent;
+ *     kernels (and one event record) on `cuda_stream`: it never allocates, never synchronises, never copies
+ *     and never touches host memory;
+ *   - ordering guarantee: every call that overwrites or frees device tables (psf_set_*, psf_plan_tune,
+ *     psf_spherical_prepare, the table rebuild inside psf_gradients, psf_plan_destroy) first waits, on the host,
+ *     for the launches of this plan's earlier psf_compute / psf_compute_spherical / psf_gradients calls, on
+ *     whatever stream they were enqueued (blocking or non-blocking): compute(stream) followed at once by
+ *     psf_set_zernike is safe, and the earlier call still sees the old tables;
+ *   - every call makes the plan's device current (cudaSetDevice) and leaves it current;
+ *   - a plan is not thread-safe; distinct plans are independent (also across threads and devices);
  *   - there is no CPU fallback: without a CUDA device of compute capability 10.x, psf_plan_create fails.
  */
 #ifndef PSF_B200_H
@@ -127,9 +134,8 @@ psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
  *   intensity : device fp32 [n_planes][M][M], x fastest (required);
  *   field     : device complex64 (interleaved re, im) [3][n_planes][M][M] = (E_x, E_y, E_z), or NULL
  *               ([1][n_planes][M][M] for PSF_MODEL_SCALAR).
- * Asynchronous; results are valid once the stream has passed this point.  One exception to "only enqueues": on a plan
- * that runs on the tensor cores, the first call with field != NULL after a table refresh first uploads the tables of
- * the FFMA kernels that write the field (a synchronous copy). */
+ * Asynchronous; results are valid once the stream has passed this point.  Enqueue-only on every kernel path: the
+ * tensor-core stage-2 kernels write the field from their epilogue, no table is uploaded here. */
 psf_status psf_compute(psf_plan *plan, void *cuda_stream, float *intensity, void *field);
 
 /* Spherical (Bessel) parametrisation of the same integral, Eq. 11-14 (Eq. 5 for PSF_MODEL_SCALAR):
@@ -154,6 +160,18 @@ psf_status psf_gradients(psf_plan *plan, void *cuda_stream, const float *dL_dI, 
 
 psf_status psf_plan_destroy(psf_plan *plan);
 
+/* Number of Zernike terms currently set (shared or per plane) = the row length K of psf_gradients' dL_dc. */
+int psf_grad_terms(const psf_plan *plan);
+
+/* Test / A-B knobs of the tensor-core path (never needed for normal use; the library reads no environment variable
+ * for them).  Rebuilds the tensor path's tables and scratch: may allocate and synchronise.
+ *   PSF_TUNE_TC_PAIR_MASK  : value ANDed with the plan's choice; bit 0 = stage 1 on CTA pairs (cta_group::2),
+ *                            bit 1 = stage 2 on CTA pairs; 0 forces the single-CTA tcgen05 kernels (default 3);
+ *   PSF_TUNE_TC_SCRATCH_MB : budget in MB of the stage-1 -> stage-2 scratch (default 0 = 4096): a smaller value splits a
+ *                            stack into several launch pairs. */
+enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2 };
+psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
+
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /
  * psf_host_tables.  Never NULL; valid until the next call on the same plan / thread. */
 const char *psf_last_error(const psf_plan *plan);
@@ -161,7 +179,8 @@ const char *psf_last_error(const psf_plan *plan);
 /* Number of kernel launches one psf_compute call of this plan enqueues (for benchmarking records). */
 int psf_launches_per_compute(const psf_plan *plan);
 
-/* Name of the kernel path the plan selected: "ffma", "tc3xtf32", "tc3xf16" (static string). */
+/* Name of the kernel path the plan selected (static string): "ffma" (fp32 FFMA tiles), "ffma_fused" (small grids: the
+ * whole path in one CTA per plane), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision). */
 const char *psf_path_name(const psf_plan *plan);
 
 /* Profiling aid for bench.py.  enable != 0: create CUDA events (this call may allocate) and make every later

@@ -21,7 +21,8 @@ PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
-           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes"]
+           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms"]
+TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB = 1, 2
 
 
 class PsfError(RuntimeError):
@@ -90,6 +91,10 @@ def load_library(build_if_missing: bool = True):
     lib.psf_profile_read.restype = C.c_int
     lib.psf_last_upload_bytes.argtypes = [P]
     lib.psf_last_upload_bytes.restype = C.c_longlong
+    lib.psf_plan_tune.argtypes = [P, C.c_int, C.c_longlong]
+    lib.psf_plan_tune.restype = C.c_int
+    lib.psf_grad_terms.argtypes = [P]
+    lib.psf_grad_terms.restype = C.c_int
     lib.psf_host_tables.argtypes = [C.POINTER(psf_plan_desc), C.POINTER(C.c_float), C.c_int, C.c_int,
                                     C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double), C.POINTER(C.c_ubyte)]
@@ -216,12 +221,18 @@ class PsfPlan:
         self._check(self._lib.psf_compute_spherical(self._h, C.c_void_p(s.cuda_stream), C.c_void_p(intensity.data_ptr())))
         return intensity
 
-    def gradients(self, dL_dI, n_terms: int = 0, stream=None):
-        """Adjoint: dL_dI is a CUDA float32 tensor [Z, M, M]; returns (dL_dz [Z], dL_dc [Z, n_terms] or None), float64
-        CUDA tensors.  n_terms = number of Zernike terms currently set (0: defocus gradients only)."""
+    def gradients(self, dL_dI, n_terms: int | None = None, stream=None):
+        """Adjoint: dL_dI is a CUDA float32 tensor [Z, M, M]; returns (dL_dz [Z], dL_dc [Z, K] or None), float64 CUDA
+        tensors.  K = the number of Zernike terms currently set (psf_grad_terms); n_terms, if given, must be 0 (defocus
+        gradients only) or K: the library writes rows of K values."""
         import torch
         dev = torch.device("cuda", self.device)
         Z, M = self.n_planes, self.out_m
+        K = int(self._lib.psf_grad_terms(self._h))
+        if n_terms is None:
+            n_terms = K
+        if n_terms not in (0, K):
+            raise ValueError(f"n_terms must be 0 or the number of Zernike terms set ({K})")
         if tuple(dL_dI.shape) != (Z, M, M) or dL_dI.dtype != torch.float32 or not dL_dI.is_contiguous() or not dL_dI.is_cuda:
             raise ValueError("dL_dI must be a contiguous CUDA float32 tensor [n_planes, M, M]")
         dz = torch.empty((Z,), dtype=torch.float64, device=dev)
@@ -230,6 +241,10 @@ class PsfPlan:
         self._check(self._lib.psf_gradients(self._h, C.c_void_p(s.cuda_stream), C.c_void_p(dL_dI.data_ptr()),
                                             C.c_void_p(dz.data_ptr()), C.c_void_p(dc.data_ptr()) if dc is not None else None))
         return dz, dc
+
+    def tune(self, knob: int, value: int):
+        """psf_plan_tune: TUNE_TC_PAIR_MASK / TUNE_TC_SCRATCH_MB (tests and A/B runs)."""
+        self._check(self._lib.psf_plan_tune(self._h, int(knob), int(value)))
 
     def profile_enable(self, enable: bool = True):
         self._check(self._lib.psf_profile_enable(self._h, int(bool(enable))))

@@ -22,6 +22,33 @@ const size_t kScratchBudget = (size_t)48 << 20;   // T scratch ring: small enoug
     }                                                                                           \
   } while (0)
 
+void set_err(psf_plan *p, const char *msg) noexcept {
+  try { if (p) p->err = msg; else g_create_err = msg; } catch (...) {}
+}
+
+// Every extern "C" body runs inside this guard: nothing throws across the ABI (psf.h).
+template <typename F>
+psf_status guarded(psf_plan *p, F &&body) noexcept {
+  try {
+    return body();
+  } catch (const std::bad_alloc &) {
+    set_err(p, "out of host memory");
+    return PSF_ERR_ALLOC;
+  } catch (const std::exception &e) {
+    set_err(p, e.what());
+    return PSF_ERR_CUDA;
+  } catch (...) {
+    set_err(p, "unknown C++ exception");
+    return PSF_ERR_CUDA;
+  }
+}
+
+// Tables on the device may still be read by launches of an earlier compute call on the caller's stream (any stream:
+// a non-blocking stream does not serialise with the copies below).  Every compute call records `done_ev` behind its
+// last launch; whoever is about to overwrite or free a table waits for it first.
+cudaError_t wait_inflight(psf_plan *p) { return p->done_ev ? cudaEventSynchronize(p->done_ev) : cudaSuccess; }
+void mark_inflight(psf_plan *p, cudaStream_t st) { if (p->done_ev) cudaEventRecord(p->done_ev, st); }
+
 template <typename T>
 psf_status upload(psf_plan *p, void **dptr, size_t *cap, const std::vector<T> &h) {
   const size_t bytes = h.size() * sizeof(T);
@@ -47,7 +74,6 @@ psf_status upload_ffma_tables(psf_plan *p) {
   if ((s = upload(p, &p->d_kt, &p->cap_kt, p->h_kt)) != PSF_OK) return s;
   p->dp.bfold = (const float4 *)p->d_bfold;
   p->dp.kt = (const float2 *)p->d_kt;
-  p->ffma_stale = false;
   return PSF_OK;
 }
 
@@ -103,11 +129,10 @@ psf_status upload_static(psf_plan *p) {
   }
   tm.mark("fold");
   psf_status s;
-  // The folded tables feed the FFMA kernels.  A plan on the tensor path needs them only for a field output, so their
-  // upload (10 MB at N = 512) is left to the first such psf_compute after a refresh.
+  // The folded tables feed the FFMA kernels only; a plan on the tensor path (whose stage-2 epilogue also writes the field
+  // output) never reads them: no upload (10 MB at N = 512).
   const bool tensor_path = d.precision != PSF_PREC_FP32 && !P.per_plane &&
                            (d.precision == PSF_PREC_3XTF32 || d.precision == PSF_PREC_3XF16 || tc_eligible(p));
-  p->ffma_stale = tensor_path;
   if (!tensor_path && (s = upload_ffma_tables(p)) != PSF_OK) return s;
   tm.mark("upload bfold, kt");
 
@@ -206,6 +231,7 @@ psf_status alloc_scratch(psf_plan *p) {
 }
 
 psf_status refresh(psf_plan *p) {
+  if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
   p->upload_bytes = 0;
   ++p->table_version;
   psf_status s = upload_static(p);
@@ -220,6 +246,7 @@ void free_all(psf_plan *p) {
     if (*b) { cudaFree(*b); *b = nullptr; }
   for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
   p->prof_ev.clear();
+  if (p->done_ev) { cudaEventDestroy(p->done_ev); p->done_ev = nullptr; }
   tc_free(p);
   bessel_free(p);
   grad_free(p);
@@ -230,6 +257,8 @@ void free_all(psf_plan *p) {
 extern "C" {
 
 psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
+  psf_plan *p = nullptr;
+  try {
   if (out) *out = nullptr;
   if (!out) { g_create_err = "out is NULL"; return PSF_ERR_INVALID_ARG; }
   std::string err;
@@ -251,7 +280,7 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
     g_create_err = "device is not sm_100 (compute capability 10.x): this library is built for B200 only";
     return PSF_ERR_UNSUPPORTED;
   }
-  psf_plan *p = new (std::nothrow) psf_plan();
+  p = new (std::nothrow) psf_plan();
   if (!p) { g_create_err = "out of host memory"; return PSF_ERR_ALLOC; }
   p->desc = *desc;
   p->z.assign(desc->z_um, desc->z_um + desc->n_planes);
@@ -262,8 +291,10 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
   DevPlan &P = p->dp;
   P.N = desc->pupil_n; P.M = desc->out_m; P.n = (P.N + 1) / 2; P.m = (P.M + 1) / 2; P.Z = desc->n_planes;
   P.per_plane = 0; P.K = 0; P.has_shift = 0;
-  if ((e = cudaSetDevice(p->device)) != cudaSuccess) {
-    g_create_err = std::string("cudaSetDevice: ") + cudaGetErrorString(e);
+  if ((e = cudaSetDevice(p->device)) != cudaSuccess || (e = cudaEventCreateWithFlags(&p->done_ev, cudaEventDisableTiming)) != cudaSuccess ||
+      (e = small_setup()) != cudaSuccess) {
+    g_create_err = std::string("plan set-up (device, event, function attributes): ") + cudaGetErrorString(e);
+    free_all(p);
     delete p;
     return PSF_ERR_CUDA;
   }
@@ -278,10 +309,17 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
   }
   *out = p;
   return PSF_OK;
+  } catch (...) {                       // std::bad_alloc from the host tables, or anything else: never across the ABI
+    if (p) { try { free_all(p); } catch (...) {} delete p; }
+    if (out) *out = nullptr;
+    set_err(nullptr, "out of host memory (or another C++ exception) while building the plan");
+    return PSF_ERR_ALLOC;
+  }
 }
 
 psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int n_coeffs, int per_plane) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (n_coeffs < 0) { p->err = "n_coeffs < 0"; return PSF_ERR_INVALID_ARG; }
   if (n_coeffs > 0 && coeffs && noll_first < 1) { p->err = "noll_first must be >= 1"; return PSF_ERR_INVALID_ARG; }
   if (n_coeffs > 64) { p->err = "at most 64 Zernike terms"; return PSF_ERR_INVALID_ARG; }
@@ -301,10 +339,12 @@ psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int
   }
   p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;
   return refresh(p);
+  });
 }
 
 psf_status psf_set_phase_mask(psf_plan *p, const float *w0_rad) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   const size_t NN = (size_t)p->desc.pupil_n * p->desc.pupil_n;
   if (w0_rad)
     for (size_t i = 0; i < NN; ++i)
@@ -314,10 +354,12 @@ psf_status psf_set_phase_mask(psf_plan *p, const float *w0_rad) {
   p->phase_mask.clear();
   if (w0_rad) p->phase_mask.assign(w0_rad, w0_rad + NN);
   return refresh(p);
+  });
 }
 
 psf_status psf_set_shifts(psf_plan *p, const float *xy_um) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (xy_um)
     for (int i = 0; i < 2 * p->dp.Z; ++i)
       if (!std::isfinite(xy_um[i])) { p->err = "non-finite shift"; return PSF_ERR_INVALID_ARG; }
@@ -327,33 +369,33 @@ psf_status psf_set_shifts(psf_plan *p, const float *xy_um) {
   if (xy_um) p->shifts.assign(xy_um, xy_um + 2 * (size_t)p->dp.Z);
   p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;
   return refresh(p);
+  });
 }
 
 psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *field) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (!intensity) { p->err = "intensity is NULL"; return PSF_ERR_INVALID_ARG; }
   if (((uintptr_t)intensity & 15) || ((uintptr_t)field & 15)) { p->err = "output pointers must be 16-byte aligned"; return PSF_ERR_INVALID_ARG; }
   if (field && p->desc.pol == PSF_POL_UNPOLARIZED && p->desc.model == PSF_MODEL_VECTORIAL) {
     p->err = "field output is undefined for PSF_POL_UNPOLARIZED (two incoherent fields)";
     return PSF_ERR_UNSUPPORTED;
   }
+  if (cudaSetDevice(p->device) != cudaSuccess) { p->err = "cudaSetDevice failed"; return PSF_ERR_CUDA; }
   if (p->prof) {
     p->prof_n = 0;
     p->prof_valid = true;
     cudaEventRecord(p->prof_ev[0], (cudaStream_t)cuda_stream);
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const bool tc = (p->path == 1 || p->path == 2) && !field;
-  if (!tc && p->ffma_stale) {                  // first field output of a tensor-path plan since the last table refresh
-    if (cudaSetDevice(p->device) != cudaSuccess) { p->err = "cudaSetDevice failed"; return PSF_ERR_CUDA; }
-    const psf_status us = upload_ffma_tables(p);
-    if (us != PSF_OK) return us;
-  }
-  cudaError_t e = tc ? launch_tc(p, st, intensity)
-                     : (p->path == 3 || small_eligible(p)) ? launch_small(p, st, intensity, (float2 *)field)
-                                                            : launch_ffma(p, st, intensity, (float2 *)field);
+  const bool tc = p->path == 1 || p->path == 2;
+  cudaError_t e = tc ? launch_tc(p, st, intensity, (float2 *)field)
+                     : p->path == 3 ? launch_small(p, st, intensity, (float2 *)field)
+                                    : launch_ffma(p, st, intensity, (float2 *)field);
+  mark_inflight(p, st);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
+  });
 }
 
 // ---- spherical (Bessel) parametrisation: axisymmetric pupils only ---------------------------------------------------
@@ -367,18 +409,23 @@ static bool axisymmetric(psf_plan *p) {
 
 psf_status psf_spherical_prepare(psf_plan *p, int n_nodes) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (n_nodes < 3 || !(n_nodes & 1) || n_nodes > (1 << 20)) { p->err = "n_nodes must be odd, >= 3 (composite Simpson)"; return PSF_ERR_INVALID_ARG; }
   if (!axisymmetric(p)) return PSF_ERR_STATE;
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
   return bessel_setup(p, n_nodes);
+  });
 }
 
 psf_status psf_compute_spherical(psf_plan *p, void *cuda_stream, float *intensity) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (!intensity || ((uintptr_t)intensity & 15)) { p->err = "intensity must be a 16-byte aligned device pointer"; return PSF_ERR_INVALID_ARG; }
   if (!p->bessel) { p->err = "psf_spherical_prepare has not been called"; return PSF_ERR_STATE; }
   if (!axisymmetric(p)) return PSF_ERR_STATE;
+  if (cudaSetDevice(p->device) != cudaSuccess) { p->err = "cudaSetDevice failed"; return PSF_ERR_CUDA; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (p->prof) {
     p->prof_n = 0;
@@ -386,30 +433,63 @@ psf_status psf_compute_spherical(psf_plan *p, void *cuda_stream, float *intensit
     cudaEventRecord(p->prof_ev[0], st);
   }
   cudaError_t e = launch_bessel(p, st, intensity);
+  mark_inflight(p, st);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
+  });
 }
 
 // ---- adjoint ---------------------------------------------------------------------------------------------------------
 psf_status psf_gradients(psf_plan *p, void *cuda_stream, const float *dL_dI, double *dL_dz, double *dL_dc) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (!dL_dI || !dL_dz) { p->err = "dL_dI and dL_dz must be device pointers"; return PSF_ERR_INVALID_ARG; }
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  if (grad_needs_setup(p) && wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
   psf_status s = grad_setup(p);               // first call, or the tables changed: (re)build the adjoint's copies
   if (s != PSF_OK) return s;
   if (dL_dc && grad_terms(p) == 0) { p->err = "dL_dc asked for, but no Zernike terms are set"; return PSF_ERR_STATE; }
   e = launch_grad(p, (cudaStream_t)cuda_stream, dL_dI, dL_dz, dL_dc);
+  mark_inflight(p, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) { p->err = std::string("kernel launch: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
   return PSF_OK;
+  });
 }
 
 psf_status psf_plan_destroy(psf_plan *p) {
   if (!p) return PSF_ERR_INVALID_ARG;
   cudaSetDevice(p->device);
-  free_all(p);
+  wait_inflight(p);                            // launches of this plan still in flight read its tables
+  try { free_all(p); } catch (...) {}
   delete p;
   return PSF_OK;
+}
+
+psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
+  if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
+    if (knob == PSF_TUNE_TC_PAIR_MASK) {
+      if (value < 0 || value > 3) { p->err = "PSF_TUNE_TC_PAIR_MASK: 0..3"; return PSF_ERR_INVALID_ARG; }
+      p->tune_pair_mask = (int)value;
+    } else if (knob == PSF_TUNE_TC_SCRATCH_MB) {
+      if (value < 0 || value > (1 << 20)) { p->err = "PSF_TUNE_TC_SCRATCH_MB: 0 (default) .. 2^20"; return PSF_ERR_INVALID_ARG; }
+      p->tune_scratch_mb = (int)value;
+    } else {
+      p->err = "unknown tuning knob";
+      return PSF_ERR_INVALID_ARG;
+    }
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+    if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+    tc_free(p);                                // the tensor path rebuilds its tables, scratch and tensor maps with the new knobs
+    return refresh(p);
+  });
+}
+
+int psf_grad_terms(const psf_plan *p) {
+  if (!p) return 0;
+  return p->K_rows > 0 ? p->K_rows : (int)p->zern_shared.size();
 }
 
 const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_create_err.c_str(); }
@@ -424,6 +504,7 @@ const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 3
 
 psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
   p->prof = false;
@@ -439,10 +520,12 @@ psf_status psf_profile_enable(psf_plan *p, int enable) {
   p->prof_stage.assign(p->prof_ev.size(), 0);
   p->prof = true;
   return PSF_OK;
+  });
 }
 
 psf_status psf_profile_read(psf_plan *p, float *stage_ms, int *launches) {
   if (!p) return PSF_ERR_INVALID_ARG;
+  return guarded(p, [&]() -> psf_status {
   if (!stage_ms || !launches) { p->err = "NULL output"; return PSF_ERR_INVALID_ARG; }
   if (!p->prof || !p->prof_valid) { p->err = "profiling is not enabled or no psf_compute ran since"; return PSF_ERR_STATE; }
   for (int i = 0; i < 4; ++i) { stage_ms[i] = 0.f; launches[i] = 0; }
@@ -455,12 +538,14 @@ psf_status psf_profile_read(psf_plan *p, float *stage_ms, int *launches) {
     launches[st] += 1;
   }
   return PSF_OK;
+  });
 }
 
 long long psf_last_upload_bytes(const psf_plan *p) { return p ? p->upload_bytes : 0; }
 
 psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int noll_first, int n_coeffs, int *n_components,
                            double *weights, double *base, double *kappa, unsigned char *mask) {
+  return guarded(nullptr, [&]() -> psf_status {
   std::string err;
   psf_status s = validate_desc(desc, err);
   if (s != PSF_OK) { g_create_err = err; return s; }
@@ -477,6 +562,7 @@ psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int n
   if (kappa) std::memcpy(kappa, hp.kappa.data(), NN * sizeof(double));
   if (mask) std::memcpy(mask, hp.mask.data(), NN);
   return PSF_OK;
+  });
 }
 
 }  // extern "C"

@@ -166,6 +166,8 @@ void grad_free(psf_plan *p) {
 }
 
 // (Re)builds the device tables of the adjoint from the plan's current host tables; allocates the per-pass scratch.
+bool grad_needs_setup(const psf_plan *p) { return !(p->grad && p->grad->version == p->table_version); }
+
 psf_status grad_setup(psf_plan *p) {
   const psf_plan_desc &d = p->desc;
   const DevPlan &D = p->dp;
@@ -221,7 +223,7 @@ psf_status grad_setup(psf_plan *p) {
   size_t zc = ((size_t)1 << 30) / per_plane;
   if (zc < 1) zc = 1;
   if (zc > (size_t)D.Z) zc = D.Z;
-  if (zc > 65535) zc = 65535;
+  if (zc > 65535 / (size_t)g->Cg) zc = 65535 / (size_t)g->Cg;   // gridDim.z of the batched products is Cg * zc
   g->zc = (int)zc;
   if (cudaMalloc(&g->d_Q, zc * g->Cg * NN * sizeof(float2)) != cudaSuccess || cudaMalloc(&g->d_B, zc * g->Cg * NN * sizeof(float2)) != cudaSuccess ||
       cudaMalloc(&g->d_T, zc * g->Cg * MN * sizeof(float2)) != cudaSuccess || cudaMalloc(&g->d_E, zc * g->Cg * MM * sizeof(float2)) != cudaSuccess)

@@ -292,15 +292,13 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
 
 template <int MQ, bool PP, bool FIELD>
 cudaError_t launch_one(const DevPlan &P, cudaStream_t st, float *intensity, float2 *field) {
-  static bool attr_set = false;
-  const int bytes = (int)sizeof(SmallSmem<MQ, PP>);
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_small<MQ, PP, FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
-  k_small<MQ, PP, FIELD><<<P.Z, SM_THREADS, bytes, st>>>(P, intensity, field);
+  k_small<MQ, PP, FIELD><<<P.Z, SM_THREADS, (int)sizeof(SmallSmem<MQ, PP>), st>>>(P, intensity, field);
   return cudaGetLastError();
+}
+
+template <int MQ, bool PP, bool FIELD>
+cudaError_t set_attr() {
+  return cudaFuncSetAttribute(k_small<MQ, PP, FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem<MQ, PP>));
 }
 
 template <int MQ>
@@ -312,6 +310,18 @@ cudaError_t launch_mq(const DevPlan &P, cudaStream_t st, float *intensity, float
 }  // namespace
 
 bool small_eligible(const psf_plan *p) { return p->dp.n <= NQ && p->dp.m <= 32; }
+
+// The dynamic shared memory of every instantiation exceeds the 48 KB default.  Function attributes are per device, so
+// every plan sets them at creation with its own device current (idempotent, no per-process flag).
+cudaError_t small_setup() {
+  cudaError_t e;
+  if ((e = set_attr<16, false, false>()) != cudaSuccess || (e = set_attr<16, false, true>()) != cudaSuccess ||
+      (e = set_attr<16, true, false>()) != cudaSuccess || (e = set_attr<16, true, true>()) != cudaSuccess ||
+      (e = set_attr<32, false, false>()) != cudaSuccess || (e = set_attr<32, false, true>()) != cudaSuccess ||
+      (e = set_attr<32, true, false>()) != cudaSuccess || (e = set_attr<32, true, true>()) != cudaSuccess)
+    return e;
+  return cudaSuccess;
+}
 
 cudaError_t launch_small(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field) {
   const DevPlan &P = p->dp;

@@ -81,7 +81,11 @@ struct psf_plan {
   psf::TcState *tc = nullptr;
   psf::BesselState *bessel = nullptr;
   psf::GradState *grad = nullptr;
-  bool ffma_stale = false;       // tensor-path plan: the FFMA tables on the device are older than the host copies
+  // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
+  int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
+  int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
+  cudaEvent_t done_ev = nullptr; // recorded on the caller's stream after the last launch of every compute call: table
+                                 // refreshes wait for it before they overwrite tables a launch in flight may still read
   long long table_version = 0;   // bumped by every table refresh (psf_set_*): derived copies check it
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
@@ -106,6 +110,7 @@ cudaError_t launch_ffma(const psf_plan *p, cudaStream_t st, float *intensity, fl
 int ffma_launches(const psf_plan *p);
 // kernels_small.cu
 bool small_eligible(const psf_plan *p);
+cudaError_t small_setup();       // per-device function attributes (call with the plan's device current)
 cudaError_t launch_small(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 // kernels_tc.cu
 bool tc_eligible(const psf_plan *p);
@@ -113,13 +118,14 @@ psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::ve
                     bool f16);
 void tc_free(psf_plan *p);
 int tc_launches(const psf_plan *p);
-cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity);
+cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 // kernels_bessel.cu
 psf_status bessel_setup(psf_plan *p, int n_nodes);
 void bessel_free(psf_plan *p);
 cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
 // kernels_grad.cu
 psf_status grad_setup(psf_plan *p);
+bool grad_needs_setup(const psf_plan *p);
 void grad_free(psf_plan *p);
 int grad_terms(const psf_plan *p);
 cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, double *dL_dz, double *dL_dc);

@@ -125,8 +125,10 @@ __device__ __forceinline__ void issue_stage_mmas2(uint32_t sbase, uint32_t d_tme
 // ---- stage 2 ----------------------------------------------------------------------------------------------------------
 struct K2PArgs {
   float *intensity;     // [Z][M][M]
-  int C, n_pad, m_pad, m, M, z0, zc;
+  float2 *field;        // [C][Z][M][M] or nullptr (FIELD kernels only)
+  int C, n_pad, m_pad, m, M, z0, zc, Z;
   float weight[5];      // intensity weights times the inverse operand scales squared
+  float fscale;         // 1 / (s_X s_T): accumulator -> field
 };
 
 constexpr int K2P_NST = 3;
@@ -204,6 +206,8 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
 }
 
 // sixteen epilogue warps: butterfly + |E|^2, running sums over the components, coalesced quadrant stores
+// (FIELD: the four mirror values of E_c are also stored, 32 bytes per thread and store, straight from the registers)
+template <bool FIELD>
 __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint32_t tmem, const K2PArgs &P, int warp, int lane, uint32_t rank,
                                              int tiles_yp, int tiles_x, int ntiles, int ncl, int cid) {
   uint64_t &acc_full = S.acc_full, &acc_empty = S.acc_empty;
@@ -256,6 +260,18 @@ __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint3
             sum[1][i] = fmaf(w, re1 * re1 + im1 * im1, sum[1][i]);
             sum[2][i] = fmaf(w, re2 * re2 + im2 * im2, sum[2][i]);
             sum[3][i] = fmaf(w, re3 * re3 + im3 * im3, sum[3][i]);
+            if (FIELD) {
+              const int my = ty * 128 + q * 32 + lane, mx = tx * 64 + e * 16 + i;
+              if (my < P.m && mx < P.m) {
+                float2 *f = P.field + ((size_t)c * P.Z + (P.z0 + zl)) * (size_t)P.M * P.M;
+                const int myr = P.M - 1 - my, mxr = P.M - 1 - mx;
+                const float fs = P.fscale;
+                f[(size_t)my * P.M + mx] = make_float2(fs * re0, fs * im0);
+                f[(size_t)my * P.M + mxr] = make_float2(fs * re1, fs * im1);
+                f[(size_t)myr * P.M + mx] = make_float2(fs * re2, fs * im2);
+                f[(size_t)myr * P.M + mxr] = make_float2(fs * re3, fs * im3);
+              }
+            }
           }
         }
       }
@@ -290,6 +306,7 @@ __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint3
   }
 }
 
+template <bool FIELD>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K2P_THREADS, 1)
 k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
         const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo, const K2PArgs P) {
@@ -325,7 +342,7 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
     k2p_feed(smem, S, tmem, map_xhi, map_xlo, map_thi, map_tlo, P, warp, rank, nk, tiles_yp, tiles_x, ntiles, ncl, cid);
   } else {
     setmaxnreg_inc<112>();
-    k2p_epilogue(staging, S, tmem, P, warp, lane, rank, tiles_yp, tiles_x, ntiles, ncl, cid);
+    k2p_epilogue<FIELD>(staging, S, tmem, P, warp, lane, rank, tiles_yp, tiles_x, ntiles, ncl, cid);
   }
   tcgen05_fence_before();
   __syncthreads();

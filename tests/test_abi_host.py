@@ -153,3 +153,46 @@ def test_host_tables_fresnel_coefficients():
     a, b, d, cx, cy = t["base"]
     for got, want in ((a, bx[0]), (b, bx[1]), (cx, bx[2]), (b, by[0]), (d, by[1]), (cy, by[2])):
         assert np.abs(got - want).max() < 1e-11 * np.abs(bx).max()
+
+
+def test_create_errors_are_per_thread_and_nothing_crosses_the_abi():
+    """psf.h: distinct plans are independent across threads; the message of a failed psf_plan_create belongs to the
+    calling thread.  Two threads fail in different ways many times over (no device is needed for either failure)."""
+    import threading
+    lib = psf.load_library()
+    bad = []
+
+    def worker(kind):
+        for _ in range(200):
+            if kind == 0:
+                desc, keep = psf.make_desc(replace(W.config1(), NA=0.0))
+                h = C.c_void_p()
+                st = lib.psf_plan_create(C.byref(desc), C.byref(h))
+                msg = lib.psf_last_error(None)
+                if st != 1 or h.value or b"NA" not in msg:
+                    bad.append((kind, st, msg))
+            else:
+                desc, keep = psf.make_desc(W.config1())
+                st = lib.psf_plan_create(C.byref(desc), None)
+                msg = lib.psf_last_error(None)
+                if st != 1 or b"NULL" not in msg:
+                    bad.append((kind, st, msg))
+
+    th = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not bad, bad[:3]
+
+
+def test_library_reads_no_environment_variable_outside_the_phase_timer():
+    """SURVEY section 5 / psf.h: no environment variables steer the product; the one getenv is the PSF_TIMING development
+    aid of PhaseTimer (plan.hpp), which only prints wall-clock phases."""
+    csrc = os.path.join(ROOT, "paper_2502_03170_b200", "csrc")
+    hits = []
+    for f in sorted(os.listdir(csrc)):
+        for i, line in enumerate(open(os.path.join(csrc, f)), 1):
+            if "getenv" in line:
+                hits.append((f, i, line.strip()))
+    assert len(hits) == 1 and hits[0][0] == "plan.hpp" and "PSF_TIMING" in hits[0][2], hits

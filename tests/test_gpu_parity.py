@@ -157,12 +157,89 @@ def test_cta_pair_kernels_ragged_sizes(psf, seed, N, M, Z, pol):
 
 @pytest.mark.parametrize("precision", PRECISIONS)
 def test_field_output_matches_oracle_field(psf, precision):
+    """field[3][Z][M][M] from every kernel path; a tensor-path plan keeps its path (the stage-2 epilogue
+    writes the field: psf_compute stays enqueue-only)."""
     case = replace(W.config2(), z_um=np.linspace(-2.0, 2.0, 5), pupil_n=96, out_m=50)
     (I, F), path = gpu_stack(psf, case, precision, want_field=True)
+    assert path == {"fp32": "ffma", "auto": "tc3xf16", "3xtf32": "tc3xtf32", "3xf16": "tc3xf16"}[precision]
     Eref = O.field_T2(case)
     scale = np.abs(Eref).max()
     assert np.abs(F - Eref).max() <= 2e-5 * scale
     assert np.abs(np.sum(np.abs(F) ** 2, axis=0) - I).max() <= 1e-5 * I.max()
+    I2, _ = gpu_stack(psf, case, precision)                  # the intensity-only kernels agree with the field kernels
+    assert np.abs(I2 - I).max() <= 1e-6 * I.max()
+
+
+@pytest.mark.parametrize("N,M,pol,model", [(200, 300, W.POL_CIRC_L, "vectorial"),     # m = 150 (pad 256): pair kernels
+                                           (131, 515, W.POL_JONES, "vectorial"),      # odd M, two pair tiles in x
+                                           (260, 257, W.POL_X, "scalar")])            # one scalar pupil, odd M
+def test_field_output_on_the_cta_pair_kernels(psf, N, M, pol, model):
+    case = replace(W.small_random_case(57, pupil_n=N, out_m=M, n_planes=2, per_plane=False, shifts=False, pol=pol), model=model)
+    (I, F), path = gpu_stack(psf, case, "auto", want_field=True)
+    assert path == "tc3xf16"
+    Eref = O.field_T2(case)
+    assert F.shape == Eref.shape
+    assert np.abs(F - Eref).max() <= 2e-5 * np.abs(Eref).max()
+    assert plane_errors(I, O.stack_T2(case)).max() <= TOL
+
+
+def test_set_zernike_right_after_compute_on_a_non_blocking_stream(psf):
+    """psf.h ordering guarantee: a table refresh waits for the plan's launches in flight on any stream.  compute() on a
+    non-blocking stream (no implicit ordering with the legacy stream the copies use) followed at once by set_zernike
+    must still give the result of the old coefficients."""
+    import torch
+    case = W.small_random_case(58, pupil_n=512, out_m=512, n_planes=24, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
+    other = replace(case, zernike=(-case.zernike).astype(np.float32))
+    ref_a, ref_b = O.stack_T2(case, planes=[0, 11, 23]), O.stack_T2(other, planes=[0, 11, 23])
+    for precision in ("auto", "fp32"):
+        plan = psf.plan_from_case(case, precision=precision)
+        s = torch.cuda.Stream()                       # non-blocking
+        out_a = torch.empty((24, 512, 512), dtype=torch.float32, device="cuda")
+        out_b = torch.empty_like(out_a)
+        torch.cuda.synchronize()
+        for _ in range(3):
+            plan.set_zernike(case.zernike, case.noll_first)
+            plan.compute(out_a, stream=s)
+            plan.set_zernike(other.zernike, other.noll_first)      # must not disturb the call in flight
+            plan.compute(out_b, stream=s)
+            s.synchronize()
+            a, b = out_a.cpu().numpy().astype(np.float64), out_b.cpu().numpy().astype(np.float64)
+            assert plane_errors(a[[0, 11, 23]], ref_a).max() <= TOL, precision
+            assert plane_errors(b[[0, 11, 23]], ref_b).max() <= TOL, precision
+        plan.destroy()
+
+
+def test_plans_on_two_threads_are_independent(psf):
+    """psf.h: distinct plans are independent, also across threads (per-device function attributes are set per plan, error
+    strings are per plan / per thread)."""
+    import threading
+    import torch
+    cases = [W.small_random_case(59, pupil_n=44, out_m=30, n_planes=3), W.config1(),
+             W.small_random_case(60, pupil_n=150, out_m=90, n_planes=2, per_plane=False, shifts=False)]
+    refs = [O.stack_T2(c) for c in cases]
+    errs = []
+
+    def work(tid):
+        try:
+            for rep in range(3):
+                for c, r in zip(cases, refs):
+                    plan = psf.plan_from_case(c)
+                    st = torch.cuda.Stream()
+                    I = plan.compute(stream=st)
+                    st.synchronize()
+                    e = plane_errors(I.cpu().numpy().astype(np.float64), r).max()
+                    plan.destroy()
+                    if e > TOL:
+                        errs.append((tid, c.name, e))
+        except Exception as ex:                      # noqa: BLE001
+            errs.append((tid, repr(ex)))
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errs, errs
 
 
 def test_unpolarised_is_mean_of_x_and_y_and_field_is_refused(psf):
@@ -209,13 +286,14 @@ def test_replan_zernike_and_shift_updates(psf):
     plan.destroy()
 
 
-def test_cta_pair_kernels_replan_chunked_and_single_plane(psf, monkeypatch):
+def test_cta_pair_kernels_replan_chunked_and_single_plane(psf):
     """Pair kernels: new shared Zernike coefficients after creation (the producer-ordered tables are rebuilt), a scratch
     budget that forces several launch pairs per stack (z-chunks of unequal size), and a one-plane stack."""
     import torch
-    monkeypatch.setenv("PSF_TC_SCRATCH_MB", "24")                      # 5.2 MB of T^T (hi or lo) per plane -> 4-plane chunks
     base = W.small_random_case(71, pupil_n=512, out_m=512, n_planes=6, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
     plan = psf.plan_from_case(base, precision="3xf16")
+    assert plan.path == "tc3xf16" and plan.launches_per_compute == 2
+    plan.tune(psf.TUNE_TC_SCRATCH_MB, 24)                              # 5.2 MB of T^T (hi or lo) per plane -> 4-plane chunks
     assert plan.path == "tc3xf16" and plan.launches_per_compute == 4
     a = plan.compute().cpu().numpy().astype(np.float64)
     assert plane_errors(a, O.stack_T2(base)).max() <= TOL
@@ -224,8 +302,11 @@ def test_cta_pair_kernels_replan_chunked_and_single_plane(psf, monkeypatch):
     b = plan.compute().cpu().numpy().astype(np.float64)
     torch.cuda.synchronize()
     assert plane_errors(b, O.stack_T2(other)).max() <= TOL
+    # the single-CTA tcgen05 kernels on the same plan (A/B knob), then back
+    plan.tune(psf.TUNE_TC_PAIR_MASK, 0)
+    c = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(c, O.stack_T2(other)).max() <= TOL
     plan.destroy()
-    monkeypatch.delenv("PSF_TC_SCRATCH_MB")
     one = replace(base, z_um=base.z_um[:1])
     I, path = gpu_stack(psf, one, "auto")
     assert path == "tc3xf16"
@@ -351,8 +432,12 @@ def test_adjoint_gradients_match_oracle(psf):
         dz_ref, dc_ref = O.grad_T2(case, G.astype(np.float64))
         plan = psf.plan_from_case(case)
         K = 0 if case.zernike is None else case.zernike.shape[-1]
-        dz, dc = plan.gradients(torch.from_numpy(G).cuda(), K)
+        dz, dc = plan.gradients(torch.from_numpy(G).cuda())
         torch.cuda.synchronize()
+        assert (dc is None) == (K == 0)
+        if K:
+            with pytest.raises(ValueError):
+                plan.gradients(torch.from_numpy(G).cuda(), K + 1)
         assert np.abs(dz.cpu().numpy() - dz_ref).max() <= GRAD_TOL * np.abs(dz_ref).max(), case.name
         if K:
             assert np.abs(dc.cpu().numpy() - dc_ref).max() <= GRAD_TOL * np.abs(dc_ref).max(), case.name
