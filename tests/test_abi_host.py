@@ -192,6 +192,8 @@ def test_library_reads_no_environment_variable_outside_the_phase_timer():
     csrc = os.path.join(ROOT, "paper_2502_03170_b200", "csrc")
     hits = []
     for f in sorted(os.listdir(csrc)):
+        if not os.path.isfile(os.path.join(csrc, f)):
+            continue
         for i, line in enumerate(open(os.path.join(csrc, f)), 1):
             if "getenv" in line:
                 hits.append((f, i, line.strip()))

@@ -1,5 +1,6 @@
 """GPU parity: the CUDA path (through the C-ABI) against the fp64 oracle, element by element, on the same seeded
 inputs.  Bar (BASELINE.json north_star): for every plane, max|I_gpu - I_oracle| <= 2e-5 max(I_oracle)."""
+import os
 from dataclasses import replace
 
 import numpy as np
@@ -452,21 +453,45 @@ def test_adjoint_gradients_match_oracle(psf):
         plan.destroy()
 
 
-def test_pair_kernels_are_deterministic_under_repetition(psf):
-    """The pair kernels sum in a fixed order: repeated psf_compute calls on one plan are bit-identical.  Guards the
-    cross-CTA hand-off of generic-proxy operand writes in k1_pair (profiles/r1j_race_k1_pair.md): with a CTA-scope
-    release about 4 % of config-5 calls had one plane computed from stale rows."""
+def _repeat_bit_identical(psf, case, calls, tune=None, flush_every=2):
+    """Repeated psf_compute on one plan: the pair kernels sum in a fixed order, so every call must reproduce the first bit
+    for bit; the first stack itself is checked against the oracle on three planes."""
     import torch
-    plan = psf.plan_from_case(W.config5())
+    plan = psf.plan_from_case(case)
+    if tune:
+        plan.tune(*tune)
+    assert plan.path == "tc3xf16"
     ref = plan.compute().clone()
     torch.cuda.synchronize()
+    sel = sorted({0, case.n_planes // 2, case.n_planes - 1})
+    assert plane_errors(ref[sel].cpu().numpy().astype(np.float64), O.stack_T2(case, planes=sel)).max() <= TOL
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     out = torch.empty_like(ref)
     bad = 0
-    for it in range(200):
-        if it & 1:
+    for it in range(calls):
+        if it % flush_every == 1:
             flush.fill_(it % 251)            # every other call starts from a cold L2
         plan.compute(out)
         bad += int(not torch.equal(out, ref))
     plan.destroy()
-    assert bad == 0
+    return bad
+
+
+def test_pair_kernels_are_deterministic_under_repetition(psf):
+    """Guards the cross-CTA hand-off of the producer-written operand rows in k1_pair (profiles/r1j_race_k1_pair.md: before
+    the fix about 4 % of config-5 calls had one plane computed from rows overwritten while still being read).  2000 calls:
+    config 5 as bench.py launches it; a pupil above 512 (the producers recompute the phasors per stage: another cadence);
+    config 5 in 6-plane launch pairs (short grids: every cluster starts and drains 43 times per call)."""
+    assert _repeat_bit_identical(psf, W.config5(), 1200) == 0
+    big = W.small_random_case(73, pupil_n=640, out_m=512, n_planes=32, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
+    assert _repeat_bit_identical(psf, big, 400) == 0
+    assert _repeat_bit_identical(psf, W.config5(), 400, tune=(psf.TUNE_TC_SCRATCH_MB, 64)) == 0
+
+
+@pytest.mark.skipif(not os.environ.get("PSF_SOAK"), reason="long soak: set PSF_SOAK=<calls> (e.g. 6000)")
+def test_pair_kernels_soak(psf):
+    """The long version (profiles/ records its runs): PSF_SOAK calls of config 5 plus half as many of a padded pair shape."""
+    n = int(os.environ["PSF_SOAK"])
+    assert _repeat_bit_identical(psf, W.config5(), n) == 0
+    pad = W.small_random_case(74, pupil_n=300, out_m=400, n_planes=64, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
+    assert _repeat_bit_identical(psf, pad, n // 2) == 0
