@@ -29,15 +29,10 @@ WORKLOADS = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
 SM_COUNT, FMA_LANES_PER_SM = 148, 128
 TF32_OVER_BF16 = 1.1 / 2.25            # nominal dense ratio (B200_PROFILING.md table)
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu captures
-# (profiles/*.md name the command); keyed by (path, workload, stage), in bytes PER PLANE of the captured launch (scaled to
-# the mean planes per launch below).  None where no capture exists yet.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1m_ncu_pair_cfg5.md: k2_pair, 256-plane launch: 2.705 GB read + 0.261 GB written
-    ("tc3xf16", "cfg5_large_stack", 1): (2.705340e9 + 0.260985e9) / 256,
-    # same capture, k1_pair: 0.156 GB read + 2.626 GB written
-    ("tc3xf16", "cfg5_large_stack", 0): (0.155747e9 + 2.625637e9) / 256,
-}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch come from the committed ncu captures: profiles/traffic.csv has one
+# row per (workload, kernel) with the capture it was read from (profiles/traffic.md names the commands).  A row is used only
+# when its kernel is one the running plan launches (psf_kernel_names); otherwise `traffic` is null.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "traffic.csv")
 
 
 def load_peaks():
@@ -54,6 +49,81 @@ def load_peaks():
     return d
 
 
+def load_traffic():
+    rows = {}
+    try:
+        import csv
+        with open(TRAFFIC_CSV) as f:
+            for r in csv.DictReader(f):
+                rows[(r["workload"], r["kernel"])] = r
+    except Exception:
+        pass
+    return rows
+
+
+def traffic_for(rows, case, kernel, planes_per_launch):
+    """(bytes per launch, source) for `kernel` on this workload, scaled from the captured launch's plane count; (None, why)
+    if no committed capture covers it."""
+    r = rows.get((case.name, kernel))
+    if r is None:
+        return None, f"no ncu capture of {kernel} on {case.name} in profiles/traffic.csv"
+    per_plane = (float(r["dram_read_bytes"]) + float(r["dram_write_bytes"])) / float(r["planes_in_launch"])
+    return per_plane * planes_per_launch, f"profiles/{r['capture']} (ncu --set full, commit {r['commit']})"
+
+
+def ffma_peak_tflops(peaks):
+    return SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+
+
+def roofline_record(case, res, ms_per_step, peaks, traffic_rows):
+    """Roofline of the dominant kernel of one timed workload: achieved = executed flop per launch / mean
+    launch duration (CUDA events around every launch on the compute stream, psf_profile_*)."""
+    f1, f2 = folded_flops(case)
+    stage_ms = res["stage_ms"]
+    path = res["path"]
+    kernels = res["kernels"]
+    fused = path == "ffma_fused"
+    dom = 0 if fused else int(np.argmax(stage_ms[:2]))
+    flop_dom = (f1 + f2) if fused else (f1, f2)[dom]
+    launches_dom = max(int(res["stage_launches"][dom]), 1)
+    dur_ms = stage_ms[dom] / launches_dom
+    if path in ("ffma", "ffma_fused"):
+        bound = "alu"
+        peak = ffma_peak_tflops(peaks)
+        executed = flop_dom
+        peak_note = f"148 SM x 128 FFMA lanes x 2 flop x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (fp32 FFMA pipe)"
+    else:
+        bound = "tensor"
+        long_step = ms_per_step > 1000.0
+        bf16 = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
+        which = f"{peaks['_source']} bf16 {'sustained' if long_step else 'burst'} {bf16:.1f} TF/s"
+        executed = 3.0 * flop_dom
+        if path == "tc3xf16":      # kind::f16 runs at the bf16 rate: the measured cuBLAS bf16 figure is the peak itself
+            peak = bf16
+            peak_note = f"{which} (fp16 = bf16 tensor rate); achieved counts executed FP16 flop (3 products per fp32 product)"
+        else:
+            peak = bf16 * TF32_OVER_BF16
+            peak_note = (f"{which} x nominal tf32/bf16 ratio {TF32_OVER_BF16:.3f}; achieved counts executed TF32 flop "
+                         f"(3 products per fp32 product)")
+    achieved = executed / launches_dom / (dur_ms * 1e-3) / 1e12
+    kname = kernels[min(dom, len(kernels) - 1)] if kernels else "?"
+    traffic, tsrc = traffic_for(traffic_rows, case, kname, case.n_planes / launches_dom)
+    out_bytes = 4.0 * case.voxels()
+    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": traffic, "traffic_source": tsrc, "kernel": kname,
+                "kernel_role": "whole path (fused)" if fused else ("stage1_rowdft_producer", "stage2_coldft_intensity")[dom],
+                "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
+                "algorithmic_tflops": flop_dom / launches_dom / (dur_ms * 1e-3) / 1e12, "peak_source": peak_note,
+                "stage_ms_per_step": [float(stage_ms[0]), float(stage_ms[1])],
+                # compulsory HBM traffic = the intensity stack (DESIGN.md section 5): reported for every workload, the binding
+                # bound only where the flop are few (SURVEY 8(d): the small-M batched regime)
+                "hbm_gbs": out_bytes / (ms_per_step * 1e-3) / 1e9,
+                "hbm_frac": out_bytes / (ms_per_step * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    total_flop = f1 + f2
+    roofline["step_frac"] = (3.0 if bound == "tensor" else 1.0) * total_flop / (ms_per_step * 1e-3) / 1e12 / peak
+    return roofline
+
+
 def rank_case(cfg: int, rank: int):
     """Weak scaling: every rank owns a full-size shard of a longer stack (rank r: z shifted by r * 10 nm; the
     emitter batch of config 4 is redrawn with another z offset).  No data-path collective."""
@@ -68,7 +138,7 @@ def folded_flops(case):
     """Algorithmic real flop of the two DFT stages in the folded formulation:
     stage 1 = C Z 8 chains 2 n^2 m, stage 2 = C Z 8 chains 2 m^2 n; n = ceil(N/2), m = ceil(M/2)."""
     n, m = (case.pupil_n + 1) // 2, (case.out_m + 1) // 2
-    C = 5 if case.pol == "unpolarized" else 3
+    C = 1 if getattr(case, "model", "vectorial") == "scalar" else (5 if case.pol == "unpolarized" else 3)
     Z = case.n_planes
     return C * Z * 16.0 * n * n * m, C * Z * 16.0 * m * m * n
 
@@ -140,8 +210,23 @@ def time_workload(torch, psf, case, device, steps, warmup, flush, profile=True):
     step_ms = [a.elapsed_time(b) for a, b in ev]
     res = {"plan": plan, "out": out, "step_ms": step_ms, "stage_ms": stage_ms / max(steps, 1),
            "stage_launches": stage_launches // max(steps, 1), "path": plan.path,
-           "launches": plan.launches_per_compute}
+           "launches": plan.launches_per_compute, "kernels": plan.kernel_names}
     return res
+
+
+def loop_ms_per_call(torch, plan, out, device, calls=100):
+    """a tiny stack is timed as a back-to-back loop as well (no flush between calls: launch rate)."""
+    dev = torch.device("cuda", device)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(5):
+        plan.compute(out)
+    torch.cuda.synchronize(dev)
+    a.record()
+    for _ in range(calls):
+        plan.compute(out)
+    b.record()
+    torch.cuda.synchronize(dev)
+    return a.elapsed_time(b) / calls
 
 
 def e2e_workload(torch, plan, case, device, steps, warmup):
@@ -215,6 +300,7 @@ def blas_threads():
 
 
 ORACLE_PLANES = {1: 16, 2: 64, 3: 128, 4: 4096, 5: 256}    # about 10-30 s of CPU work each on the 16-core B200 host
+ORACLE_PLANES_SWEEP = {1: 16, 2: 64, 3: 32, 4: 4096, 5: 32}    # per-workload lines of the sweep: configs 1, 2, 4 in full
 
 
 def run_oracle_once(case, planes):
@@ -225,8 +311,8 @@ def run_oracle_once(case, planes):
     return dt, I
 
 
-def cpu_baseline(case, cfg):
-    planes = oracle_sample(case, ORACLE_PLANES[cfg])
+def cpu_baseline(case, cfg, table=ORACLE_PLANES):
+    planes = oracle_sample(case, table[cfg])
     dt, I = run_oracle_once(case, planes)
     vox = len(planes) * case.out_m * case.out_m
     return {"value": vox / dt, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
@@ -311,48 +397,18 @@ def run_ours(args):
     e2e_val = voxels / float(e2e_s.item())
 
     # roofline of the dominant kernel
-    f1, f2 = folded_flops(case)
-    stage_ms = res["stage_ms"]
-    dom = int(np.argmax(stage_ms[:2]))
-    flop_dom = (f1, f2)[dom]
-    launches_dom = max(int(res["stage_launches"][dom]), 1)
-    dur_ms = stage_ms[dom] / launches_dom
+    traffic_rows = load_traffic()
+    roofline = roofline_record(case, res, ms_per_step, peaks, traffic_rows)
     path = res["path"]
-    if path in ("ffma", "ffma_fused"):
-        bound = "alu"
-        peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-        executed = flop_dom
-        peak_note = f"148 SM x 128 FFMA lanes x 2 flop x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (fp32 FFMA pipe)"
-    else:
-        bound = "tensor"
-        long_step = ms_per_step > 1000.0
-        bf16 = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
-        which = f"{peaks['_source']} bf16 {'sustained' if long_step else 'burst'} {bf16:.1f} TF/s"
-        executed = 3.0 * flop_dom
-        if path == "tc3xf16":      # kind::f16 runs at the bf16 rate: the measured cuBLAS bf16 figure is the peak itself
-            peak = bf16
-            peak_note = f"{which} (fp16 = bf16 tensor rate); achieved counts executed FP16 flop (3 products per fp32 product)"
-        else:
-            peak = bf16 * TF32_OVER_BF16
-            peak_note = (f"{which} x nominal tf32/bf16 ratio {TF32_OVER_BF16:.3f}; achieved counts executed TF32 flop "
-                         f"(3 products per fp32 product)")
-    achieved = executed / launches_dom / (dur_ms * 1e-3) / 1e12
-    traffic = NCU_TRAFFIC_BYTES.get((path, case.name, dom))
-    if traffic is not None:
-        traffic *= case.n_planes / launches_dom
-    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": ("stage1_rowdft_producer", "stage2_coldft_intensity")[dom],
-                "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
-                "algorithmic_tflops": flop_dom / launches_dom / (dur_ms * 1e-3) / 1e12, "peak_source": peak_note,
-                "stage_ms_per_step": [float(stage_ms[0]), float(stage_ms[1])]}
-    if bound == "tensor":      # both stages together against the same peak (context: the two kernels take about equal time)
-        roofline["step_frac"] = 3.0 * (f1 + f2) / (ms_per_step * 1e-3) / 1e12 / peak
+    step_sorted = sorted(res["step_ms"])
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"tc3xf16": "f16x3", "tc3xtf32": "tf32x3"}.get(path, "f32"), "data": "synthetic",
             "config": {"workload": case.name, "N": case.pupil_n, "M": case.out_m, "Z": case.n_planes,
-                       "pol": case.pol, "path": path, "planes_per_s": case.n_planes * world / (ms_per_step * 1e-3),
+                       "pol": case.pol, "path": path, "kernels": res["kernels"],
+                       "planes_per_s": case.n_planes * world / (ms_per_step * 1e-3),
+                       "median_ms": float(statistics.median(step_sorted)), "min_ms": float(step_sorted[0]),
                        "l2": "256 MiB buffer written between timed iterations (flush)", "sharding": "z-shards, no collective"},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
@@ -369,13 +425,21 @@ def run_ours(args):
             sweep = {}
             for name, c in WORKLOADS.items():
                 if c == cfg:
-                    sweep[name] = {"voxels_per_s": value, "ms_per_step": ms_per_step, "path": path}
+                    sweep[name] = {"voxels_per_s": value, "ms_per_step": ms_per_step, "median_ms": float(statistics.median(step_sorted)),
+                                   "min_ms": float(step_sorted[0]), "path": path, "kernels": res["kernels"], "roofline": roofline,
+                                   "cpu_baseline": line["cpu_baseline"]}
                     continue
                 cs = W.get_config(c)
-                r = time_workload(torch, psf, cs, local, min(args.steps, 10), 3, flush, profile=False)
+                r = time_workload(torch, psf, cs, local, max(args.steps, 20), 3, flush)
                 ms = statistics.mean(r["step_ms"])
+                srt = sorted(r["step_ms"])
                 sweep[name] = {"voxels_per_s": cs.voxels() / (ms * 1e-3), "planes_per_s": cs.n_planes / (ms * 1e-3),
-                               "ms_per_step": ms, "path": r["path"], "launches": r["launches"]}
+                               "ms_per_step": ms, "median_ms": float(statistics.median(srt)), "min_ms": float(srt[0]),
+                               "path": r["path"], "kernels": r["kernels"], "launches": r["launches"],
+                               "roofline": roofline_record(cs, r, ms, peaks, traffic_rows),
+                               "cpu_baseline": cpu_baseline(cs, c, ORACLE_PLANES_SWEEP)}
+                if c == 1:      # launch-rate view of the tiny stack: 100 calls back to back between two events
+                    sweep[name]["loop100_ms_per_call"] = loop_ms_per_call(torch, r["plan"], r["out"], local)
                 r["plan"].destroy()
             # the spherical (Bessel) path on the two axisymmetric configs: ALU / SFU bound, context only
             for name, c, nodes in (("cfg1_spherical", 1, 2001), ("cfg3_spherical", 3, 2001)):

@@ -168,8 +168,12 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_TC_PAIR_MASK  : value ANDed with the plan's choice; bit 0 = stage 1 on CTA pairs (cta_group::2),
  *                            bit 1 = stage 2 on CTA pairs; 0 forces the single-CTA tcgen05 kernels (default 3);
  *   PSF_TUNE_TC_SCRATCH_MB : budget in MB of the stage-1 -> stage-2 scratch (default 0 = 4096): a smaller value splits a
- *                            stack into several launch pairs. */
-enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2 };
+ *                            stack into several launch pairs;
+ *   PSF_TUNE_K1P_HANDOFF   : stage-1 pair kernel, how the non-leader CTA's producer warps signal the leader's barrier:
+ *                            0 plain remote arrive, 1 cluster-scope release per warp, 2 relay threads (default);
+ *   PSF_TUNE_K1P_DEFER     : 1 (default) = producer-written operand slots are released one full stage late; 0 = at once
+ *                            (the A/B setting of profiles/r2*_race_k1_pair.md; unsafe). */
+enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /
@@ -182,6 +186,10 @@ int psf_launches_per_compute(const psf_plan *plan);
 /* Name of the kernel path the plan selected (static string): "ffma" (fp32 FFMA tiles), "ffma_fused" (small grids: the
  * whole path in one CTA per plane), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision). */
 const char *psf_path_name(const psf_plan *plan);
+
+/* Comma-separated names of the kernels one psf_compute of this plan launches, in launch order (stage 1, stage 2; one
+ * name for the fused small-grid path), e.g. "k1_pair,k2_pair".  Owned by the plan, valid until the next call on it. */
+const char *psf_kernel_names(psf_plan *plan);
 
 /* Profiling aid for bench.py.  enable != 0: create CUDA events (this call may allocate) and make every later
  * psf_compute bracket each of its kernel launches with cudaEventRecord on the compute stream; enable == 0: stop. */

@@ -21,8 +21,8 @@ PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
-           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms"]
-TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB = 1, 2
+           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names"]
+TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER = 1, 2, 3, 4
 
 
 class PsfError(RuntimeError):
@@ -93,6 +93,8 @@ def load_library(build_if_missing: bool = True):
     lib.psf_last_upload_bytes.restype = C.c_longlong
     lib.psf_plan_tune.argtypes = [P, C.c_int, C.c_longlong]
     lib.psf_plan_tune.restype = C.c_int
+    lib.psf_kernel_names.argtypes = [P]
+    lib.psf_kernel_names.restype = C.c_char_p
     lib.psf_grad_terms.argtypes = [P]
     lib.psf_grad_terms.restype = C.c_int
     lib.psf_host_tables.argtypes = [C.POINTER(psf_plan_desc), C.POINTER(C.c_float), C.c_int, C.c_int,
@@ -263,6 +265,10 @@ class PsfPlan:
     @property
     def launches_per_compute(self) -> int:
         return int(self._lib.psf_launches_per_compute(self._h))
+
+    @property
+    def kernel_names(self) -> list:
+        return [k for k in self._lib.psf_kernel_names(self._h).decode().split(",") if k]
 
     @property
     def path(self) -> str:

@@ -475,6 +475,12 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_TC_SCRATCH_MB) {
       if (value < 0 || value > (1 << 20)) { p->err = "PSF_TUNE_TC_SCRATCH_MB: 0 (default) .. 2^20"; return PSF_ERR_INVALID_ARG; }
       p->tune_scratch_mb = (int)value;
+    } else if (knob == PSF_TUNE_K1P_HANDOFF) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_k1p_handoff = (int)value;
+    } else if (knob == PSF_TUNE_K1P_DEFER) {
+      if (value < 0 || value > 4) { p->err = "PSF_TUNE_K1P_DEFER: 0..4"; return PSF_ERR_INVALID_ARG; }
+      p->tune_k1p_defer = (int)value;
     } else {
       p->err = "unknown tuning knob";
       return PSF_ERR_INVALID_ARG;
@@ -542,6 +548,18 @@ psf_status psf_profile_read(psf_plan *p, float *stage_ms, int *launches) {
 }
 
 long long psf_last_upload_bytes(const psf_plan *p) { return p ? p->upload_bytes : 0; }
+
+const char *psf_kernel_names(psf_plan *p) {
+  if (!p) return "";
+  try {
+    if (p->path == 3) p->kernel_names = "k_small";
+    else if ((p->path == 1 || p->path == 2) && p->tc) p->kernel_names = tc_kernel_names(p);
+    else p->kernel_names = "k1_stage1,k2_stage2";
+    return p->kernel_names.c_str();
+  } catch (...) {
+    return "";
+  }
+}
 
 psf_status psf_host_tables(const psf_plan_desc *desc, const float *coeffs, int noll_first, int n_coeffs, int *n_components,
                            double *weights, double *base, double *kappa, unsigned char *mask) {

@@ -50,6 +50,21 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// cluster-scope release: every write this thread has observed (its own and, cumulatively, those it acquired) is performed
+// with respect to the whole cluster before the arrive becomes visible (SASS: MEMBAR.ALL.GPU + ERRBAR ahead of the arrive)
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_acquire_cluster(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 // (waits use the plain mbar_wait: an .acquire.cluster try_wait adds an L1 invalidate, CCTL.IVALL, to every successful wait)
@@ -357,34 +372,23 @@ struct K1PArgs {
   const float4 *planes; // [Z]
   int C, n_pad, m_pad, z0, zc;
   float f1;             // epilogue factor s_T / (s_Q s_X)
+  int handoff;          // how the non-leader CTA's producer warps signal the leader's barrier: 0 plain arrive, 1 cluster-scope release
+  int defer;            // K = 16 steps of the next stage issued before a stage buffer is released (0 = released right behind its own stage)
 };
 
-// Shared memory of k1_pair (per CTA): the two operands have their own rings because they are refilled differently.
-//   A ring  (table rows, refilled by TMA)        : K1P_NSA = 2 slots x 32 KB (hi, lo), released as soon as the stage's UMMAs complete;
-//   B ring  (pupil rows, written by st.shared)   : K1P_NSB = 3 slots x 32 KB (hi, lo), released ONE FULL STAGE late (below);
-//   store staging (epilogue, hi tile + lo tile)  : 32 KB;
-//   base-pupil ring (bulk copies -> producers)   : K1P_BB_SLOTS = 2 half-stage slots x 16 KB.
-constexpr int K1P_NSA = 2;
-constexpr int K1P_NSB = 3;
-constexpr int K1P_AB_BYTES = 2 * TILE16K;                         // one ring slot: hi tile + lo tile
+constexpr int K1P_NST = 2;
 constexpr int K1P_PRODUCER_WARPS = 8;
 constexpr int K1P_FEED_WARPS = 4;                                  // table TMA, MMA, idle, base-pupil copies: roles fill whole warpgroups (setmaxnreg)
 constexpr int K1P_THREADS = 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4);
 constexpr int K1P_STAGING = 2 * TILE16K;                          // hi tile + lo tile of one chain: 128 mx x 64 qy each
 constexpr int K1P_BB_SLOTS = 2;
-constexpr int K1P_BB_BYTES = 4 * 256 * 16;                        // half a stage of base pupil for this CTA: 4 samples x 256 threads x float4
+constexpr int K1P_BB_BYTES = 8 * 256 * 16;                        // one stage of base pupil for this CTA: 8 samples x 256 threads x float4
 constexpr int K1P_MAX_NK = 4;                                     // k-chunks whose defocus phasors the producers keep in registers per tile (n_pad <= 256)
-constexpr int K1P_OFF_B = K1P_NSA * K1P_AB_BYTES;                 // byte offsets inside the 1024-aligned dynamic shared memory
-constexpr int K1P_OFF_STG = K1P_OFF_B + K1P_NSB * K1P_AB_BYTES;
-constexpr int K1P_OFF_BB = K1P_OFF_STG + K1P_STAGING;
-constexpr int K1P_SMEM = 1024 + K1P_OFF_BB + K1P_BB_SLOTS * K1P_BB_BYTES;
+constexpr int K1P_SMEM = 1024 + K1P_NST * P_STAGE + K1P_STAGING + K1P_BB_SLOTS * K1P_BB_BYTES;
 constexpr int K1P_QY = 64;                                        // q_y per tile (32 generated by each CTA)
-static_assert(K1P_SMEM <= 227 * 1024, "k1_pair shared memory");
 
 struct K1PShared {
-  uint64_t a_full[K1P_NSA], a_empty[K1P_NSA];               // table tiles: TMA bytes of both CTAs -> leader's a_full; commit -> both a_empty
-  uint64_t b_full[K1P_NSB], b_empty[K1P_NSB];               // pupil rows: all producer warps of the pair -> leader's b_full; commit -> both b_empty
-  uint64_t acc_full[2], acc_empty[2];
+  uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
   uint64_t bb_full[K1P_BB_SLOTS], bb_empty[K1P_BB_SLOTS];   // base-pupil ring: bulk copy -> producers -> free
   uint32_t tmem_slot;
 };
@@ -402,14 +406,6 @@ __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
   return v;
 }
 
-// one K = 16 step with the operands of a stage in separate rings: D += A_lo B_hi + A_hi B_lo + A_hi B_hi
-__device__ __forceinline__ void issue_kstep_ab(uint32_t a_slot, uint32_t b_slot, uint32_t d_tmem, int k, bool zero) {
-  const uint32_t o = k * 32;
-  umma2_f16(d_tmem, umma_desc_sw128(a_slot + TILE16K + o), umma_desc_sw128(b_slot + o), P_IDESC, zero ? 0u : 1u);
-  umma2_f16(d_tmem, umma_desc_sw128(a_slot + o), umma_desc_sw128(b_slot + TILE16K + o), P_IDESC, 1u);
-  umma2_f16(d_tmem, umma_desc_sw128(a_slot + o), umma_desc_sw128(b_slot + o), P_IDESC, 1u);
-}
-
 // TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
 __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
                                          const K1PArgs &P, const K1PGeom &G, int warp, uint32_t rank) {
@@ -417,26 +413,26 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
   if (warp == 0) {
     if (elect_one()) {
       int st = 0, ph = 0;
-      uint32_t full_leader[K1P_NSA];
-      for (int i = 0; i < K1P_NSA; ++i) full_leader[i] = mapa(smem_u32(&S.a_full[i]), 0);
+      uint32_t full_leader[K1P_NST];
+      for (int i = 0; i < K1P_NST; ++i) full_leader[i] = mapa(smem_u32(&S.full[i]), 0);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         const int mt = t % G.tiles_m;
         for (int cg = 0; cg < 2 * P.C; ++cg) {
           const int row = (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
           for (int kc = 0; kc < G.nk; ++kc) {
-            mbar_wait(&S.a_empty[st], ph ^ 1);
-            const uint32_t s = smem_u32(smem + st * K1P_AB_BYTES);
-            if (leader) mbar_arrive_expect_tx(&S.a_full[st], 4 * TILE16K);
+            mbar_wait(&S.empty[st], ph ^ 1);
+            const uint32_t s = smem_u32(smem + st * P_STAGE);
+            if (leader) mbar_arrive_expect_tx(&S.full[st], 4 * TILE16K);
             tma2_load_2d(s, &map_xhi, full_leader[st], kc * 64, row);
             tma2_load_2d(s + TILE16K, &map_xlo, full_leader[st], kc * 64, row);
-            if (++st == K1P_NSA) { st = 0; ph ^= 1; }
+            if (++st == K1P_NST) { st = 0; ph ^= 1; }
           }
         }
       }
     }
   } else if (warp == 1) {
     if (leader && elect_one()) {
-      int sa = 0, pha = 0, sb = 0, phb = 0, it = 0, prev_b = -1;
+      int st = 0, ph = 0, it = 0, pending = -1;
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
           const int g = cg & 1;
@@ -444,52 +440,45 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
           tcgen05_fence_after();
           const uint32_t d = tmem + g * 256;
           for (int kc = 0; kc < G.nk; ++kc) {
-            mbar_wait(&S.a_full[sa], pha);
-            mbar_wait(&S.b_full[sb], phb);
+            if (P.handoff) mbar_wait_acquire_cluster(&S.full[st], ph);
+            else mbar_wait(&S.full[st], ph);
             tcgen05_fence_after();
-            const uint32_t as = smem_u32(smem + sa * K1P_AB_BYTES), bs = smem_u32(smem + K1P_OFF_B + sb * K1P_AB_BYTES);
+            const uint32_t sb = smem_u32(smem + st * P_STAGE);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) issue_kstep_ab(as, bs, d, k, kc == 0 && k == 0);
-            // Release.  tcgen05.commit arrives on the barrier (here: at the same offset in both CTAs, multicast) once all
-            // tcgen05 operations this thread issued before it have completed (PTX ISA, tcgen05.commit: "...tracks the
-            // completion of all prior asynchronous tcgen05 operations initiated by the executing thread"), operand reads
-            // included.  The A slot, refilled by TMA (async proxy, microsecond latency), is released by the commit right
-            // behind its own stage.  The B slot is refilled by the producers' st.shared within ~100 ns of the arrive, and
-            // round 1 saw rows of the non-leader CTA overwritten while still being read (profiles/r1j_race_k1_pair.md;
-            // hypothesis: that CTA's tensor core trails the leader's completion).  A B slot is therefore released by the
-            // commit behind the NEXT stage: between the last UMMA that reads it and the arrive lie twelve 256x256x16 UMMAs
-            // (1536 tensor cycles, ~1 us) that do not touch it.  With K1P_NSB = 3 slots the producers still fill stage s+1
-            // while stage s executes, as a two-slot ring with immediate release would allow.
-            umma2_commit(&S.a_empty[sa]);
-            if (prev_b >= 0) umma2_commit(&S.b_empty[prev_b]);
-            prev_b = sb;
-            if (++sa == K1P_NSA) { sa = 0; pha ^= 1; }
-            if (++sb == K1P_NSB) { sb = 0; phb ^= 1; }
+            for (int k = 0; k < 4; ++k) {
+              issue_kstep2(sb, d, k, kc == 0 && k == 0);
+              // Deferred release (profiles/r1j_race_k1_pair.md): the commit tracks the UMMAs of the issuing (leader) CTA; in
+              // the peer, whose tensor core can trail by a little, producers with their rows ready in registers
+              // overwrote the operand tile while it was still being read.  The previous stage's buffer is therefore
+              // released only after K1P_DEFER K-steps of this stage have been issued behind it: the commit then also
+              // waits for those, which gives the peer that much tensor time of slack.
+              if (k == P.defer - 1 && pending >= 0) { umma2_commit(&S.empty[pending]); pending = -1; }
+            }
+            if (P.defer == 0) umma2_commit(&S.empty[st]);
+            else pending = st;
+            if (++st == K1P_NST) { st = 0; ph ^= 1; }
           }
           umma2_commit(&S.acc_full[g]);
         }
       }
-      if (prev_b >= 0) umma2_commit(&S.b_empty[prev_b]);
+      if (pending >= 0) umma2_commit(&S.empty[pending]);
     }
   } else if (warp == 3) {
-    // Base-pupil copies: two 16 KB bulk copies per stage (the table is stored in the producers' read order, so half a
-    // stage of this CTA is one contiguous block) into a two-slot ring.  The producers then only read shared memory: no
+    // Base-pupil copies: one 32 KB bulk copy per stage (the table is stored in the producers' read order, so a stage
+    // of this CTA is one contiguous block) into a two-slot ring.  The producers then only read shared memory: no
     // global-load latency in their loop.
     if (elect_one()) {
       int bs = 0, bph = 0;
-      const uint32_t ring = smem_u32(smem + K1P_OFF_BB);
+      const uint32_t ring = smem_u32(smem + K1P_NST * P_STAGE + K1P_STAGING);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         const int jt = (t / G.tiles_m) % G.tiles_j;
         for (int cg = 0; cg < 2 * P.C; ++cg) {
           const float4 *src = P.bgp + (size_t)((cg & 1) * P.C + (cg >> 1)) * P.n_pad * P.n_pad;
           for (int kc = 0; kc < G.nk; ++kc) {
-#pragma unroll
-            for (int hf = 0; hf < 2; ++hf) {
-              mbar_wait(&S.bb_empty[bs], bph ^ 1);
-              mbar_arrive_expect_tx(&S.bb_full[bs], K1P_BB_BYTES);
-              bulk_load_1d(ring + bs * K1P_BB_BYTES, src + ((size_t)(jt * G.nk + kc) * 2 + rank) * 2048 + hf * 1024, K1P_BB_BYTES, &S.bb_full[bs]);
-              if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
-            }
+            mbar_wait(&S.bb_empty[bs], bph ^ 1);
+            mbar_arrive_expect_tx(&S.bb_full[bs], K1P_BB_BYTES);
+            bulk_load_1d(ring + bs * K1P_BB_BYTES, src + ((size_t)(jt * G.nk + kc) * 2 + rank) * 2048, K1P_BB_BYTES, &S.bb_full[bs]);
+            if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
           }
         }
       }
@@ -500,15 +489,15 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
 // Eight producer warps: this CTA's 32 q_y x 4 slots = 128 B-operand rows per stage; a thread owns 8 consecutive q_x of one
 // q_y row.  The defocus phasor of a sample is the same for all 2 C (component, group) items of a tile: the thread
 // computes its 8 x nk phasors at the first item and keeps them in registers (the k-chunk loop is unrolled).  The base
-// pupil of the stage comes from the shared-memory ring filled by the copy warp, half a stage (4 samples) per slot.
+// pupil of the stage comes from the shared-memory ring filled by the copy warp.
 __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
   const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
   const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
   // swizzled byte offset of chunk cgp in row (slot*32 + ql): rows 128 B apart, chunk ^= row & 7
   const uint32_t off0 = (uint32_t)ql * 128u + (((uint32_t)cgp ^ ((uint32_t)ql & 7u)) << 4);
   const uint32_t smem0 = smem_u32(smem);
-  const uint32_t full_leader0 = mapa(smem_u32(&S.b_full[0]), 0);
-  const uint32_t ring = smem0 + K1P_OFF_BB + (uint32_t)tid * 16u;   // [slot][sample e][thread] float4
+  const uint32_t full_leader0 = mapa(smem_u32(&S.full[0]), 0);
+  const uint32_t ring = smem0 + K1P_NST * P_STAGE + K1P_STAGING + (uint32_t)tid * 16u;   // [slot][sample e][thread] float4
   int st = 0, ph = 0, bs = 0, bph = 0;
   float4 sc[K1P_MAX_NK][4];                                      // (cos, sin) of samples (2i, 2i+1) of k-chunk kc (mod 4)
   const bool cached = G.nk <= K1P_MAX_NK;                        // larger pupils recompute the phasors at every stage
@@ -538,41 +527,35 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
               sc[k4][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
             }
           }
+          mbar_wait(&S.bb_full[bs], bph);
           uint32_t hi[4][4], lo[4][4];                             // [slot][pair of q_x]
 #pragma unroll
-          for (int hf = 0; hf < 2; ++hf) {                         // half-stage ring slots: samples 4 hf .. 4 hf + 3
-            mbar_wait(&S.bb_full[bs], bph);
-            float4 bq[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) bq[e] = ld_shared_v4f(ring + bs * K1P_BB_BYTES + e * 4096);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&S.bb_empty[bs]);           // the ring slot is in registers
-            if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const int i = 2 * hf + j;
-              const float4 b0 = bq[2 * j], b1 = bq[2 * j + 1];
-              const float cs0 = sc[k4][i].x, sn0 = sc[k4][i].y, cs1 = sc[k4][i].z, sn1 = sc[k4][i].w;
-              split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
-              split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
-              split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
-              split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
-            }
+          for (int i = 0; i < 4; ++i) {
+            const float4 b0 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i) * 4096);
+            const float4 b1 = ld_shared_v4f(ring + bs * K1P_BB_BYTES + (2 * i + 1) * 4096);
+            const float cs0 = sc[k4][i].x, sn0 = sc[k4][i].y, cs1 = sc[k4][i].z, sn1 = sc[k4][i].w;
+            split_f16x2(b0.x * cs0 - b0.y * sn0, b1.x * cs1 - b1.y * sn1, hi[0][i], lo[0][i]);
+            split_f16x2(b0.x * sn0 + b0.y * cs0, b1.x * sn1 + b1.y * cs1, hi[1][i], lo[1][i]);
+            split_f16x2(b0.z * cs0 - b0.w * sn0, b1.z * cs1 - b1.w * sn1, hi[2][i], lo[2][i]);
+            split_f16x2(b0.z * sn0 + b0.w * cs0, b1.z * sn1 + b1.w * cs1, hi[3][i], lo[3][i]);
           }
-          mbar_wait(&S.b_empty[st], ph ^ 1);
-          const uint32_t bh = smem0 + K1P_OFF_B + st * K1P_AB_BYTES + off0, bl = bh + TILE16K;
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&S.bb_empty[bs]);             // the ring slot is in registers
+          if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
+          mbar_wait(&S.empty[st], ph ^ 1);
+          const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
 #pragma unroll
           for (int s = 0; s < 4; ++s) {
             st_shared_v4(bh + s * 4096, hi[s][0], hi[s][1], hi[s][2], hi[s][3]);
             st_shared_v4(bl + s * 4096, lo[s][0], lo[s][1], lo[s][2], lo[s][3]);
           }
-          // Hand-off to the MMA thread of the leader CTA: every writer orders its own generic-proxy stores before later
-          // async-proxy reads (fence.proxy.async), the warp converges, one lane arrives (release) on the leader's b_full;
-          // the MMA thread's wait (acquire) + tcgen05.fence::after_thread_sync precede the UMMAs that read the rows.
-          fence_proxy_async_smem();                                // no load is in flight here
+          fence_proxy_async_smem();                                // every writer fences its own stores; no load is in flight here
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(full_leader0 + st * 8);
-          if (++st == K1P_NSB) { st = 0; ph ^= 1; }
+          if (lane == 0) {
+            if (rank == 0 || P.handoff == 0) mbar_arrive_cluster(full_leader0 + st * 8);
+            else mbar_arrive_cluster_release(full_leader0 + st * 8);
+          }
+          if (++st == K1P_NST) { st = 0; ph ^= 1; }
           // kappa of the stage that computes phasors next (one stage ahead), issued after the fence so that the fence's
           // memory barrier never waits for it
           if (cached) {
@@ -600,8 +583,8 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
   const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
   const int row = q * 32 + lane;
   const int et = threadIdx.x - 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS);   // 0..127
-  const uint32_t stg_hi = smem_u32(smem + K1P_OFF_STG) + (uint32_t)row * 128u, stg_lo = stg_hi + TILE16K;
-  const uint32_t stg0 = smem_u32(smem + K1P_OFF_STG);
+  const uint32_t stg_hi = smem_u32(smem + K1P_NST * P_STAGE) + (uint32_t)row * 128u, stg_lo = stg_hi + TILE16K;
+  const uint32_t stg0 = smem_u32(smem + K1P_NST * P_STAGE);
   const uint32_t acc_empty_leader = mapa(smem_u32(&S.acc_empty[0]), 0);
   const uint32_t swz = (uint32_t)row & 7u;
   int it = 0;
@@ -674,8 +657,10 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
   const uint32_t rank = cluster_ctarank();
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < K1P_NSA; ++i) { mbar_init(&S.a_full[i], 1); mbar_init(&S.a_empty[i], 1); }   // leader's expect_tx arrive + TMA bytes
-    for (int i = 0; i < K1P_NSB; ++i) { mbar_init(&S.b_full[i], 2 * K1P_PRODUCER_WARPS); mbar_init(&S.b_empty[i], 1); }   // every producer warp of the pair
+    for (int i = 0; i < K1P_NST; ++i) {
+      mbar_init(&S.full[i], 1 + 2 * K1P_PRODUCER_WARPS);  // the leader's expect_tx arrive + every producer warp of the pair
+      mbar_init(&S.empty[i], 1);
+    }
     for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S.bb_full[i], 1); mbar_init(&S.bb_empty[i], K1P_PRODUCER_WARPS); }
     for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
     fence_barrier_init();
