@@ -500,16 +500,100 @@ def run_ours(args):
     return 0
 
 
+def time_calls(torch, fn, flush, calls=20, warmup=3):
+    """Mean / min milliseconds of `calls` device-timed calls of fn(), L2 flushed before each."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for i in range(calls):
+        flush.fill_(float(i % 251))
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return statistics.mean(ts), min(ts)
+
+
+def run_fig5(args):
+    """--workload fig5: the paper's own benchmark shape (Fig. 5: one 201 x 201 plane at focus against the
+    pupil size, all four propagators) on this build, and the matrix-vs-FFT crossover study of SURVEY 8(f) NEXT-4: the
+    tensor-core product form against the chirp-Z / FFT form (PSF_PREC_CZT_FFT) at M = 201 and at M = N.  The paper prints no
+    numbers for Fig. 5 (plot only) and its library defaults are not stated: config-1 optics, x-polarised input for the
+    vectorial model, are used.  Context, not the headline metric."""
+    import torch
+    from dataclasses import replace
+    import paper_2502_03170_b200 as psf
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    base = replace(W.config1(), out_m=201, z_um=np.array([0.0]), name="fig5_single_plane")
+    sizes = [64, 128, 256, 512, 1024, 2048, 4096]
+    sampler = ClockSampler(0)
+    fig5, cross = [], []
+
+    def timed(case, precision, spherical_nodes=0):
+        plan = psf.plan_from_case(case, precision=precision)
+        out = torch.empty((case.n_planes, case.out_m, case.out_m), dtype=torch.float32, device=dev)
+        if spherical_nodes:
+            mean, mn = time_calls(torch, lambda: plan.compute_spherical(spherical_nodes, out), flush)
+            path = "spherical_bessel"
+        else:
+            mean, mn = time_calls(torch, lambda: plan.compute(out), flush)
+            path = plan.path
+        plan.destroy()
+        return {"us_mean": mean * 1e3, "us_min": mn * 1e3, "path": path}
+
+    for N in sizes:
+        row = {"N": N, "M": 201}
+        for model in ("vectorial", "scalar"):
+            c = replace(base, pupil_n=N, model=model)
+            row[model + "_cartesian"] = timed(c, "auto")
+            row[model + "_cartesian_czt_fft"] = timed(c, "czt_fft")
+            row[model + "_spherical"] = timed(c, "auto", spherical_nodes=N + 1)
+        fig5.append(row)
+    # crossover: stacks of 8 planes so that launch overhead does not hide the kernels; M = 201 and M = N
+    z8 = np.linspace(-1.0, 1.0, 8)
+    for N in [256, 512, 1024, 2048, 4096]:
+        for M in (201, N):
+            c = replace(base, pupil_n=N, out_m=M, z_um=z8, pixel_um=0.04 * 201 / M if M != 201 else 0.04)
+            a, f = timed(c, "auto"), timed(c, "czt_fft")
+            n, m = (N + 1) // 2, (M + 1) // 2
+            L = 1 << int(np.ceil(np.log2(N + M - 1)))
+            cross.append({"N": N, "M": M, "Z": 8, "matrix": a, "czt_fft": f, "fft_length": L,
+                          "matrix_executed_flop": 3 * 3 * 8 * 16.0 * n * m * (n + m),
+                          "fft_flop": 3 * 8 * (N + M) * 2 * 5.0 * L * np.log2(L),
+                          "ratio_czt_over_matrix": f["us_mean"] / a["us_mean"]})
+    clocks = sampler.stop()
+    ref = next(r for r in fig5 if r["N"] == 512)
+    ms = ref["vectorial_cartesian"]["us_mean"] * 1e-3
+    line = {"metric": METRIC, "value": 201 * 201 / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": 20, "warmup": 3,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16x3",
+            "data": "synthetic",
+            "config": {"workload": "fig5_single_plane (PAPER.md:239: one 201 x 201 plane at focus vs pupil size); value = the "
+                                   "N = 512 vectorial Cartesian point", "l2": "256 MiB buffer written between timed calls"},
+            "clocks": clocks, "fig5_us_per_psf": fig5, "crossover_matrix_vs_fft": cross, "gpu_launches": 2 * 20}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS) + ["fig5"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the per-workload table of the other four configs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.workload == "fig5":
+        if args.impl == "reference":
+            print(json.dumps({"impl": "reference", "unavailable": "the fig5 workload has no reference arm: the paper prints no numbers for Fig. 5"}))
+            return 0
+        return run_fig5(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

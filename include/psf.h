@@ -83,8 +83,13 @@ typedef enum {
   PSF_PREC_AUTO = 0,   /* the library picks per problem size: 3XF16 when the tensor tiles fill, FP32 otherwise  */
   PSF_PREC_3XTF32 = 1, /* tcgen05 tensor cores, both operands split hi/lo in TF32 (fp32-level accuracy)         */
   PSF_PREC_FP32 = 2,   /* plain fp32 FFMA tiles                                                                 */
-  PSF_PREC_3XF16 = 3   /* tcgen05 tensor cores, both operands pre-scaled by powers of two and split hi/lo in FP16:
+  PSF_PREC_3XF16 = 3,  /* tcgen05 tensor cores, both operands pre-scaled by powers of two and split hi/lo in FP16:
                           same 11-bit parts as 3XTF32, half the bytes, twice the tensor rate     */
+  PSF_PREC_CZT_FFT = 4 /* the paper's own formulation of the zoomed DFT: chirp-Z transform per row and
+                          column by hand-written shared-memory fp32 FFTs of length 2^ceil(log2(N + M - 1)) (Bluestein; an
+                          exact re-association of the same finite sum).  Static mode only (no per-plane Zernike rows or
+                          shifts: PSF_ERR_UNSUPPORTED), N + M - 1 <= 8192.  Never chosen by PSF_PREC_AUTO: on B200 the
+                          tensor-core product form is faster at every measured size (profiles/r2_czt_crossover.md)      */
 } psf_precision;
 
 typedef struct {
@@ -184,7 +189,7 @@ const char *psf_last_error(const psf_plan *plan);
 int psf_launches_per_compute(const psf_plan *plan);
 
 /* Name of the kernel path the plan selected (static string): "ffma" (fp32 FFMA tiles), "ffma_fused" (small grids: the
- * whole path in one CTA per plane), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision). */
+ * whole path in one CTA per plane), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision), "czt_fft" (chirp-Z by FFT). */
 const char *psf_path_name(const psf_plan *plan);
 
 /* Comma-separated names of the kernels one psf_compute of this plan launches, in launch order (stage 1, stage 2; one

@@ -16,7 +16,7 @@ STATUS_NAMES = {0: "PSF_OK", 1: "PSF_ERR_INVALID_ARG", 2: "PSF_ERR_UNSUPPORTED",
 POL = {"x": 0, "y": 1, "circ_l": 2, "circ_r": 3, "jones": 4, "unpolarized": 5}
 FLAG_APODIZE, FLAG_GIBSON_LANNI, FLAG_FRESNEL, FLAG_GAUSSIAN_ENVELOPE = 1, 2, 4, 8
 MODEL = {"vectorial": 0, "scalar": 1}
-PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3}
+PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3, "czt_fft": 4}
 
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",

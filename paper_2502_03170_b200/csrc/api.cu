@@ -98,6 +98,21 @@ psf_status upload_static(psf_plan *p) {
   for (int c = 0; c < 5; ++c) P.weight[c] = (float)hp.weight[c];
 
   tm.mark("apply_shared_zernike");
+  if (d.precision == PSF_PREC_CZT_FFT) {          // chirp-Z path: unfolded pupil with the input chirps folded in, plane table
+    std::string why;
+    if (!czt_supported(p, why)) { p->err = why; return PSF_ERR_UNSUPPORTED; }
+    std::vector<float4> planes(d.n_planes);
+    for (int b = 0; b < d.n_planes; ++b) {
+      float zh, zl;
+      split2(p->z[b], zh, zl);
+      planes[b] = make_float4(zh, zl, 0.f, 0.f);
+    }
+    psf_status sc;
+    if ((sc = upload(p, &p->d_planes, &p->cap_planes, planes)) != PSF_OK) return sc;
+    P.planes = (const float4 *)p->d_planes;
+    p->path = 4;
+    return czt_setup(p);
+  }
   std::vector<float4> &bfold = p->h_bfold;
   std::vector<float2> &kt = p->h_kt;
   bfold.resize((size_t)C * nn * 2);
@@ -214,6 +229,7 @@ psf_status upload_dft(psf_plan *p) {
 
 psf_status alloc_scratch(psf_plan *p) {
   const DevPlan &P = p->dp;
+  if (p->path == 4) return PSF_OK;              // the chirp-Z path owns its scratch
   const size_t per_plane = (size_t)P.C * 8 * P.n * P.m * sizeof(float);
   size_t zc = kScratchBudget / per_plane;
   if (zc < 1) zc = 1;
@@ -248,6 +264,7 @@ void free_all(psf_plan *p) {
   p->prof_ev.clear();
   if (p->done_ev) { cudaEventDestroy(p->done_ev); p->done_ev = nullptr; }
   tc_free(p);
+  czt_free(p);
   bessel_free(p);
   grad_free(p);
 }
@@ -300,8 +317,9 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
   }
   p->path = 0;
   build_host_pupil(p->desc, nullptr, 1, 0, p->hp0);
-  build_dft_phase(p->desc, p->phi);
-  if ((s = refresh(p)) != PSF_OK || (s = upload_dft(p)) != PSF_OK) {
+  const bool czt = p->desc.precision == PSF_PREC_CZT_FFT;
+  if (!czt) build_dft_phase(p->desc, p->phi);
+  if ((s = refresh(p)) != PSF_OK || (!czt && (s = upload_dft(p)) != PSF_OK)) {
     g_create_err = p->err;
     free_all(p);
     delete p;
@@ -390,6 +408,7 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool tc = p->path == 1 || p->path == 2;
   cudaError_t e = tc ? launch_tc(p, st, intensity, (float2 *)field)
+                     : p->path == 4 ? launch_czt(p, st, intensity, (float2 *)field)
                      : p->path == 3 ? launch_small(p, st, intensity, (float2 *)field)
                                     : launch_ffma(p, st, intensity, (float2 *)field);
   mark_inflight(p, st);
@@ -503,10 +522,11 @@ const char *psf_last_error(const psf_plan *p) { return p ? p->err.c_str() : g_cr
 int psf_launches_per_compute(const psf_plan *p) {
   if (!p) return 0;
   if (p->path == 3) return 1;
+  if (p->path == 4) return p->czt ? czt_launches(p) : 0;
   return (p->path >= 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
 }
 
-const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 3 ? "ffma_fused" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
+const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 4 ? "czt_fft" : p->path == 3 ? "ffma_fused" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
 
 psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!p) return PSF_ERR_INVALID_ARG;
@@ -518,6 +538,7 @@ psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!enable) return PSF_OK;
   size_t need = (size_t)ffma_launches(p) + 1;
   if (p->tc && (size_t)tc_launches(p) + 1 > need) need = (size_t)tc_launches(p) + 1;
+  if (p->czt && (size_t)czt_launches(p) + 1 > need) need = (size_t)czt_launches(p) + 1;
   while (p->prof_ev.size() < need) {
     cudaEvent_t ev;
     if ((e = cudaEventCreate(&ev)) != cudaSuccess) { p->err = std::string("cudaEventCreate: ") + cudaGetErrorString(e); return PSF_ERR_CUDA; }
@@ -553,6 +574,7 @@ const char *psf_kernel_names(psf_plan *p) {
   if (!p) return "";
   try {
     if (p->path == 3) p->kernel_names = "k_small";
+    else if (p->path == 4) p->kernel_names = "czt_rows,czt_cols";
     else if ((p->path == 1 || p->path == 2) && p->tc) p->kernel_names = tc_kernel_names(p);
     else p->kernel_names = "k1_stage1,k2_stage2";
     return p->kernel_names.c_str();

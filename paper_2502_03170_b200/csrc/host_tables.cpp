@@ -28,7 +28,7 @@ psf_status validate_desc(const psf_plan_desc *d, std::string &err) {
   if (d->pol == PSF_POL_JONES)
     for (int i = 0; i < 4; ++i)
       if (!std::isfinite(d->jones[i])) return bad("jones holds a non-finite value");
-  if ((int)d->precision < 0 || (int)d->precision > (int)PSF_PREC_3XF16) return bad("unknown precision");
+  if ((int)d->precision < 0 || (int)d->precision > (int)PSF_PREC_CZT_FFT) return bad("unknown precision");
   if (d->flags & ~(unsigned)(PSF_FLAG_APODIZE | PSF_FLAG_GIBSON_LANNI | PSF_FLAG_FRESNEL | PSF_FLAG_GAUSSIAN_ENVELOPE))
     return bad("unknown flag bit");
   if ((int)d->model != (int)PSF_MODEL_VECTORIAL && (int)d->model != (int)PSF_MODEL_SCALAR) return bad("unknown model");

@@ -39,6 +39,7 @@ struct DevPlan {
 struct TcState;      // tcgen05 path (kernels_tc.cu)
 struct BesselState;  // spherical parametrisation (kernels_bessel.cu)
 struct GradState;    // adjoint / gradients (kernels_grad.cu)
+struct CztState;     // chirp-Z by FFT (kernels_czt.cu)
 
 }  // namespace psf
 
@@ -78,10 +79,11 @@ struct psf_plan {
   size_t cap_zbq = 0, cap_coefq = 0;
   size_t T_bytes = 0;
   size_t cap_bfold = 0, cap_kt = 0, cap_bunf = 0, cap_zb = 0, cap_coef = 0, cap_planes = 0, cap_cos = 0, cap_sin = 0;
-  int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16, 3 = ffma_fused (small grids)
+  int path = 0;                  // 0 = ffma, 1 = tc3xtf32, 2 = tc3xf16, 3 = ffma_fused (small grids), 4 = czt_fft
   psf::TcState *tc = nullptr;
   psf::BesselState *bessel = nullptr;
   psf::GradState *grad = nullptr;
+  psf::CztState *czt = nullptr;
   // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
   int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
   int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
@@ -127,6 +129,12 @@ cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity, floa
 psf_status bessel_setup(psf_plan *p, int n_nodes);
 void bessel_free(psf_plan *p);
 cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
+// kernels_czt.cu
+bool czt_supported(const psf_plan *p, std::string &why);
+psf_status czt_setup(psf_plan *p);
+void czt_free(psf_plan *p);
+int czt_launches(const psf_plan *p);
+cudaError_t launch_czt(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 // kernels_grad.cu
 psf_status grad_setup(psf_plan *p);
 bool grad_needs_setup(const psf_plan *p);

@@ -497,3 +497,47 @@ def test_pair_kernels_soak(psf):
     assert _repeat_bit_identical(psf, W.config5(), n) == 0
     pad = W.small_random_case(74, pupil_n=300, out_m=400, n_planes=64, per_plane=False, shifts=False, pol=W.POL_UNPOLARIZED)
     assert _repeat_bit_identical(psf, pad, n // 2) == 0
+
+
+@pytest.mark.parametrize("seed,N,M,Z,pol", [(201, 2, 1, 1, W.POL_X), (202, 13, 8, 2, W.POL_JONES), (203, 37, 33, 3, W.POL_CIRC_R),
+                                            (204, 130, 67, 3, W.POL_UNPOLARIZED), (205, 300, 400, 2, W.POL_UNPOLARIZED),
+                                            (206, 512, 201, 2, W.POL_CIRC_L), (207, 1000, 201, 1, W.POL_X),
+                                            (208, 257, 768, 1, W.POL_Y)])
+def test_chirp_z_fft_path_matches_oracle(psf, seed, N, M, Z, pol):
+    """the paper's own formulation (chirp-Z transform by FFTs, here hand-written
+    shared-memory FFTs of length 2^ceil(log2(N+M-1))).  Bluestein's identity is an exact re-association of the same finite
+    sum, so the separable fp64 oracle is the oracle and 2e-5 of the plane peak is the bar; sizes cover FFT lengths 4 ... 2048
+    with odd and even log2, odd / even N and M, M > N and M < N, every polarisation, Gibson-Lanni and shared Zernike terms."""
+    case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, per_plane=False, shifts=False, pol=pol)
+    I, path = gpu_stack(psf, case, "czt_fft")
+    assert path == "czt_fft"
+    ref = O.stack_T2(case)
+    assert plane_errors(I, ref).max() <= TOL, (path, seed, plane_errors(I, ref))
+
+
+def test_chirp_z_fft_path_configs_field_and_refusals(psf):
+    for case in (W.config1(), W.config2(), replace(W.config3(), z_um=W.config3().z_um[::16])):
+        I, path = gpu_stack(psf, case, "czt_fft")
+        assert path == "czt_fft"
+        assert plane_errors(I, O.stack_T2(case)).max() <= TOL, case.name
+    # field output (output chirps applied), vectorial and scalar
+    for case in (replace(W.config2(), z_um=np.linspace(-2.0, 2.0, 3), pupil_n=96, out_m=50),
+                 replace(W.config1(), pupil_n=70, out_m=45, z_um=np.array([-0.3, 0.2]), model="scalar", envelope_s=0.9)):
+        (I, F), path = gpu_stack(psf, case, "czt_fft", want_field=True)
+        Eref = O.field_T2(case)
+        assert F.shape == Eref.shape and np.abs(F - Eref).max() <= 2e-5 * np.abs(Eref).max()
+        assert np.abs(np.sum(np.abs(F) ** 2, axis=0) - I).max() <= 1e-5 * I.max()
+    # per-plane rows / shifts are not offered on this path
+    plan = psf.PsfPlan(W.config1(), precision="czt_fft")
+    with pytest.raises(psf.PsfError) as e:
+        plan.set_shifts(np.zeros((16, 2), np.float32))
+    assert e.value.status == 2
+    plan.destroy()
+    # new shared coefficients after creation
+    case = W.small_random_case(209, pupil_n=90, out_m=70, n_planes=2, per_plane=False, shifts=False)
+    plan = psf.plan_from_case(case, precision="czt_fft")
+    other = replace(case, zernike=(-0.5 * case.zernike).astype(np.float32))
+    plan.set_zernike(other.zernike, other.noll_first)
+    I = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(I, O.stack_T2(other)).max() <= TOL
+    plan.destroy()
