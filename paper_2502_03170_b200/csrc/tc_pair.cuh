@@ -392,7 +392,29 @@ struct K1PShared {
   uint64_t bb_full[K1P_BB_SLOTS], bb_empty[K1P_BB_SLOTS];   // base-pupil ring: bulk copy -> producers -> free
   uint32_t tmem_slot;
 };
-struct K1PGeom { int nk, tiles_j, tiles_m, ntiles, ncl, cid; };
+struct K1PGeom { int nk, tiles_j, tiles_m, ntiles, ncl, cid, nitems; };
+
+// Two tilings share the kernel (template parameter GM):
+//   GM = false (m_pad a multiple of 256): a tile is (plane, 64 q_y, 256 m_x); the CTAs of a pair hold the two 128-row halves
+//       of the table rows (A) and generate the two 32-q_y halves of the pupil rows (B); 2 C items (component, x-parity group)
+//       per tile, every accumulator column is used.
+//   GM = true ("group mode", m_pad an odd multiple of 128, i.e. output half-sizes up to 128 and 257..384, ...): a tile is
+//       (plane, 32 q_y, 128 m_x) and the pair splits by x-parity GROUP instead: CTA 0 holds the cos rows of the 128 m_x and
+//       generates the x-even chains, CTA 1 holds the sin rows and generates the x-odd chains, C items per tile.  Each CTA's
+//       accumulator half that multiplies its table with the other group's chains is computed and discarded: half of the
+//       tensor work is waste, in exchange for the pair kernel's producer / epilogue machinery on shapes that have only 128
+//       output rows (before: the single-CTA k1_tc at 0.24 of the tensor peak, issue-bound).
+template <bool GM> struct K1PTile {
+  int mt, jt, zl, jt64, half;
+  __device__ __forceinline__ K1PTile(int t, const K1PGeom &G, uint32_t rank) {
+    mt = t % G.tiles_m;
+    const int r = t / G.tiles_m;
+    jt = r % G.tiles_j;
+    zl = r / G.tiles_j;
+    jt64 = GM ? (jt >> 1) : jt;
+    half = GM ? (jt & 1) : (int)rank;            // which 32-q_y half of the 64-q_y table block this CTA generates
+  }
+};
 
 // 1-D bulk copy global -> shared of this CTA, completion bytes on a local mbarrier
 __device__ __forceinline__ void bulk_load_1d(uint32_t smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
@@ -407,6 +429,7 @@ __device__ __forceinline__ float4 ld_shared_v4f(uint32_t saddr) {
 }
 
 // TMA warp (both CTAs: table rows of the CTA's own 128 mx) and MMA warp (leader CTA)
+template <bool GM>
 __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
                                          const K1PArgs &P, const K1PGeom &G, int warp, uint32_t rank) {
   const bool leader = rank == 0;
@@ -417,8 +440,8 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
       for (int i = 0; i < K1P_NST; ++i) full_leader[i] = mapa(smem_u32(&S.full[i]), 0);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
         const int mt = t % G.tiles_m;
-        for (int cg = 0; cg < 2 * P.C; ++cg) {
-          const int row = (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
+        for (int cg = 0; cg < G.nitems; ++cg) {
+          const int row = GM ? (int)rank * P.m_pad + mt * 128 : (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
           for (int kc = 0; kc < G.nk; ++kc) {
             mbar_wait(&S.empty[st], ph ^ 1);
             const uint32_t s = smem_u32(smem + st * P_STAGE);
@@ -434,8 +457,8 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
     if (leader && elect_one()) {
       int st = 0, ph = 0, it = 0, pending = -1;
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-        for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
-          const int g = cg & 1;
+        for (int cg = 0; cg < G.nitems; ++cg, ++it) {
+          const int g = it & 1;                                      // accumulator half (= the x-parity group when GM is false)
           mbar_wait(&S.acc_empty[g], ((it >> 1) & 1) ^ 1);
           tcgen05_fence_after();
           const uint32_t d = tmem + g * 256;
@@ -471,13 +494,14 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
       int bs = 0, bph = 0;
       const uint32_t ring = smem_u32(smem + K1P_NST * P_STAGE + K1P_STAGING);
       for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-        const int jt = (t / G.tiles_m) % G.tiles_j;
-        for (int cg = 0; cg < 2 * P.C; ++cg) {
-          const float4 *src = P.bgp + (size_t)((cg & 1) * P.C + (cg >> 1)) * P.n_pad * P.n_pad;
+        const K1PTile<GM> T(t, G, rank);
+        for (int cg = 0; cg < G.nitems; ++cg) {
+          const int grp = GM ? (int)rank : (cg & 1), c = GM ? cg : (cg >> 1);
+          const float4 *src = P.bgp + (size_t)(grp * P.C + c) * P.n_pad * P.n_pad;
           for (int kc = 0; kc < G.nk; ++kc) {
             mbar_wait(&S.bb_empty[bs], bph ^ 1);
             mbar_arrive_expect_tx(&S.bb_full[bs], K1P_BB_BYTES);
-            bulk_load_1d(ring + bs * K1P_BB_BYTES, src + ((size_t)(jt * G.nk + kc) * 2 + rank) * 2048, K1P_BB_BYTES, &S.bb_full[bs]);
+            bulk_load_1d(ring + bs * K1P_BB_BYTES, src + ((size_t)(T.jt64 * G.nk + kc) * 2 + T.half) * 2048, K1P_BB_BYTES, &S.bb_full[bs]);
             if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
           }
         }
@@ -490,6 +514,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
 // q_y row.  The defocus phasor of a sample is the same for all 2 C (component, group) items of a tile: the thread
 // computes its 8 x nk phasors at the first item and keeps them in registers (the k-chunk loop is unrolled).  The base
 // pupil of the stage comes from the shared-memory ring filled by the copy warp.
+template <bool GM>
 __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K1PArgs &P, const K1PGeom &G, int lane, uint32_t rank) {
   const int tid = threadIdx.x - 32 * K1P_FEED_WARPS;
   const int ql = tid >> 3, cgp = tid & 7;                        // row within the CTA's 32 q_y, 16-byte chunk (8 q_x)
@@ -503,17 +528,17 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
   const bool cached = G.nk <= K1P_MAX_NK;                        // larger pupils recompute the phasors at every stage
   float4 kt[4];
   // kappa of (tile, kc): [jt][kc][half][4 sample pairs][256 threads] float4
-  auto load_kt = [&](int jt, int kc) {
-    const float4 *k4 = P.ktq + ((size_t)(jt * G.nk + kc) * 2 + rank) * 1024 + tid;
+  auto load_kt = [&](int t, int kc) {                           // kappa of (tile t, k-chunk kc)
+    const K1PTile<GM> T(t, G, rank);
+    const float4 *k4 = P.ktq + ((size_t)(T.jt64 * G.nk + kc) * 2 + T.half) * 1024 + tid;
 #pragma unroll
     for (int i = 0; i < 4; ++i) kt[i] = __ldg(k4 + i * 256);
   };
-  if (G.cid < G.ntiles) load_kt((G.cid / G.tiles_m) % G.tiles_j, 0);
+  if (G.cid < G.ntiles) load_kt(G.cid, 0);
   for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-    const int r = t / G.tiles_m;
-    const int jt = r % G.tiles_j;
-    const float4 pl = __ldg(P.planes + P.z0 + r / G.tiles_j);
-    for (int cg = 0; cg < 2 * P.C; ++cg) {
+    const K1PTile<GM> T(t, G, rank);
+    const float4 pl = __ldg(P.planes + P.z0 + T.zl);
+    for (int cg = 0; cg < G.nitems; ++cg) {
      for (int kcb = 0; kcb < G.nk; kcb += K1P_MAX_NK) {
 #pragma unroll
       for (int k4 = 0; k4 < K1P_MAX_NK; ++k4) {
@@ -559,14 +584,14 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           // kappa of the stage that computes phasors next (one stage ahead), issued after the fence so that the fence's
           // memory barrier never waits for it
           if (cached) {
-            if (cg == 0 && kc + 1 < G.nk) load_kt(jt, kc + 1);
-            if (cg == 2 * P.C - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+            if (cg == 0 && kc + 1 < G.nk) load_kt(t, kc + 1);
+            if (cg == G.nitems - 1 && kc == G.nk - 1 && t + G.ncl < G.ntiles) load_kt(t + G.ncl, 0);
           } else if (kc + 1 < G.nk) {
-            load_kt(jt, kc + 1);
-          } else if (cg + 1 < 2 * P.C) {
-            load_kt(jt, 0);
+            load_kt(t, kc + 1);
+          } else if (cg + 1 < G.nitems) {
+            load_kt(t, 0);
           } else if (t + G.ncl < G.ntiles) {
-            load_kt(((t + G.ncl) / G.tiles_m) % G.tiles_j, 0);
+            load_kt(t + G.ncl, 0);
           }
         }
       }
@@ -576,48 +601,52 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
 }
 
 // Four epilogue warps: TMEM -> scale -> fp16 hi / lo -> swizzled staging tiles -> TMA store of T^T[chain][mx][qy].
-// The hi tile and the lo tile are separate 16 KB buffers, each stored by its own bulk group, so writing one overlaps the
-// TMA read of the other.
+// The hi tile and the lo tile are separate buffers, each stored by its own bulk group, so writing one overlaps the
+// TMA read of the other.  GM = false: 64 q_y per row (128-byte rows, SWIZZLE_128B); GM = true: this CTA's own 128
+// accumulator columns only, 32 q_y per row (64-byte rows, SWIZZLE_64B: 16-byte chunk ^= (row >> 1) & 3).
+template <bool GM>
 __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_this, const CUtensorMap &map_tlos,
                                              const K1PArgs &P, const K1PGeom &G, int warp, int lane, uint32_t rank) {
   const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
   const int row = q * 32 + lane;
   const int et = threadIdx.x - 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS);   // 0..127
-  const uint32_t stg_hi = smem_u32(smem + K1P_NST * P_STAGE) + (uint32_t)row * 128u, stg_lo = stg_hi + TILE16K;
   const uint32_t stg0 = smem_u32(smem + K1P_NST * P_STAGE);
+  const uint32_t stg_hi = stg0 + (uint32_t)row * (GM ? 64u : 128u), stg_lo = stg_hi + TILE16K;
   const uint32_t acc_empty_leader = mapa(smem_u32(&S.acc_empty[0]), 0);
-  const uint32_t swz = (uint32_t)row & 7u;
+  const uint32_t swz = GM ? (((uint32_t)row >> 1) & 3u) : ((uint32_t)row & 7u);
   int it = 0;
   for (int t = G.cid; t < G.ntiles; t += G.ncl) {
-    const int mt = t % G.tiles_m;
-    const int r = t / G.tiles_m;
-    const int jt = r % G.tiles_j;
-    const int zl = r / G.tiles_j;
-    const int mx0 = mt * 256 + (int)rank * 128;
-    for (int cg = 0; cg < 2 * P.C; ++cg, ++it) {
-      const int g = cg & 1, c = cg >> 1;
+    const K1PTile<GM> T(t, G, rank);
+    const int mx0 = GM ? T.mt * 128 : T.mt * 256 + (int)rank * 128;
+    const int qy0 = T.jt * (GM ? 32 : K1P_QY);
+    for (int cg = 0; cg < G.nitems; ++cg, ++it) {
+      const int g = it & 1;                                            // accumulator half
+      const int grp = GM ? (int)rank : (cg & 1), c = GM ? cg : (cg >> 1);
       mbar_wait(&S.acc_full[g], (it >> 1) & 1);
       tcgen05_fence_after();
 #pragma unroll 1
-      for (int s = 0; s < 4; ++s) {
-        const int chain = (zl * P.C + c) * 8 + (s >> 1) * 4 + g * 2 + (s & 1);     // chain index of slot s in group g
+      for (int s = 0; s < (GM ? 2 : 4); ++s) {
+        // GM false: round s = slot s (one chain), both q_y halves.  GM true: round s = slots 2 s and 2 s + 1 of this CTA's
+        // group = two consecutive chains, stored by one TMA box of 2 chains (the staging tile holds them back to back).
+        const int chain = (T.zl * P.C + c) * 8 + (GM ? s * 4 + grp * 2 : (s >> 1) * 4 + grp * 2 + (s & 1));
         uint32_t pl[2][16];
         // the hi buffer was handed to the TMA store two bulk groups ago (hi, lo of the previous slot)
         if (et == 0) bulk_wait_read<1>();
         named_bar_sync(2, 128);
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {            // q_y half h was generated by CTA h: columns h*128 + s*32 + 0..31
+        for (int h = 0; h < 2; ++h) {            // GM false: q_y half h was generated by CTA h: columns h*128 + s*32 + 0..31
           uint32_t v[32], ph[16];
-          tmem_ld_32x32b_x32(tmem + ((uint32_t)(q * 32) << 16) + g * 256 + h * 128 + s * 32, v);
+          tmem_ld_32x32b_x32(tmem + ((uint32_t)(q * 32) << 16) + g * 256 + (GM ? (int)rank * 128 + (2 * s + h) * 32 : h * 128 + s * 32), v);
           tmem_ld_wait();
 #pragma unroll
           for (int e = 0; e < 16; ++e)
             split_f16x2(__uint_as_float(v[2 * e]) * P.f1, __uint_as_float(v[2 * e + 1]) * P.f1, ph[e], pl[h][e]);
 #pragma unroll
-          for (int j = 0; j < 4; ++j)            // 16-byte chunk h*4 + j of the 128-byte row
-            st_shared_v4(stg_hi + ((((uint32_t)(h * 4 + j)) ^ swz) << 4), ph[4 * j], ph[4 * j + 1], ph[4 * j + 2], ph[4 * j + 3]);
+          for (int j = 0; j < 4; ++j)            // GM false: 16-byte chunk h*4 + j of the 128-byte row; GM true: chunk j of the 64-byte row of chain h
+            st_shared_v4(stg_hi + (GM ? (uint32_t)h * 8192u + ((((uint32_t)j) ^ swz) << 4) : ((((uint32_t)(h * 4 + j)) ^ swz) << 4)),
+                         ph[4 * j], ph[4 * j + 1], ph[4 * j + 2], ph[4 * j + 3]);
         }
-        if (s == 3) {                            // every TMEM read of this item is done: release the accumulator
+        if (s == (GM ? 1 : 3)) {                 // every TMEM read of this item is done: release the accumulator
           tcgen05_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(acc_empty_leader + g * 8);
@@ -625,7 +654,7 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
         fence_proxy_async_smem();
         named_bar_sync(2, 128);
         if (et == 0) {
-          tma_store_3d(&map_this, stg0, jt * K1P_QY, mx0, chain);
+          tma_store_3d(&map_this, stg0, qy0, mx0, chain);
           bulk_commit();
           bulk_wait_read<1>();                   // the lo buffer of the previous slot has been read
         }
@@ -634,11 +663,12 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
         for (int h = 0; h < 2; ++h)
 #pragma unroll
           for (int j = 0; j < 4; ++j)
-            st_shared_v4(stg_lo + ((((uint32_t)(h * 4 + j)) ^ swz) << 4), pl[h][4 * j], pl[h][4 * j + 1], pl[h][4 * j + 2], pl[h][4 * j + 3]);
+            st_shared_v4(stg_lo + (GM ? (uint32_t)h * 8192u + ((((uint32_t)j) ^ swz) << 4) : ((((uint32_t)(h * 4 + j)) ^ swz) << 4)),
+                         pl[h][4 * j], pl[h][4 * j + 1], pl[h][4 * j + 2], pl[h][4 * j + 3]);
         fence_proxy_async_smem();
         named_bar_sync(2, 128);
         if (et == 0) {
-          tma_store_3d(&map_tlos, stg0 + TILE16K, jt * K1P_QY, mx0, chain);
+          tma_store_3d(&map_tlos, stg0 + TILE16K, qy0, mx0, chain);
           bulk_commit();
         }
       }
@@ -647,6 +677,7 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
   if (et == 0) bulk_wait_all();
 }
 
+template <bool GM>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K1P_THREADS, 1)
 k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
         const __grid_constant__ CUtensorMap map_this, const __grid_constant__ CUtensorMap map_tlos, const K1PArgs P) {
@@ -675,22 +706,23 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
 
   K1PGeom G;
   G.nk = P.n_pad / 64;
-  G.tiles_j = P.n_pad / K1P_QY;
-  G.tiles_m = P.m_pad / 256;
-  G.ntiles = P.zc * G.tiles_j * G.tiles_m;                        // a tile = (plane, jt, mx pair-tile); c and g loop inside
+  G.tiles_j = P.n_pad / (GM ? 32 : K1P_QY);
+  G.tiles_m = P.m_pad / (GM ? 128 : 256);
+  G.ntiles = P.zc * G.tiles_j * G.tiles_m;                        // a tile = (plane, q_y tile, m_x tile); the items loop inside
+  G.nitems = GM ? P.C : 2 * P.C;
   G.ncl = gridDim.x >> 1;
   G.cid = blockIdx.x >> 1;
 
   // register budget (launch: 512 x 128; setmaxnreg acts on whole warpgroups): feeders 24, producers 184, epilogue 104
   if (warp < K1P_FEED_WARPS) {
     setmaxnreg_dec<24>();
-    k1p_feed(smem, S, tmem, map_xhi, map_xlo, P, G, warp, rank);
+    k1p_feed<GM>(smem, S, tmem, map_xhi, map_xlo, P, G, warp, rank);
   } else if (warp < K1P_FEED_WARPS + K1P_PRODUCER_WARPS) {
     setmaxnreg_inc<184>();
-    k1p_produce(smem, S, P, G, lane, rank);
+    k1p_produce<GM>(smem, S, P, G, lane, rank);
   } else {
     setmaxnreg_dec<104>();
-    k1p_epilogue(smem, S, tmem, map_this, map_tlos, P, G, warp, lane, rank);
+    k1p_epilogue<GM>(smem, S, tmem, map_this, map_tlos, P, G, warp, lane, rank);
   }
   tcgen05_fence_before();
   __syncthreads();
