@@ -82,7 +82,7 @@ def roofline_record(case, res, ms_per_step, peaks, traffic_rows):
     stage_ms = res["stage_ms"]
     path = res["path"]
     kernels = res["kernels"]
-    fused = path == "ffma_fused"
+    fused = path == "ffma_fused" or kernels == ["k12_fused"]      # one kernel does the whole path
     dom = 0 if fused else int(np.argmax(stage_ms[:2]))
     flop_dom = (f1 + f2) if fused else (f1, f2)[dom]
     launches_dom = max(int(res["stage_launches"][dom]), 1)

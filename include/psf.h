@@ -177,8 +177,11 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_K1P_HANDOFF   : stage-1 pair kernel, how the non-leader CTA's producer warps signal the leader's barrier:
  *                            0 plain remote arrive, 1 cluster-scope release per warp, 2 relay threads (default);
  *   PSF_TUNE_K1P_DEFER     : 1 (default) = producer-written operand slots are released one full stage late; 0 = at once
- *                            (the A/B setting of profiles/r2*_race_k1_pair.md; unsafe). */
-enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4 };
+ *                            (the A/B setting of profiles/r2*_race_k1_pair.md; unsafe);
+ *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
+ *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
+ *                            clusters, so that it stays in L2; 0 = always two kernels. */
+enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

@@ -248,6 +248,10 @@ psf_status alloc_scratch(psf_plan *p) {
 
 psf_status refresh(psf_plan *p) {
   if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+  if (tc_fused_aborted(p)) {
+    p->err = "an earlier psf_compute of this plan (fused launch) gave up waiting for a stage-1 / stage-2 dependency: its stack is invalid";
+    return PSF_ERR_CUDA;
+  }
   p->upload_bytes = 0;
   ++p->table_version;
   psf_status s = upload_static(p);
@@ -494,6 +498,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_TC_SCRATCH_MB) {
       if (value < 0 || value > (1 << 20)) { p->err = "PSF_TUNE_TC_SCRATCH_MB: 0 (default) .. 2^20"; return PSF_ERR_INVALID_ARG; }
       p->tune_scratch_mb = (int)value;
+    } else if (knob == PSF_TUNE_TC_FUSED) {
+      if (value < 0 || value > 8) { p->err = "PSF_TUNE_TC_FUSED: 0 (off), 1 (on), 2..8 (on, ring depth forced)"; return PSF_ERR_INVALID_ARG; }
+      p->tune_fused = (int)value;
     } else if (knob == PSF_TUNE_K1P_HANDOFF) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_handoff = (int)value;

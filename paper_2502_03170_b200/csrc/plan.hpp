@@ -87,6 +87,7 @@ struct psf_plan {
   // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
   int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
   int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
+  int tune_fused = 1;            // 1: both stages in one launch (k12_fused) where eligible; 0: always two launches
   int tune_k1p_handoff = 0;      // k1_pair: 0 plain remote arrive, 1 .release.cluster arrive per producer warp of the non-leader CTA
   int tune_k1p_defer = 1;        // k1_pair: K = 16 steps of the next stage issued before a stage buffer is released
   cudaEvent_t done_ev = nullptr; // recorded on the caller's stream after the last launch of every compute call: table
@@ -123,6 +124,7 @@ psf_status tc_setup(psf_plan *p, const std::vector<float4> &bfold, const std::ve
                     bool f16);
 void tc_free(psf_plan *p);
 int tc_launches(const psf_plan *p);
+bool tc_fused_aborted(const psf_plan *p);
 const char *tc_kernel_names(const psf_plan *p);
 cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
 // kernels_bessel.cu

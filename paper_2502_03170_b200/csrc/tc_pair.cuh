@@ -146,6 +146,52 @@ struct K2PArgs {
   float fscale;         // 1 / (s_X s_T): accumulator -> field
 };
 
+// ---- fused launch (k12_fused): both stages in one persistent kernel, stage-2 clusters consuming T^T right behind the stage-1
+// clusters that produce it, so that the hand-off scratch is a small ring that stays in L2 instead of a 2.7 GB round trip
+// through HBM (config 5).  Global flags carry the dependencies:
+//   ready[z C + c]    += 1 by each stage-1 CTA whose TMA stores of (plane z, component c) have completed   (target 2 a1)
+//   consumed[z C + c] += 1 by each stage-2 cluster whose TMA loads of (plane z, component c) have landed  (target a2)
+// Clusters are scheduled round-robin over tiles, a1 (a2) consecutive stage-1 (stage-2) tiles per plane, n1 = Pg a1 stage-1
+// clusters and Pg a2 stage-2 clusters: Pg planes are in flight, plane z belongs to group z % Pg, and the (plane, component)
+// units of a group rotate through U ring slots of the scratch.  Everything is resident at once (one cluster per SM pair),
+// so the spins cannot deadlock; a spin that runs out sets `abort`, after which nobody waits (the results are then wrong and
+// the host reports it, but the launch ends).
+struct FuseCtx {
+  int *ready, *consumed, *abort;
+  int n1, a1, a2, Pg, U;
+};
+struct FuseUnit { int ring, prev; };     // ring unit of (plane, component); flag index of the unit that used the slot before (-1: none)
+__device__ __forceinline__ FuseUnit fuse_unit(const FuseCtx &F, int C, int zl, int c) {
+  const int gi = zl % F.Pg, k = zl / F.Pg;
+  const int i = k * C + c;
+  FuseUnit u;
+  u.ring = gi * F.U + i % F.U;
+  const int ip = i - F.U;
+  u.prev = ip < 0 ? -1 : (gi + (ip / C) * F.Pg) * C + ip % C;
+  return u;
+}
+__device__ __forceinline__ int ld_acquire_gpu(const int *p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_gpu_add(int *p, int v) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void fuse_wait(const FuseCtx &F, const int *flag, int target) {
+  unsigned spins = 0;
+  while (ld_acquire_gpu(flag) < target) {
+    __nanosleep(40);
+    if ((++spins & 0xFFFu) == 0) {
+      if (ld_acquire_gpu(F.abort)) break;
+      if (spins > (1u << 24)) { atomicExch(F.abort, 1); break; }      // ~1 s: something is wrong; stop waiting everywhere
+    }
+  }
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait_complete() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+
 constexpr int K2P_NST = 3;
 constexpr int K2P_EPI_WARPS = 16;
 constexpr int K2P_THREADS = 32 * (4 + K2P_EPI_WARPS);
@@ -159,9 +205,10 @@ struct K2PShared {
 };
 
 // TMA warp (both CTAs) and MMA warp (leader CTA)
+template <bool FUSED>
 __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t tmem, const CUtensorMap &map_xhi, const CUtensorMap &map_xlo,
                                          const CUtensorMap &map_thi, const CUtensorMap &map_tlo, const K2PArgs &P, int warp, uint32_t rank,
-                                         int nk, int tiles_yp, int tiles_x, int ntiles, int ncl, int cid) {
+                                         int nk, int tiles_yp, int tiles_x, int ntiles, int ncl, int cid, const FuseCtx &F) {
   const bool leader = rank == 0;
   uint64_t *full = S.full, *empty = S.empty;
   uint64_t &acc_full = S.acc_full, &acc_empty = S.acc_empty;
@@ -178,9 +225,15 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
         const int zl = r / tiles_x;
         const int ty = typ * 2 + (int)rank;
         for (int c = 0; c < P.C; ++c) {
+          int unit = zl * P.C + c;
+          if (FUSED) {                                     // T^T of (plane, component) is complete in the ring scratch
+            unit = fuse_unit(F, P.C, zl, c).ring;
+            fuse_wait(F, F.ready + zl * P.C + c, 2 * F.a1);
+            fence_proxy_async_all();                       // the TMA reads below are ordered behind the acquire
+          }
           for (int a = 0; a < 2; ++a) {
             const int arow = a * P.m_pad + ty * 128;
-            const int chain0 = (zl * P.C + c) * 8 + 4 * a + 2 * (int)rank;
+            const int chain0 = unit * 8 + 4 * a + 2 * (int)rank;
             for (int kc = 0; kc < nk; ++kc) {
               mbar_wait(&empty[st], ph ^ 1);
               const uint32_t s = smem_u32(smem + st * P_STAGE);
@@ -212,6 +265,10 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
               umma2_commit(&empty[st]);
               if (++st == K2P_NST) { st = 0; ph ^= 1; }
             }
+          }
+          if (FUSED) {                                     // every T^T tile of (plane, component) has landed in the pair's shared memory
+            const int zl = (t / tiles_yp) / tiles_x;
+            red_release_gpu_add(F.consumed + zl * P.C + c, 1);
           }
           umma2_commit(&acc_full);
         }
@@ -311,7 +368,7 @@ __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint3
               const int mx = tx * 64 + col;
               if (mx < P.m) {
                 const int x = (qd & 1) ? P.M - 1 - mx : mx;
-                Ib[(size_t)y * P.M + x] = staging[row * K2P_PITCH + col];
+                __stcs(Ib + (size_t)y * P.M + x, staging[row * K2P_PITCH + col]);   // streaming: the output should not displace T^T in L2
               }
             }
           }
@@ -354,7 +411,7 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
   // register budget: launch = 640 x 96; the four feeder warps drop to 24 registers, the sixteen epilogue warps take 112 (128 x 24 + 512 x 112 <= 640 x 96)
   if (warp < 4) {
     setmaxnreg_dec<24>();
-    k2p_feed(smem, S, tmem, map_xhi, map_xlo, map_thi, map_tlo, P, warp, rank, nk, tiles_yp, tiles_x, ntiles, ncl, cid);
+    k2p_feed<false>(smem, S, tmem, map_xhi, map_xlo, map_thi, map_tlo, P, warp, rank, nk, tiles_yp, tiles_x, ntiles, ncl, cid, FuseCtx{});
   } else {
     setmaxnreg_inc<112>();
     k2p_epilogue<FIELD>(staging, S, tmem, P, warp, lane, rank, tiles_yp, tiles_x, ntiles, ncl, cid);
@@ -604,9 +661,9 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
 // The hi tile and the lo tile are separate buffers, each stored by its own bulk group, so writing one overlaps the
 // TMA read of the other.  GM = false: 64 q_y per row (128-byte rows, SWIZZLE_128B); GM = true: this CTA's own 128
 // accumulator columns only, 32 q_y per row (64-byte rows, SWIZZLE_64B: 16-byte chunk ^= (row >> 1) & 3).
-template <bool GM>
+template <bool GM, bool FUSED>
 __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32_t tmem, const CUtensorMap &map_this, const CUtensorMap &map_tlos,
-                                             const K1PArgs &P, const K1PGeom &G, int warp, int lane, uint32_t rank) {
+                                             const K1PArgs &P, const K1PGeom &G, int warp, int lane, uint32_t rank, const FuseCtx &F) {
   const int q = warp & 3;                       // TMEM lane quarter = 32 of this CTA's 128 mx rows
   const int row = q * 32 + lane;
   const int et = threadIdx.x - 32 * (K1P_FEED_WARPS + K1P_PRODUCER_WARPS);   // 0..127
@@ -622,13 +679,20 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
     for (int cg = 0; cg < G.nitems; ++cg, ++it) {
       const int g = it & 1;                                            // accumulator half
       const int grp = GM ? (int)rank : (cg & 1), c = GM ? cg : (cg >> 1);
+      int unit = T.zl * P.C + c;
+      if (FUSED) {
+        const FuseUnit fu = fuse_unit(F, P.C, T.zl, c);
+        unit = fu.ring;
+        // first item of a component: its ring slot must have been read by every stage-2 cluster of the unit before it
+        if (et == 0 && grp == 0 && fu.prev >= 0) fuse_wait(F, F.consumed + fu.prev, F.a2);
+      }
       mbar_wait(&S.acc_full[g], (it >> 1) & 1);
       tcgen05_fence_after();
 #pragma unroll 1
       for (int s = 0; s < (GM ? 2 : 4); ++s) {
         // GM false: round s = slot s (one chain), both q_y halves.  GM true: round s = slots 2 s and 2 s + 1 of this CTA's
         // group = two consecutive chains, stored by one TMA box of 2 chains (the staging tile holds them back to back).
-        const int chain = (T.zl * P.C + c) * 8 + (GM ? s * 4 + grp * 2 : (s >> 1) * 4 + grp * 2 + (s & 1));
+        const int chain = unit * 8 + (GM ? s * 4 + grp * 2 : (s >> 1) * 4 + grp * 2 + (s & 1));
         uint32_t pl[2][16];
         // the hi buffer was handed to the TMA store two bulk groups ago (hi, lo of the previous slot)
         if (et == 0) bulk_wait_read<1>();
@@ -672,6 +736,19 @@ __device__ __forceinline__ void k1p_epilogue(uint8_t *smem, K1PShared &S, uint32
           bulk_commit();
         }
       }
+      if (FUSED && et == 0 && cg >= 1) {
+        // an item issues 8 bulk groups (4 slots x hi, lo): everything older than the last 8 has completed, i.e. item cg - 1
+        bulk_wait_complete<8>();
+        if ((cg - 1) & 1) {                      // item cg - 1 was the second (last) item of component (cg - 1) / 2
+          fence_proxy_async_all();
+          red_release_gpu_add(F.ready + T.zl * P.C + ((cg - 1) >> 1), 1);
+        }
+      }
+    }
+    if (FUSED && et == 0) {                      // last component of the tile
+      bulk_wait_complete<0>();
+      fence_proxy_async_all();
+      red_release_gpu_add(F.ready + T.zl * P.C + (P.C - 1), 1);
     }
   }
   if (et == 0) bulk_wait_all();
@@ -722,7 +799,91 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
     k1p_produce<GM>(smem, S, P, G, lane, rank);
   } else {
     setmaxnreg_dec<104>();
-    k1p_epilogue<GM>(smem, S, tmem, map_this, map_tlos, P, G, warp, lane, rank);
+    k1p_epilogue<GM, false>(smem, S, tmem, map_this, map_tlos, P, G, warp, lane, rank, FuseCtx{});
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == 1) tmem_dealloc2(tmem, 512);
+}
+
+// Both stages in one launch: clusters [0, n1) run the stage-1 roles of k1_pair, the others the stage-2 roles of k2_pair,
+// coupled by the flags of FuseCtx.  640 threads as k2_pair; in a stage-1 cluster the fifth warpgroup gives its registers
+// back and idles.  Register budget after setmaxnreg (pool 640 x 96): stage 1 24 / 160 / 104 / 24, stage 2 24 / 112.
+constexpr int K12_SMEM = K1P_SMEM > K2P_SMEM ? K1P_SMEM : K2P_SMEM;
+
+template <bool FIELD>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(K2P_THREADS, 1)
+k12_fused(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUtensorMap map_xlo,
+          const __grid_constant__ CUtensorMap map_this, const __grid_constant__ CUtensorMap map_tlos,
+          const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo,
+          const K1PArgs P1, const K2PArgs P2, const FuseCtx F) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ K1PShared S1;
+  __shared__ K2PShared S2;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cluster = blockIdx.x >> 1, nclusters = gridDim.x >> 1;
+  const bool stage1 = cluster < F.n1;
+
+  if (threadIdx.x == 0) {
+    if (stage1) {
+      for (int i = 0; i < K1P_NST; ++i) { mbar_init(&S1.full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&S1.empty[i], 1); }
+      for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S1.bb_full[i], 1); mbar_init(&S1.bb_empty[i], K1P_PRODUCER_WARPS); }
+      for (int i = 0; i < 2; ++i) { mbar_init(&S1.acc_full[i], 1); mbar_init(&S1.acc_empty[i], 8); }
+    } else {
+      for (int i = 0; i < K2P_NST; ++i) { mbar_init(&S2.full[i], 1); mbar_init(&S2.empty[i], 1); }
+      mbar_init(&S2.acc_full, 1);
+      mbar_init(&S2.acc_empty, 2 * K2P_EPI_WARPS);
+    }
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&map_xhi); prefetch_tmap(&map_xlo);
+    if (stage1) { prefetch_tmap(&map_this); prefetch_tmap(&map_tlos); } else { prefetch_tmap(&map_thi); prefetch_tmap(&map_tlo); }
+  }
+  if (warp == 1) tmem_alloc2(stage1 ? &S1.tmem_slot : &S2.tmem_slot, 512);
+  tcgen05_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tcgen05_fence_after();
+  const uint32_t tmem = stage1 ? S1.tmem_slot : S2.tmem_slot;
+
+  if (stage1) {
+    K1PGeom G;
+    G.nk = P1.n_pad / 64;
+    G.tiles_j = P1.n_pad / K1P_QY;
+    G.tiles_m = P1.m_pad / 256;
+    G.ntiles = P1.zc * G.tiles_j * G.tiles_m;
+    G.nitems = 2 * P1.C;
+    G.ncl = F.n1;
+    G.cid = cluster;
+    if (warp < K1P_FEED_WARPS) {
+      setmaxnreg_dec<24>();
+      k1p_feed<false>(smem, S1, tmem, map_xhi, map_xlo, P1, G, warp, rank);
+    } else if (warp < K1P_FEED_WARPS + K1P_PRODUCER_WARPS) {
+      setmaxnreg_inc<160>();
+      k1p_produce<false>(smem, S1, P1, G, lane, rank);
+    } else if (warp < K1P_FEED_WARPS + K1P_PRODUCER_WARPS + 4) {
+      setmaxnreg_inc<104>();
+      k1p_epilogue<false, true>(smem, S1, tmem, map_this, map_tlos, P1, G, warp, lane, rank, F);
+    } else {
+      setmaxnreg_dec<24>();
+    }
+  } else {
+    float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
+    const int nk = P2.n_pad / 64;
+    const int tiles_yp = (P2.m_pad / 128 + 1) / 2, tiles_x = P2.m_pad / 64;
+    const int ntiles = P2.zc * tiles_yp * tiles_x;
+    const int ncl = nclusters - F.n1, cid = cluster - F.n1;
+    if (warp < 4) {
+      setmaxnreg_dec<24>();
+      k2p_feed<true>(smem, S2, tmem, map_xhi, map_xlo, map_thi, map_tlo, P2, warp, rank, nk, tiles_yp, tiles_x, ntiles, ncl, cid, F);
+    } else {
+      setmaxnreg_inc<112>();
+      k2p_epilogue<FIELD>(staging, S2, tmem, P2, warp, lane, rank, tiles_yp, tiles_x, ntiles, ncl, cid);
+    }
   }
   tcgen05_fence_before();
   __syncthreads();

@@ -541,3 +541,30 @@ def test_chirp_z_fft_path_configs_field_and_refusals(psf):
     I = plan.compute().cpu().numpy().astype(np.float64)
     assert plane_errors(I, O.stack_T2(other)).max() <= TOL
     plan.destroy()
+
+
+def test_fused_launch_matches_the_two_kernel_path_bit_for_bit(psf):
+    """k12_fused (both stages in one persistent kernel, T^T in an L2-resident ring, dependencies through global flags) runs
+    the same arithmetic in the same order as k1_pair + k2_pair: the stacks must be bit-identical, the field too, and the
+    stack must match the oracle.  Shapes: balanced stages with a1 != a2 tiles per plane, padded tiles, an odd plane count
+    that leaves plane groups of unequal length."""
+    import torch
+    for seed, N, M, Z, pol, field in ((75, 260, 300, 23, W.POL_CIRC_L, True), (76, 512, 512, 21, W.POL_UNPOLARIZED, False),
+                                     (77, 640, 512, 19, W.POL_X, False)):
+        case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, per_plane=False, shifts=False, pol=pol)
+        pf = psf.plan_from_case(case)
+        pu = psf.plan_from_case(case)
+        pu.tune(psf.TUNE_TC_FUSED, 0)
+        assert pf.kernel_names == ["k12_fused"] and pu.kernel_names == ["k1_pair", "k2_pair"], (pf.kernel_names, pu.kernel_names)
+        a = pf.compute(want_field=field)
+        b = pu.compute(want_field=field)
+        torch.cuda.synchronize()
+        if field:
+            assert torch.equal(a[1], b[1])
+            a, b = a[0], b[0]
+        assert torch.equal(a, b)
+        sel = [0, Z // 2, Z - 1]
+        assert plane_errors(a[sel].cpu().numpy().astype(np.float64), O.stack_T2(case, planes=sel)).max() <= TOL
+        pf.set_zernike(case.zernike, case.noll_first)        # the refresh path also checks the sticky abort word of the fused launch
+        pf.destroy()
+        pu.destroy()
