@@ -170,6 +170,7 @@ __device__ __forceinline__ FuseUnit fuse_unit(const FuseCtx &F, int C, int zl, i
   u.prev = ip < 0 ? -1 : (gi + (ip / C) * F.Pg) * C + ip % C;
   return u;
 }
+// (the abort word is in mapped host memory: polled every 4096 spins only)
 __device__ __forceinline__ int ld_acquire_gpu(const int *p) {
   int v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -184,8 +185,8 @@ __device__ __forceinline__ void fuse_wait(const FuseCtx &F, const int *flag, int
   while (ld_acquire_gpu(flag) < target) {
     __nanosleep(40);
     if ((++spins & 0xFFFu) == 0) {
-      if (ld_acquire_gpu(F.abort)) break;
-      if (spins > (1u << 24)) { atomicExch(F.abort, 1); break; }      // ~1 s: something is wrong; stop waiting everywhere
+      if (*(volatile int *)F.abort) break;
+      if (spins > (1u << 24)) { atomicExch_system(F.abort, 1); break; }   // ~1 s: something is wrong; stop waiting everywhere
     }
   }
 }
