@@ -180,8 +180,11 @@ int psf_grad_terms(const psf_plan *plan);
  *                            (the A/B setting of profiles/r2*_race_k1_pair.md; unsafe);
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
- *                            clusters, so that it stays in L2; 0 = always two kernels. */
-enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5 };
+ *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;
+ *   PSF_TUNE_SMLM          : 1 (default) = small grids in per-plane mode (emitter batches) run the emitter-batch kernel k_smlm where
+ *                            the plan qualifies; 0 = always k_small. */
+enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
+       PSF_TUNE_SMLM = 6 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

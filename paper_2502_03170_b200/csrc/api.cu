@@ -187,9 +187,13 @@ psf_status upload_static(psf_plan *p) {
     if ((s = upload(p, &p->d_coefq, &p->cap_coefq, coefq)) != PSF_OK) return s;
     P.zbq = (const float *)p->d_zbq;
     P.coefq = (const float *)p->d_coefq;
+    // the emitter-batch kernel for small grids (falls back to k_small when the plan does not qualify)
+    smlm_free(p);
+    if (p->tune_smlm && small_eligible(p) && d.precision != PSF_PREC_CZT_FFT && (s = smlm_setup(p, zbq)) != PSF_OK) return s;
   } else {
     P.K = 0;
     for (int i = 0; i < 4; ++i) P.zcnt[i] = 0;
+    smlm_free(p);
   }
   // plane table
   std::vector<float4> planes(d.n_planes);
@@ -269,6 +273,7 @@ void free_all(psf_plan *p) {
   if (p->done_ev) { cudaEventDestroy(p->done_ev); p->done_ev = nullptr; }
   tc_free(p);
   czt_free(p);
+  smlm_free(p);
   bessel_free(p);
   grad_free(p);
 }
@@ -413,6 +418,7 @@ psf_status psf_compute(psf_plan *p, void *cuda_stream, float *intensity, void *f
   const bool tc = p->path == 1 || p->path == 2;
   cudaError_t e = tc ? launch_tc(p, st, intensity, (float2 *)field)
                      : p->path == 4 ? launch_czt(p, st, intensity, (float2 *)field)
+                     : (p->path == 3 && p->smlm && !field) ? launch_smlm(p, st, intensity)
                      : p->path == 3 ? launch_small(p, st, intensity, (float2 *)field)
                                     : launch_ffma(p, st, intensity, (float2 *)field);
   mark_inflight(p, st);
@@ -501,6 +507,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_TC_FUSED) {
       if (value < 0 || value > 8) { p->err = "PSF_TUNE_TC_FUSED: 0 (off), 1 (on), 2..8 (on, ring depth forced)"; return PSF_ERR_INVALID_ARG; }
       p->tune_fused = (int)value;
+    } else if (knob == PSF_TUNE_SMLM) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_SMLM: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_smlm = (int)value;
     } else if (knob == PSF_TUNE_K1P_HANDOFF) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_handoff = (int)value;
@@ -580,7 +589,7 @@ long long psf_last_upload_bytes(const psf_plan *p) { return p ? p->upload_bytes 
 const char *psf_kernel_names(psf_plan *p) {
   if (!p) return "";
   try {
-    if (p->path == 3) p->kernel_names = "k_small";
+    if (p->path == 3) p->kernel_names = p->smlm ? "k_smlm" : "k_small";
     else if (p->path == 4) p->kernel_names = "czt_rows,czt_cols";
     else if ((p->path == 1 || p->path == 2) && p->tc) p->kernel_names = tc_kernel_names(p);
     else p->kernel_names = "k1_stage1,k2_stage2";

@@ -1,0 +1,421 @@
+// Emitter-batch kernel (k_smlm): the per-plane mode of the fused small-grid path, restructured for the SMLM regime of
+// BASELINE.json config 4 (thousands of independent single-plane PSFs, n = ceil(N/2) <= 32, m = ceil(M/2) <= 32, each emitter
+// with its own defocus, tilt and Zernike row).  Same arithmetic route as k_small (kernels_small.cu: phasors -> folded pupil Q ->
+// row DFT -> column DFT -> mirror butterfly -> |E|^2, all fp32 out of shared memory); what changes is where the time went
+// there (profiles/r2_ncu_cfg4.md: issue-bound at 4 warps per scheduler, every emitter re-reading 130 KB of tables from L2):
+//
+//   * persistent CTAs, one per SM, of LANES independent 128-thread "lanes", each working through its own emitters with its
+//     own named barrier: the FFMA-heavy and the latency-heavy phases of different emitters overlap on the same SM;
+//   * the static tables are staged in shared memory ONCE per CTA: folded Zernike basis, kappa, the cos / sin table and the
+//     base pupil - the latter not unfolded (98 KB) but split into its parity classes on the folded quadrant,
+//         P_c(s_x q_x, s_y q_y) = sum_ab sigma_ab(s_x, s_y) B_c,ab(q),   sigma_ee = 1, sigma_eo = s_x, sigma_oe = s_y, sigma_oo = s_x s_y,
+//     of which a pure polarisation component has ONE non-zero class (8 KB); with the parity transform of the phasor field,
+//         Phi_g(q) = sum_mirrors sigma_g exp(i phi(mirror)),   the folded pupil is   Q_c,g(q) = sum_ab B_c,ab(q) Phi_(g xor ab)(q):
+//     four complex multiplies per sample and class instead of four loads, four multiplies and the fold;
+//   * the two FFMA loops run on the packed fp32 FMA of sm_100 (fma.rn.f32x2: the re / im chains of a class are one register
+//     pair; the broadcast pairs (c, c), (s, s) of the table are built in registers - a table stored as broadcast pairs
+//     doubled the shared-memory wavefronts and made the kernel slower than k_small): 16 FFMA2 + 4..5 LDS.128 + 4..8 MOV per
+//     contraction index where k_small issues 32 FFMA + 4..6 loads.
+// Measured (profiles/r2_ncu_cfg4.md): config 4 0.374 -> 0.285 ms; 117 M warp instructions instead of 175 M, 49 M shared-memory
+// wavefronts; still issue-latency bound at three warps per scheduler (40 % issue activity).
+#include <algorithm>
+#include <cmath>
+#include <complex>
+
+#include "plan.hpp"
+#include "pupil_gen.cuh"
+
+namespace psf {
+
+struct SmlmState {
+  int ncls = 0, lanes = 0, K = 0;
+  int comp_start[6] = {0, 0, 0, 0, 0, 0};
+  int cls_ab[12] = {0};
+  void *d_bcls = nullptr;      // [ncls][32][32] float2, zero padded
+  void *d_xd = nullptr;        // [32][MQ] float2 = (cos, sin) of k s_max u_q x_m, zero padded
+  void *d_ktp = nullptr;       // [32][32] float2 kappa / 2 pi (hi, lo), zero padded
+  void *d_zbp = nullptr;       // [K][32][32] float folded basis / 2 pi, terms sorted by parity class, zero padded
+  int smem = 0, mq = 16;
+  long long version = -1;
+};
+
+namespace {
+
+constexpr int SL_THREADS = 128;
+constexpr int SL_NQ = 32;
+constexpr int SL_QROW = SL_NQ * 8 + 4;
+constexpr int SL_KMAX = 12;
+constexpr int SL_MAXCLS = 6;
+
+struct SmlmArgs {
+  const float2 *bcls;
+  const float2 *xd;
+  const float2 *ktp;
+  const float *zbp;
+  int ncls, K;
+  int comp_start[6];
+  int cls_ab[12];
+};
+
+__device__ __forceinline__ void sl_sincos_turns(float t, float &sn, float &cs) {
+  t -= rintf(t);
+  const float x = 6.283185307179586f * t;
+  sn = __sinf(x);
+  cs = __cosf(x);
+}
+__device__ __forceinline__ void sl_bar(int lane_id) { asm volatile("bar.sync %0, %1;" ::"r"(1 + lane_id), "r"(SL_THREADS) : "memory"); }
+__device__ __forceinline__ float2 cfma(float2 a, float2 b, float2 c) {   // c + a b
+  return make_float2(fmaf(a.x, b.x, fmaf(-a.y, b.y, c.x)), fmaf(a.x, b.y, fmaf(a.y, b.x, c.y)));
+}
+
+template <int MQ, int LANES>
+__global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, const SmlmArgs A, float *__restrict__ I) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  // layout: Xd [32][MQ] float2 | kt [32][32] float2 | bcls [ncls][32][32] float2 | zb [K][32][32] float | per lane: Qs, Ts
+  float2 *Xd = reinterpret_cast<float2 *>(smem_raw);
+  float2 *kts = reinterpret_cast<float2 *>(Xd + SL_NQ * MQ);
+  float2 *bcl = kts + SL_NQ * SL_NQ;
+  float *zbs = reinterpret_cast<float *>(bcl + (size_t)A.ncls * SL_NQ * SL_NQ);
+  constexpr int TS_ROW = 2 * MQ * 4 + 4;
+  float *lane_base = zbs + (size_t)A.K * SL_NQ * SL_NQ;
+  const int lane_id = threadIdx.x / SL_THREADS, lt = threadIdx.x % SL_THREADS;
+  float *Qs = lane_base + (size_t)lane_id * (SL_NQ * SL_QROW + SL_NQ * TS_ROW + 16);
+  float *Ts = Qs + SL_NQ * SL_QROW;
+  float *cfs = Ts + SL_NQ * TS_ROW;             // the emitter's coefficient row (16 floats)
+
+  // ---- stage the static tables (whole CTA) ----
+  for (int i = threadIdx.x; i < SL_NQ * MQ; i += blockDim.x) Xd[i] = __ldg(A.xd + i);
+  for (int i = threadIdx.x; i < SL_NQ * SL_NQ; i += blockDim.x) kts[i] = __ldg(A.ktp + i);
+  for (int i = threadIdx.x; i < A.ncls * SL_NQ * SL_NQ; i += blockDim.x) bcl[i] = __ldg(A.bcls + i);
+  for (int i = threadIdx.x; i < A.K * SL_NQ * SL_NQ; i += blockDim.x) zbs[i] = __ldg(A.zbp + i);
+  __syncthreads();
+
+  const int m = P.m, M = P.M, N = P.N, K = A.K;
+  constexpr int PASS1 = MQ / 16, PASS2 = (MQ / 2) * (MQ / 2) / 64;
+
+  for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
+    const float4 pl = __ldg(P.planes + b);
+    if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
+    sl_bar(lane_id);
+
+    // ---- phase 0: the parity transform Phi_g of the emitter's phasor field, 8 folded samples per thread, in registers ----
+    float2 phi[8][4];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      const int f = lt + SL_THREADS * r;
+      const int qy = f >> 5, qx = f & 31;
+      float pcl[4] = {kz_turns(kts[f], pl.x, pl.y), 0.f, 0.f, 0.f};     // phase parts: even/even, x-odd, y-odd, odd/odd (turns)
+      {
+        int j = 0;
+        for (int e = P.zcnt[0]; j < e; ++j) pcl[0] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[0]);
+        for (int e = j + P.zcnt[1]; j < e; ++j) pcl[1] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[1]);
+        for (int e = j + P.zcnt[2]; j < e; ++j) pcl[2] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[2]);
+        for (int e = j + P.zcnt[3]; j < e; ++j) pcl[3] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[3]);
+      }
+      if (P.has_shift) {
+        const float ux = (float)(2 * qx + 1 - N) / (float)N, uy = (float)(2 * qy + 1 - N) / (float)N;
+        pcl[1] = fmaf(-ux, pl.z, pcl[1]);
+        pcl[2] = fmaf(-uy, pl.w, pcl[2]);
+      }
+      float2 e[4];
+#pragma unroll
+      for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb) {
+          const float sx = bb ? -1.f : 1.f, sy = a ? -1.f : 1.f;
+          sl_sincos_turns(pcl[0] + sx * pcl[1] + sy * pcl[2] + sx * sy * pcl[3], e[a * 2 + bb].y, e[a * 2 + bb].x);
+        }
+      const float2 s01 = make_float2(e[0].x + e[1].x, e[0].y + e[1].y), d01 = make_float2(e[0].x - e[1].x, e[0].y - e[1].y);
+      const float2 s23 = make_float2(e[2].x + e[3].x, e[2].y + e[3].y), d23 = make_float2(e[2].x - e[3].x, e[2].y - e[3].y);
+      phi[r][0] = make_float2(s01.x + s23.x, s01.y + s23.y);      // sigma = 1
+      phi[r][1] = make_float2(d01.x + d23.x, d01.y + d23.y);      // sigma = s_x
+      phi[r][2] = make_float2(s01.x - s23.x, s01.y - s23.y);      // sigma = s_y
+      phi[r][3] = make_float2(d01.x - d23.x, d01.y - d23.y);      // sigma = s_x s_y
+    }
+
+    float inten[PASS2][2][4];
+#pragma unroll
+    for (int p = 0; p < PASS2; ++p)
+#pragma unroll
+      for (int ix = 0; ix < 2; ++ix)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) inten[p][ix][q] = 0.f;
+
+    for (int c = 0; c < P.C; ++c) {
+      sl_bar(lane_id);                                   // Qs / Ts of the previous component (or emitter) are free
+      // ---- Q_g = sum_ab B_ab Phi_(g xor ab) ----
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int f = lt + SL_THREADS * r;
+        float2 o[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        for (int ci = A.comp_start[c]; ci < A.comp_start[c + 1]; ++ci) {
+          const float2 bv = bcl[ci * (SL_NQ * SL_NQ) + f];
+          switch (A.cls_ab[ci]) {                        // static register indices in every branch
+            case 0: o[0] = cfma(bv, phi[r][0], o[0]); o[1] = cfma(bv, phi[r][1], o[1]); o[2] = cfma(bv, phi[r][2], o[2]); o[3] = cfma(bv, phi[r][3], o[3]); break;
+            case 1: o[0] = cfma(bv, phi[r][1], o[0]); o[1] = cfma(bv, phi[r][0], o[1]); o[2] = cfma(bv, phi[r][3], o[2]); o[3] = cfma(bv, phi[r][2], o[3]); break;
+            case 2: o[0] = cfma(bv, phi[r][2], o[0]); o[1] = cfma(bv, phi[r][3], o[1]); o[2] = cfma(bv, phi[r][0], o[2]); o[3] = cfma(bv, phi[r][1], o[3]); break;
+            default: o[0] = cfma(bv, phi[r][3], o[0]); o[1] = cfma(bv, phi[r][2], o[1]); o[2] = cfma(bv, phi[r][1], o[2]); o[3] = cfma(bv, phi[r][0], o[3]); break;
+          }
+        }
+        float4 *dst = reinterpret_cast<float4 *>(&Qs[(f >> 5) * SL_QROW + (f & 31) * 8]);
+        const float4 v0 = make_float4(o[0].x, o[0].y, o[1].x, o[1].y);     // ee, eo
+        const float4 v1 = make_float4(o[2].x, o[2].y, o[3].x, o[3].y);     // oe, oo
+        const int hsw = lt & 1;                          // odd lanes store their second half first: no two-way bank conflict
+        dst[hsw] = hsw ? v1 : v0;
+        dst[hsw ^ 1] = hsw ? v0 : v1;
+      }
+      sl_bar(lane_id);
+
+      // ---- stage 1: rows.  thread = (qy, group of 4 mx); a register pair = (re, im) of one class ----
+      {
+        const int qy = lt >> 2;
+#pragma unroll
+        for (int p = 0; p < PASS1; ++p) {
+          const int mx0 = ((lt & 3) + 4 * p) * 4;
+          float2 acc[4][4];                              // [class][mx]
+#pragma unroll
+          for (int g = 0; g < 4; ++g)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[g][i] = make_float2(0.f, 0.f);
+#pragma unroll 8
+          for (int k = 0; k < SL_NQ; ++k) {
+            const float4 q0 = *reinterpret_cast<const float4 *>(&Qs[qy * SL_QROW + k * 8]);
+            const float4 q1 = *reinterpret_cast<const float4 *>(&Qs[qy * SL_QROW + k * 8 + 4]);
+            const float4 x01 = *reinterpret_cast<const float4 *>(&Xd[k * MQ + mx0]);       // (c, s) of mx0, mx0 + 1
+            const float4 x23 = *reinterpret_cast<const float4 *>(&Xd[k * MQ + mx0 + 2]);
+            const float cc[4] = {x01.x, x01.z, x23.x, x23.z}, ss[4] = {x01.y, x01.w, x23.y, x23.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float2 xc = make_float2(cc[i], cc[i]), xs = make_float2(ss[i], ss[i]);   // broadcast pairs built in registers
+              acc[0][i] = __ffma2_rn(make_float2(q0.x, q0.y), xc, acc[0][i]);   // ee: even in x -> cos
+              acc[1][i] = __ffma2_rn(make_float2(q0.z, q0.w), xs, acc[1][i]);   // eo: odd in x -> sin
+              acc[2][i] = __ffma2_rn(make_float2(q1.x, q1.y), xc, acc[2][i]);   // oe
+              acc[3][i] = __ffma2_rn(make_float2(q1.z, q1.w), xs, acc[3][i]);   // oo
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            *reinterpret_cast<float4 *>(&Ts[qy * TS_ROW + (mx0 + i) * 4]) = make_float4(acc[0][i].x, acc[0][i].y, acc[1][i].x, acc[1][i].y);
+            *reinterpret_cast<float4 *>(&Ts[qy * TS_ROW + MQ * 4 + (mx0 + i) * 4]) = make_float4(acc[2][i].x, acc[2][i].y, acc[3][i].x, acc[3][i].y);
+          }
+        }
+      }
+      sl_bar(lane_id);
+
+      // ---- stage 2: columns.  lane pair = one 2 x 2 pixel tile, each lane sums every other q_y ----
+      const float w = P.weight[c];
+      const int kh = lt & 1;
+#pragma unroll
+      for (int p = 0; p < PASS2; ++p) {
+        const int tile = (lt >> 1) + 64 * p;
+        const int my0 = (tile / (MQ / 2)) * 2, mx0 = (tile % (MQ / 2)) * 2;
+        float2 acc[4][2][2];                             // [class][iy][ix]
+#pragma unroll
+        for (int g = 0; g < 4; ++g) acc[g][0][0] = acc[g][0][1] = acc[g][1][0] = acc[g][1][1] = make_float2(0.f, 0.f);
+#pragma unroll 4
+        for (int kk = 0; kk < SL_NQ / 2; ++kk) {
+          const int qy = 2 * kk + kh;
+          const float4 y01 = *reinterpret_cast<const float4 *>(&Xd[qy * MQ + my0]);              // (c, s) of my0, my0 + 1
+          const float4 t00 = *reinterpret_cast<const float4 *>(&Ts[qy * TS_ROW + mx0 * 4]);            // ee, eo at mx0
+          const float4 t01 = *reinterpret_cast<const float4 *>(&Ts[qy * TS_ROW + mx0 * 4 + 4]);        // ee, eo at mx0 + 1
+          const float4 t10 = *reinterpret_cast<const float4 *>(&Ts[qy * TS_ROW + MQ * 4 + mx0 * 4]);   // oe, oo
+          const float4 t11 = *reinterpret_cast<const float4 *>(&Ts[qy * TS_ROW + MQ * 4 + mx0 * 4 + 4]);
+          const float2 yc[2] = {make_float2(y01.x, y01.x), make_float2(y01.z, y01.z)};
+          const float2 ys[2] = {make_float2(y01.y, y01.y), make_float2(y01.w, y01.w)};
+#pragma unroll
+          for (int iy = 0; iy < 2; ++iy) {
+            acc[0][iy][0] = __ffma2_rn(make_float2(t00.x, t00.y), yc[iy], acc[0][iy][0]);   // ee, eo: even in y -> cos
+            acc[0][iy][1] = __ffma2_rn(make_float2(t01.x, t01.y), yc[iy], acc[0][iy][1]);
+            acc[1][iy][0] = __ffma2_rn(make_float2(t00.z, t00.w), yc[iy], acc[1][iy][0]);
+            acc[1][iy][1] = __ffma2_rn(make_float2(t01.z, t01.w), yc[iy], acc[1][iy][1]);
+            acc[2][iy][0] = __ffma2_rn(make_float2(t10.x, t10.y), ys[iy], acc[2][iy][0]);   // oe, oo: odd in y -> sin
+            acc[2][iy][1] = __ffma2_rn(make_float2(t11.x, t11.y), ys[iy], acc[2][iy][1]);
+            acc[3][iy][0] = __ffma2_rn(make_float2(t10.z, t10.w), ys[iy], acc[3][iy][0]);
+            acc[3][iy][1] = __ffma2_rn(make_float2(t11.z, t11.w), ys[iy], acc[3][iy][1]);
+          }
+        }
+        // combine the two halves of the contraction; lane kh then finishes pixel row my0 + kh
+        float2 a[4][2];
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+#pragma unroll
+          for (int ix = 0; ix < 2; ++ix) {
+            float2 r0, r1;
+            r0.x = acc[g][0][ix].x + __shfl_xor_sync(0xffffffffu, acc[g][0][ix].x, 1);
+            r0.y = acc[g][0][ix].y + __shfl_xor_sync(0xffffffffu, acc[g][0][ix].y, 1);
+            r1.x = acc[g][1][ix].x + __shfl_xor_sync(0xffffffffu, acc[g][1][ix].x, 1);
+            r1.y = acc[g][1][ix].y + __shfl_xor_sync(0xffffffffu, acc[g][1][ix].y, 1);
+            a[g][ix] = kh ? r1 : r0;
+          }
+#pragma unroll
+        for (int ix = 0; ix < 2; ++ix) {
+          const float a0 = a[0][ix].x, a1 = a[0][ix].y, a2 = a[1][ix].x, a3 = a[1][ix].y;
+          const float a4 = a[2][ix].x, a5 = a[2][ix].y, a6 = a[3][ix].x, a7 = a[3][ix].y;
+          // E(sy, sx) = F_ee + i sx F_eo + i sy F_oe - sx sy F_oo
+          const float re0 = a0 - a3 - a5 - a6, im0 = a1 + a2 + a4 - a7;   // (+y, +x)
+          const float re1 = a0 + a3 - a5 + a6, im1 = a1 - a2 + a4 + a7;   // (+y, -x)
+          const float re2 = a0 - a3 + a5 + a6, im2 = a1 + a2 - a4 + a7;   // (-y, +x)
+          const float re3 = a0 + a3 + a5 - a6, im3 = a1 - a2 - a4 - a7;   // (-y, -x)
+          inten[p][ix][0] = fmaf(w, re0 * re0 + im0 * im0, inten[p][ix][0]);
+          inten[p][ix][1] = fmaf(w, re1 * re1 + im1 * im1, inten[p][ix][1]);
+          inten[p][ix][2] = fmaf(w, re2 * re2 + im2 * im2, inten[p][ix][2]);
+          inten[p][ix][3] = fmaf(w, re3 * re3 + im3 * im3, inten[p][ix][3]);
+        }
+      }
+    }
+
+    float *Ib = I + (size_t)b * M * M;
+#pragma unroll
+    for (int p = 0; p < PASS2; ++p) {
+      const int tile = (lt >> 1) + 64 * p;
+      const int my = (tile / (MQ / 2)) * 2 + (lt & 1), mx0 = (tile % (MQ / 2)) * 2;
+      if (my < m) {
+        const int myr = M - 1 - my;
+        // the two pixels of the thread are adjacent: 8-byte stores (M even: every pair is aligned in all four quadrants)
+        if (mx0 + 1 < m) {
+          *reinterpret_cast<float2 *>(Ib + (size_t)my * M + mx0) = make_float2(inten[p][0][0], inten[p][1][0]);
+          *reinterpret_cast<float2 *>(Ib + (size_t)my * M + (M - 2 - mx0)) = make_float2(inten[p][1][1], inten[p][0][1]);
+          *reinterpret_cast<float2 *>(Ib + (size_t)myr * M + mx0) = make_float2(inten[p][0][2], inten[p][1][2]);
+          *reinterpret_cast<float2 *>(Ib + (size_t)myr * M + (M - 2 - mx0)) = make_float2(inten[p][1][3], inten[p][0][3]);
+        } else if (mx0 < m) {
+          Ib[(size_t)my * M + mx0] = inten[p][0][0];
+          Ib[(size_t)my * M + (M - 1 - mx0)] = inten[p][0][1];
+          Ib[(size_t)myr * M + mx0] = inten[p][0][2];
+          Ib[(size_t)myr * M + (M - 1 - mx0)] = inten[p][0][3];
+        }
+      }
+    }
+  }
+}
+
+template <int MQ, int LANES>
+cudaError_t sl_launch(const psf_plan *p, const SmlmState *t, const SmlmArgs &A, cudaStream_t st, float *intensity) {
+  const int per = (p->dp.Z + LANES - 1) / LANES;
+  const int grid = per < p->sm_count ? per : p->sm_count;
+  k_smlm<MQ, LANES><<<grid, SL_THREADS * LANES, t->smem, st>>>(p->dp, A, intensity);
+  return cudaGetLastError();
+}
+
+template <typename T>
+bool sl_up(void **d, const std::vector<T> &h, long long *acc) {
+  if (*d) { cudaFree(*d); *d = nullptr; }
+  if (h.empty()) return true;
+  if (cudaMalloc(d, h.size() * sizeof(T)) != cudaSuccess) return false;
+  if (cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+  if (acc) *acc += (long long)(h.size() * sizeof(T));
+  return true;
+}
+
+}  // namespace
+
+void smlm_free(psf_plan *p) {
+  SmlmState *t = p->smlm;
+  if (!t) return;
+  void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp};
+  for (void *b : bufs)
+    if (b) cudaFree(b);
+  delete t;
+  p->smlm = nullptr;
+}
+
+// Builds the emitter-batch tables if the plan qualifies: per-plane mode, even N (no self-mirror row / column), n <= 32,
+// m <= 32 (M even), at most SL_KMAX per-plane Zernike terms, and few enough non-zero parity classes of the base pupil for at
+// least two lanes to fit in shared memory.  Returns PSF_OK with p->smlm == nullptr when it does not (k_small runs then).
+psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted) {
+  smlm_free(p);
+  const DevPlan &D = p->dp;
+  const int N = D.N, n = D.n, m = D.m, C = D.C, K = p->K_rows;
+  if (!D.per_plane || (N & 1) || (D.M & 1) || n > SL_NQ || m > 32 || K > SL_KMAX) return PSF_OK;
+  const size_t NN = (size_t)N * N;
+  // parity classes of the base pupil on the folded quadrant
+  std::vector<float2> bcls;
+  SmlmState *t = new SmlmState();
+  double bmax = 0.0;
+  for (size_t i = 0; i < (size_t)C * NN; ++i) bmax = std::max(bmax, std::abs(p->h_base[i]));
+  int ncls = 0;
+  for (int c = 0; c < C; ++c) {
+    t->comp_start[c] = ncls;
+    const cplx *B = p->h_base.data() + (size_t)c * NN;
+    for (int ab = 0; ab < 4; ++ab) {
+      std::vector<float2> cls((size_t)SL_NQ * SL_NQ, make_float2(0.f, 0.f));
+      double cmax = 0.0;
+      for (int qy = 0; qy < n; ++qy)
+        for (int qx = 0; qx < n; ++qx) {
+          const int ry = N - 1 - qy, rx = N - 1 - qx;
+          const cplx p00 = B[(size_t)qy * N + qx], p01 = B[(size_t)qy * N + rx], p10 = B[(size_t)ry * N + qx], p11 = B[(size_t)ry * N + rx];
+          const double sx = (ab & 1) ? -1.0 : 1.0, sy = (ab & 2) ? -1.0 : 1.0;     // sigma_ab at the mirrored index
+          const cplx v = 0.25 * (p00 + sx * p01 + sy * p10 + sx * sy * p11);
+          cmax = std::max(cmax, std::abs(v));
+          cls[(size_t)qy * SL_NQ + qx] = make_float2((float)v.real(), (float)v.imag());
+        }
+      if (cmax > 1e-9 * bmax) {
+        if (ncls >= 12) { delete t; return PSF_OK; }
+        t->cls_ab[ncls++] = ab;
+        bcls.insert(bcls.end(), cls.begin(), cls.end());
+      }
+    }
+  }
+  for (int c = C; c < 6; ++c) t->comp_start[c] = ncls;
+  t->ncls = ncls;
+  t->K = K;
+  t->mq = m <= 16 ? 16 : 32;
+  const size_t fixed = (size_t)SL_NQ * t->mq * 8 + (size_t)SL_NQ * SL_NQ * 8 + (size_t)ncls * SL_NQ * SL_NQ * 8 + (size_t)K * SL_NQ * SL_NQ * 4;
+  const size_t lane = ((size_t)SL_NQ * SL_QROW + (size_t)SL_NQ * (2 * t->mq * 4 + 4) + 16) * 4;
+  const size_t limit = 227 * 1024 - 256;
+  t->lanes = (fixed + 3 * lane <= limit) ? 3 : (fixed + 2 * lane <= limit) ? 2 : 0;
+  if (t->lanes == 0 || ncls > SL_MAXCLS * 2) { delete t; return PSF_OK; }
+  t->smem = (int)(fixed + t->lanes * lane);
+  // tables, zero padded to 32 (x MQ)
+  const int mq = t->mq;
+  std::vector<float2> xd((size_t)SL_NQ * mq, make_float2(0.f, 0.f));
+  for (int mi = 0; mi < m; ++mi)
+    for (int q = 0; q < n; ++q) {
+      const double ph = p->phi[(size_t)mi * n + q];
+      const float cs = (float)std::cos(ph), sn = (float)std::sin(ph);
+      xd[(size_t)q * mq + mi] = make_float2(cs, sn);
+    }
+  std::vector<float2> ktp((size_t)SL_NQ * SL_NQ, make_float2(0.f, 0.f));
+  for (int qy = 0; qy < n; ++qy)
+    for (int qx = 0; qx < n; ++qx) ktp[(size_t)qy * SL_NQ + qx] = p->h_kt[(size_t)qy * n + qx];
+  std::vector<float> zbp((size_t)K * SL_NQ * SL_NQ, 0.f);
+  for (int k = 0; k < K; ++k)
+    for (int qy = 0; qy < n; ++qy)
+      for (int qx = 0; qx < n; ++qx) zbp[((size_t)k * SL_NQ + qy) * SL_NQ + qx] = zbq_sorted[(size_t)k * n * n + (size_t)qy * n + qx];
+  auto fail = [&](const char *msg) { p->err = msg; delete t; return PSF_ERR_ALLOC; };
+  p->smlm = t;
+  if (!sl_up(&t->d_bcls, bcls, &p->upload_bytes) || !sl_up(&t->d_xd, xd, &p->upload_bytes) || !sl_up(&t->d_ktp, ktp, &p->upload_bytes) ||
+      !sl_up(&t->d_zbp, zbp, &p->upload_bytes)) {
+    p->smlm = nullptr;
+    void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp};
+    for (void *b : bufs)
+      if (b) cudaFree(b);
+    return fail("smlm: table upload failed");
+  }
+  cudaError_t e = cudaSuccess;
+  if (mq == 16) {
+    e = t->lanes == 3 ? cudaFuncSetAttribute(k_smlm<16, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem)
+                      : cudaFuncSetAttribute(k_smlm<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem);
+  } else {
+    e = t->lanes == 3 ? cudaFuncSetAttribute(k_smlm<32, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem)
+                      : cudaFuncSetAttribute(k_smlm<32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem);
+  }
+  if (e != cudaSuccess) { p->err = std::string("smlm: cudaFuncSetAttribute: ") + cudaGetErrorString(e); smlm_free(p); return PSF_ERR_CUDA; }
+  t->version = p->table_version;
+  return PSF_OK;
+}
+
+cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity) {
+  const SmlmState *t = p->smlm;
+  SmlmArgs A;
+  A.bcls = (const float2 *)t->d_bcls; A.xd = (const float2 *)t->d_xd; A.ktp = (const float2 *)t->d_ktp; A.zbp = (const float *)t->d_zbp;
+  A.ncls = t->ncls; A.K = t->K;
+  for (int i = 0; i < 6; ++i) A.comp_start[i] = t->comp_start[i];
+  for (int i = 0; i < 12; ++i) A.cls_ab[i] = t->cls_ab[i];
+  cudaError_t e;
+  if (t->mq == 16) e = t->lanes == 3 ? sl_launch<16, 3>(p, t, A, st, intensity) : sl_launch<16, 2>(p, t, A, st, intensity);
+  else e = t->lanes == 3 ? sl_launch<32, 3>(p, t, A, st, intensity) : sl_launch<32, 2>(p, t, A, st, intensity);
+  prof_mark(p, st, 0);
+  return e;
+}
+
+}  // namespace psf

@@ -40,6 +40,7 @@ struct TcState;      // tcgen05 path (kernels_tc.cu)
 struct BesselState;  // spherical parametrisation (kernels_bessel.cu)
 struct GradState;    // adjoint / gradients (kernels_grad.cu)
 struct CztState;     // chirp-Z by FFT (kernels_czt.cu)
+struct SmlmState;    // emitter-batch kernel (kernels_smlm.cu)
 
 }  // namespace psf
 
@@ -84,6 +85,8 @@ struct psf_plan {
   psf::BesselState *bessel = nullptr;
   psf::GradState *grad = nullptr;
   psf::CztState *czt = nullptr;
+  psf::SmlmState *smlm = nullptr;
+  int tune_smlm = 1;             // 1: the emitter-batch kernel k_smlm where it qualifies; 0: always k_small
   // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
   int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
   int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
@@ -131,6 +134,10 @@ cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity, floa
 psf_status bessel_setup(psf_plan *p, int n_nodes);
 void bessel_free(psf_plan *p);
 cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
+// kernels_smlm.cu
+psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted);
+void smlm_free(psf_plan *p);
+cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity);
 // kernels_czt.cu
 bool czt_supported(const psf_plan *p, std::string &why);
 psf_status czt_setup(psf_plan *p);

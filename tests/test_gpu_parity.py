@@ -568,3 +568,35 @@ def test_fused_launch_matches_the_two_kernel_path_bit_for_bit(psf):
         pf.set_zernike(case.zernike, case.noll_first)        # the refresh path also checks the sticky abort word of the fused launch
         pf.destroy()
         pu.destroy()
+
+
+@pytest.mark.parametrize("seed,N,M,Z,pol,kw", [
+    (401, 64, 32, 40, W.POL_X, {}),                                   # config 4's shape: one parity class per component, three lanes
+    (402, 64, 64, 9, W.POL_JONES, {}),                                # m = 32: the wide instantiation; two classes per component
+    (403, 50, 30, 7, W.POL_CIRC_L, {}),                               # n = 25, m = 15 (odd half-size: the last pixel pair is a single pixel)
+    (404, 12, 8, 5, W.POL_Y, {}),
+    (405, 64, 32, 11, W.POL_UNPOLARIZED, {}),                         # five pupils
+    (406, 40, 28, 6, W.POL_X, {"model": "scalar"}),
+    (407, 64, 32, 6, W.POL_X, {"fresnel": True, "envelope_s": 0.7}),
+])
+def test_emitter_batch_kernel(psf, seed, N, M, Z, pol, kw):
+    """k_smlm (kernels_smlm.cu): per-plane Zernike rows + shifts on small even grids, against the fp64 oracle, and bit-level
+    agreement is not expected with k_small (different association), so both are checked against the oracle."""
+    import torch
+    case = replace(W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, pol=pol), **kw)
+    ref = O.stack_T2(case)
+    plan = psf.plan_from_case(case)
+    assert plan.kernel_names == ["k_smlm"], plan.kernel_names
+    I = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(I, ref).max() <= TOL, plane_errors(I, ref)
+    plan.tune(psf.TUNE_SMLM, 0)
+    assert plan.kernel_names == ["k_small"]
+    I0 = plan.compute().cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
+    assert plane_errors(I0, ref).max() <= TOL
+    plan.destroy()
+    # shifts only (no Zernike rows), and rows only
+    for drop in ("zernike", "shifts_um"):
+        c2 = replace(case, **{drop: None})
+        I2, _ = gpu_stack(psf, c2)
+        assert plane_errors(I2, O.stack_T2(c2)).max() <= TOL, drop
