@@ -488,7 +488,7 @@ def run_ours(args):
                 cg = 6 if cs.pol == "unpolarized" else 3
                 flop = 2 * 8.0 * cs.pupil_n * cs.out_m * (cs.pupil_n + cs.out_m) * cg * cs.n_planes     # forward + back-projection
                 ffma_peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-                sweep[name] = {"ms_per_step": ms, "planes_per_s": cs.n_planes / (ms * 1e-3), "path": "adjoint_ffma",
+                sweep[name] = {"ms_per_step": ms, "planes_per_s": cs.n_planes / (ms * 1e-3), "path": plan.grad_path,
                                "tflops": flop / (ms * 1e-3) / 1e12, "frac_of_ffma_peak": flop / (ms * 1e-3) / 1e12 / ffma_peak,
                                "zernike_terms": int(K)}
                 plan.destroy()

@@ -160,10 +160,17 @@ psf_status psf_compute_spherical(psf_plan *plan, void *cuda_stream, float *inten
  *           the contribution of plane b: for shared coefficients the gradient is the column sum over the planes.
  * dL_dI is device fp32 [n_planes][M][M].  All polarisations incl. PSF_POL_UNPOLARIZED, both models, every correction
  * factor.  The first call (and the first call after any psf_set_*) builds device copies of the unfolded tables and
- * allocates scratch, so it may allocate and synchronise; later calls only enqueue on `cuda_stream`. */
+ * allocates scratch, so it may allocate and synchronise; later calls only enqueue on `cuda_stream`.
+ * On a plan that runs on the tensor cores (3xFP16, static mode) both transforms of the adjoint run there too: the field
+ * from the forward kernels, then the back-projection as the same zoomed transform with the two grids swapped (a second,
+ * internal plan), scratch 8 bytes x (C Z M^2 + C Z N^2) + 32 bytes x C Z ceil(M/2)^2 (padded). */
 psf_status psf_gradients(psf_plan *plan, void *cuda_stream, const float *dL_dI, double *dL_dz, double *dL_dc);
 
 psf_status psf_plan_destroy(psf_plan *plan);
+
+/* Route the last psf_gradients of this plan took: "adjoint_tc3xf16" (both transforms on the tensor cores: static mode on the
+ * 3xFP16 path), "adjoint_ffma" (fp32 FFMA products: every other case), "" before the first call (static string). */
+const char *psf_grad_path_name(const psf_plan *plan);
 
 /* Number of Zernike terms currently set (shared or per plane) = the row length K of psf_gradients' dL_dc. */
 int psf_grad_terms(const psf_plan *plan);
@@ -182,9 +189,11 @@ int psf_grad_terms(const psf_plan *plan);
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
  *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;
  *   PSF_TUNE_SMLM          : 1 (default) = small grids in per-plane mode (emitter batches) run the emitter-batch kernel k_smlm where
- *                            the plan qualifies; 0 = always k_small. */
+ *                            the plan qualifies; 0 = always k_small;
+ *   PSF_TUNE_GRAD_TENSOR   : 1 (default) = psf_gradients runs its two transforms on the tensor cores where the plan is on the 3xFP16
+ *                            path in static mode; 0 = the fp32 FFMA route of round 1. */
 enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
-       PSF_TUNE_SMLM = 6 };
+       PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

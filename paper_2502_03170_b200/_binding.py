@@ -21,8 +21,8 @@ PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3, "czt_fft": 4}
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
-           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names"]
-TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER, TUNE_TC_FUSED, TUNE_SMLM = 1, 2, 3, 4, 5, 6
+           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names", "psf_grad_path_name"]
+TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER, TUNE_TC_FUSED, TUNE_SMLM, TUNE_GRAD_TENSOR = 1, 2, 3, 4, 5, 6, 7
 
 
 class PsfError(RuntimeError):
@@ -95,6 +95,8 @@ def load_library(build_if_missing: bool = True):
     lib.psf_plan_tune.restype = C.c_int
     lib.psf_kernel_names.argtypes = [P]
     lib.psf_kernel_names.restype = C.c_char_p
+    lib.psf_grad_path_name.argtypes = [P]
+    lib.psf_grad_path_name.restype = C.c_char_p
     lib.psf_grad_terms.argtypes = [P]
     lib.psf_grad_terms.restype = C.c_int
     lib.psf_host_tables.argtypes = [C.POINTER(psf_plan_desc), C.POINTER(C.c_float), C.c_int, C.c_int,
@@ -265,6 +267,10 @@ class PsfPlan:
     @property
     def launches_per_compute(self) -> int:
         return int(self._lib.psf_launches_per_compute(self._h))
+
+    @property
+    def grad_path(self) -> str:
+        return self._lib.psf_grad_path_name(self._h).decode()
 
     @property
     def kernel_names(self) -> list:

@@ -280,6 +280,17 @@ void free_all(psf_plan *p) {
 
 }  // namespace
 
+namespace psf {
+psf_status plan_set_materialised(psf_plan *p, double qmax, double rmax) {
+  p->mat_mode = 1;
+  p->mat_qmax = qmax;
+  p->mat_rmax = rmax;
+  if (cudaSetDevice(p->device) != cudaSuccess) { p->err = "cudaSetDevice failed"; return PSF_ERR_CUDA; }
+  tc_free(p);
+  return refresh(p);
+}
+}  // namespace psf
+
 extern "C" {
 
 psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
@@ -507,6 +518,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_TC_FUSED) {
       if (value < 0 || value > 8) { p->err = "PSF_TUNE_TC_FUSED: 0 (off), 1 (on), 2..8 (on, ring depth forced)"; return PSF_ERR_INVALID_ARG; }
       p->tune_fused = (int)value;
+    } else if (knob == PSF_TUNE_GRAD_TENSOR) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_GRAD_TENSOR: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_grad_tensor = (int)value;
     } else if (knob == PSF_TUNE_SMLM) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_SMLM: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_smlm = (int)value;
@@ -527,6 +541,8 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     return refresh(p);
   });
 }
+
+const char *psf_grad_path_name(const psf_plan *p) { return p ? grad_route(p) : ""; }
 
 int psf_grad_terms(const psf_plan *p) {
   if (!p) return 0;

@@ -6,10 +6,20 @@
 //     B_c[p]      = sum_x w_c G(x) conj(E_c(x)) A(x, p)          back-projection: the same two products, transposed
 //     dL/dphi[p]  = -2 sum_c Im(Q_c[p] B_c[p])                   pupil-side sensitivity
 //     dL/dz_b     = sum_p k cos(theta_p) dL/dphi[p],    dL/dc_bj = sum_p Z_j[p] dL/dphi[p].
-// First correct version: unfolded complex fp32 FFMA products (one generic batched kernel C = A B^T used four times), own
-// forward pass (the optimised kernels keep neither the unfolded pupil nor the fields of unpolarised light).  The tensor
-// path is the next step; this file is the correctness vehicle and the API.
+// Two routes:
+//   * FFMA (round 1, the correctness vehicle; every mode): unfolded complex fp32 products (one generic batched kernel
+//     C = A B^T used four times) with an own forward pass;
+//   * tensor cores (static mode on the 3xFP16 path): the back-projection B_c = A_y^T H_c A_x, H_c = w_c G conj(E_c), is the
+//     forward zoomed transform with the roles of the two grids swapped (pupil grid := the M x M image grid, output grid := the
+//     N x N pupil grid, pixel' = pixel M / N: k s_max u_p x_m is symmetric in the two).  So: E_c from the plan's own tensor
+//     kernels (field epilogue), one kernel that weights with G / max|G| and folds H_c into the four parity classes in the
+//     stage-1 producers' table order, the SAME tensor kernels on a second plan ("plan B") whose stage 1 reads that
+//     per-plane folded pupil instead of generating one (materialised-pupil mode, launch_tc_mat), and a reduction of
+//     Im(Q B) against kappa and the Zernike basis with Q regenerated on the fly.  Neither Q nor T is written to HBM; E, the
+//     folded H and B are (8 B per sample each).
+#include <algorithm>
 #include <cmath>
+#include <complex>
 #include <vector>
 
 #include "plan.hpp"
@@ -29,6 +39,17 @@ struct GradState {
   void *d_axt = nullptr;      // float2 [N][M]      its transpose
   void *d_Q = nullptr, *d_T = nullptr, *d_E = nullptr, *d_B = nullptr;   // per-pass scratch
   long long version = -1;     // table version these copies were made from
+  // tensor-core route
+  bool tensor = false;
+  psf_plan *planB = nullptr;  // the back-projection plan (sizes swapped), owned
+  int C5 = 0;                 // scalar pupils of the forward tensor path (1, 3, or 5 for unpolarised light)
+  float w5[5] = {0, 0, 0, 0, 0};
+  void *d_base5 = nullptr;    // float2 [C5][N][N]
+  void *d_fieldE = nullptr;   // float2 [C5][Z][M][M]
+  void *d_fieldB = nullptr;   // float2 [C5][Z][N][N]
+  void *d_hfold = nullptr;    // float4 [Z][2][C5][npB][npB], the pair producers' order, times plan B's operand scale
+  void *d_dummyI = nullptr;   // float  [Z][max(M, N)^2]
+  void *d_gmax = nullptr;     // one float (bit pattern of max |G|)
 };
 
 namespace {
@@ -153,11 +174,111 @@ g_reduce(const float2 *__restrict__ Q, const float2 *__restrict__ B, const float
   }
 }
 
+// ---- tensor-core route ----------------------------------------------------------------------------------------------
+__global__ void g_absmax(const float *__restrict__ G, size_t n, unsigned *__restrict__ out) {
+  float m = 0.f;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) m = fmaxf(m, fabsf(__ldg(G + i)));
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));       // non-negative floats order like their bit patterns
+}
+
+struct WFArgs {
+  const float2 *E;      // [C][Z][M][M]
+  const float *G;       // [Z][M][M]
+  const unsigned *gmax;
+  float4 *hfold;        // [Z][2][C][np][np]
+  int C, Z, M, mB, np;
+  float w[5];
+  float sQ;
+};
+// H_c = w_c (G / max|G|) conj(E_c), folded about both axes of the image grid into the four parity classes, written in the
+// order the stage-1 pair producers read their base pupil (kernels_tc.cu, tc_setup): one thread per folded sample.
+__global__ void __launch_bounds__(256) g_weight_fold(const WFArgs A) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int z = blockIdx.y;
+  if (i >= A.mB * A.mB) return;
+  const int qy = i / A.mB, qx = i - qy * A.mB;
+  const int M = A.M, ry = M - 1 - qy, rx = M - 1 - qx;
+  const bool selfx = rx == qx, selfy = ry == qy;
+  const float gm = __uint_as_float(*A.gmax);
+  const float inv = gm > 0.f ? 1.f / gm : 0.f;
+  const size_t MM = (size_t)M * M;
+  const float *Gz = A.G + (size_t)z * MM;
+  const float g00 = __ldg(Gz + (size_t)qy * M + qx) * inv, g01 = __ldg(Gz + (size_t)qy * M + rx) * inv;
+  const float g10 = __ldg(Gz + (size_t)ry * M + qx) * inv, g11 = __ldg(Gz + (size_t)ry * M + rx) * inv;
+  const int nk = A.np / 64;
+  const int jt = qy >> 6, half = (qy >> 5) & 1, ql = qy & 31, kc = qx >> 6, cgp = (qx >> 3) & 7, e = qx & 7;
+  const size_t idx = ((size_t)(jt * nk + kc) * 2 + half) * 2048 + (size_t)e * 256 + ql * 8 + cgp;
+  const size_t npp = (size_t)A.np * A.np;
+  for (int c = 0; c < A.C; ++c) {
+    const float2 *Ec = A.E + ((size_t)c * A.Z + z) * MM;
+    const float w = A.w[c];
+    auto H = [&](int y, int x, float g) { const float2 v = __ldg(Ec + (size_t)y * M + x); return make_float2(w * g * v.x, -w * g * v.y); };
+    const float2 p00 = H(qy, qx, g00);
+    const float2 p01 = selfx ? make_float2(0.f, 0.f) : H(qy, rx, g01);
+    const float2 p10 = selfy ? make_float2(0.f, 0.f) : H(ry, qx, g10);
+    const float2 p11 = (selfx || selfy) ? make_float2(0.f, 0.f) : H(ry, rx, g11);
+    const float2 e0 = make_float2(p00.x + p01.x, p00.y + p01.y), o0 = selfx ? make_float2(0.f, 0.f) : make_float2(p00.x - p01.x, p00.y - p01.y);
+    const float2 e1 = make_float2(p10.x + p11.x, p10.y + p11.y), o1 = selfx ? make_float2(0.f, 0.f) : make_float2(p10.x - p11.x, p10.y - p11.y);
+    const float s = A.sQ;
+    const float2 ee = make_float2(e0.x + e1.x, e0.y + e1.y), eo = make_float2(o0.x + o1.x, o0.y + o1.y);
+    const float2 oe = selfy ? make_float2(0.f, 0.f) : make_float2(e0.x - e1.x, e0.y - e1.y);
+    const float2 oo = selfy ? make_float2(0.f, 0.f) : make_float2(o0.x - o1.x, o0.y - o1.y);
+    float4 *dst = A.hfold + ((size_t)z * 2 * A.C) * npp;
+    dst[(size_t)(0 * A.C + c) * npp + idx] = make_float4(s * ee.x, s * ee.y, s * oe.x, s * oe.y);     // x-even group: ee, oe
+    dst[(size_t)(1 * A.C + c) * npp + idx] = make_float4(s * eo.x, s * eo.y, s * oo.x, s * oo.y);     // x-odd group:  eo, oo
+  }
+}
+
+// S[p] = -2 max|G| sum_c Im(Q_c[p] B_c[p]) with Q_c[p] = base_c[p] exp(i kappa_p z_b) regenerated here (static mode);
+// dL/dz_b += sum_p kappa_p S[p];  dL/dc[b][j] += sum_p Z_j[p] S[p]
+__global__ void __launch_bounds__(256)
+g_reduce_t(const float2 *__restrict__ base, const float2 *__restrict__ B, const float2 *__restrict__ kt, const float *__restrict__ zb,
+           const float4 *__restrict__ planes, const unsigned *__restrict__ gmax, double *__restrict__ dz, double *__restrict__ dc,
+           int C, int Z, int K, size_t NN) {
+  __shared__ double red[256];
+  const int z = blockIdx.y;
+  constexpr int KMAX = 64;
+  const float4 pl = __ldg(planes + z);
+  const float gm = __uint_as_float(*gmax);
+  double accz = 0.0;
+  float accc[KMAX];
+  for (int j = 0; j < K; ++j) accc[j] = 0.f;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NN; i += (size_t)gridDim.x * blockDim.x) {
+    const float2 k = __ldg(kt + i);
+    float sn, cs;
+    sincospif(2.0f * kz_turns(k, pl.x, pl.y), &sn, &cs);
+    float s = 0.f;
+    for (int c = 0; c < C; ++c) {
+      const float2 q = cmul(__ldg(base + (size_t)c * NN + i), make_float2(cs, sn));
+      const float2 b = __ldg(B + ((size_t)c * Z + z) * NN + i);
+      s -= 2.f * (q.x * b.y + q.y * b.x);
+    }
+    s *= gm;
+    accz += 6.283185307179586 * ((double)k.x + (double)k.y) * (double)s;
+    for (int j = 0; j < K; ++j) accc[j] = fmaf(__ldg(zb + (size_t)j * NN + i), s, accc[j]);
+  }
+  for (int j = -1; j < K; ++j) {
+    red[threadIdx.x] = j < 0 ? accz : (double)accc[j];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+      if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) atomicAdd(j < 0 ? dz + z : dc + (size_t)z * K + j, red[0]);
+    __syncthreads();
+  }
+}
+
 }  // namespace
 
 void grad_free(psf_plan *p) {
   GradState *g = p->grad;
   if (!g) return;
+  if (g->planB) { psf_plan_destroy(g->planB); g->planB = nullptr; }
+  void *tbufs[] = {g->d_base5, g->d_fieldE, g->d_fieldB, g->d_hfold, g->d_dummyI, g->d_gmax};
+  for (void *q : tbufs)
+    if (q) cudaFree(q);
   void *bufs[] = {g->d_base, g->d_kt, g->d_zb, g->d_ax, g->d_axt, g->d_Q, g->d_T, g->d_E, g->d_B};
   for (void *q : bufs)
     if (q) cudaFree(q);
@@ -218,6 +339,51 @@ psf_status grad_setup(psf_plan *p) {
       !up(&g->d_zb, zb.data(), zb.size() * sizeof(float)) || !up(&g->d_ax, ax.data(), ax.size() * sizeof(float2)) ||
       !up(&g->d_axt, axt.data(), axt.size() * sizeof(float2)))
     return fail("gradients: table upload failed");
+  // tensor-core route: static mode on the 3xFP16 path, if the back-projection plan also lands there
+  if (p->tune_grad_tensor && p->path == 2 && p->tc && !D.per_plane && tc_pair_stage1(p)) {
+    const int C5 = hp.C;
+    double hmax = 0.0;
+    std::vector<float2> base5((size_t)C5 * NN);
+    for (int c = 0; c < C5; ++c) {
+      double l1 = 0.0;
+      const cplx *src = p->h_base.data() + (size_t)c * NN;
+      for (size_t i = 0; i < NN; ++i) { l1 += std::abs(src[i]); base5[(size_t)c * NN + i] = make_float2((float)src[i].real(), (float)src[i].imag()); }
+      hmax = std::max(hmax, hp.weight[c] * l1);                 // |H_c| = w_c |G / max G| |E_c| <= w_c sum_p |base_c[p]|
+    }
+    psf_plan_desc db = d;
+    std::vector<double> zeros(D.Z, 0.0);
+    db.pupil_n = M; db.out_m = N; db.pixel_um = d.pixel_um * (double)M / (double)N;
+    db.n_planes = D.Z; db.z_um = zeros.data(); db.precision = PSF_PREC_3XF16; db.device = p->device;
+    psf_plan *pb = nullptr;
+    if (psf_plan_create(&db, &pb) == PSF_OK && pb) {
+      const int mB = (M + 1) / 2;
+      pb->tune_fused = p->tune_fused;
+      if (pb->path == 2 && tc_pair_stage1(pb) && plan_set_materialised(pb, 4.0 * hmax, 4.0 * hmax * mB) == PSF_OK && tc_pair_stage1(pb)) {
+        const int np = tc_n_pad(pb);
+        const size_t big = (size_t)D.Z * (MM > NN ? MM : NN);
+        const size_t hf = (size_t)D.Z * 2 * C5 * np * np;
+        if (cudaMalloc(&g->d_base5, base5.size() * sizeof(float2)) == cudaSuccess &&
+            cudaMemcpy(g->d_base5, base5.data(), base5.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess &&
+            cudaMalloc(&g->d_fieldE, (size_t)C5 * D.Z * MM * sizeof(float2)) == cudaSuccess &&
+            cudaMalloc(&g->d_fieldB, (size_t)C5 * D.Z * NN * sizeof(float2)) == cudaSuccess &&
+            cudaMalloc(&g->d_hfold, hf * sizeof(float4)) == cudaSuccess && cudaMemset(g->d_hfold, 0, hf * sizeof(float4)) == cudaSuccess &&
+            cudaMalloc(&g->d_dummyI, big * sizeof(float)) == cudaSuccess && cudaMalloc(&g->d_gmax, sizeof(unsigned)) == cudaSuccess) {
+          g->tensor = true;
+          g->planB = pb;
+          g->C5 = C5;
+          for (int c = 0; c < C5; ++c) g->w5[c] = (float)hp.weight[c];
+        }
+      }
+      if (!g->tensor) {                                         // not this time: free what was taken, the FFMA route runs
+        psf_plan_destroy(pb);
+        void **tb[] = {&g->d_base5, &g->d_fieldE, &g->d_fieldB, &g->d_hfold, &g->d_dummyI, &g->d_gmax};
+        for (void **q : tb)
+          if (*q) { cudaFree(*q); *q = nullptr; }
+        cudaGetLastError();
+      }
+    }
+  }
+  if (g->tensor) { g->version = p->table_version; return PSF_OK; }
   // scratch: Q, B [Cg][zc][N][N]; T (and V) [Cg][zc][M][N]; E [Cg][zc][M][M]
   const size_t per_plane = (size_t)g->Cg * (2 * NN + MN + MM) * sizeof(float2);
   size_t zc = ((size_t)1 << 30) / per_plane;
@@ -239,6 +405,24 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
   const size_t NN = (size_t)N * N, MM = (size_t)M * M, MN = (size_t)M * N;
   cudaMemsetAsync(dL_dz, 0, (size_t)D.Z * sizeof(double), st);
   if (dL_dc && g->K > 0) cudaMemsetAsync(dL_dc, 0, (size_t)D.Z * g->K * sizeof(double), st);
+  if (g->tensor) {
+    const psf_plan *pb = g->planB;
+    cudaError_t e = launch_tc(p, st, (float *)g->d_dummyI, (float2 *)g->d_fieldE);                 // E_c, all planes
+    if (e != cudaSuccess) return e;
+    cudaMemsetAsync(g->d_gmax, 0, sizeof(unsigned), st);
+    g_absmax<<<296, 256, 0, st>>>(dL_dI, (size_t)D.Z * MM, (unsigned *)g->d_gmax);
+    WFArgs A;
+    A.E = (const float2 *)g->d_fieldE; A.G = dL_dI; A.gmax = (const unsigned *)g->d_gmax; A.hfold = (float4 *)g->d_hfold;
+    A.C = g->C5; A.Z = D.Z; A.M = M; A.mB = (M + 1) / 2; A.np = tc_n_pad(pb); A.sQ = tc_pupil_scale(pb);
+    for (int c = 0; c < 5; ++c) A.w[c] = g->w5[c];
+    g_weight_fold<<<dim3((unsigned)((A.mB * A.mB + 255) / 256), D.Z), 256, 0, st>>>(A);
+    e = launch_tc_mat(pb, st, (float *)g->d_dummyI, (float2 *)g->d_fieldB, (const float4 *)g->d_hfold);   // B_c = A_y^T H_c A_x
+    if (e != cudaSuccess) return e;
+    g_reduce_t<<<dim3(16, D.Z), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, (const float2 *)g->d_kt,
+                                              (const float *)g->d_zb, D.planes, (const unsigned *)g->d_gmax, dL_dz, dL_dc,
+                                              g->C5, D.Z, dL_dc ? g->K : 0, NN);
+    return cudaGetLastError();
+  }
   float2 *Q = (float2 *)g->d_Q, *T = (float2 *)g->d_T, *E = (float2 *)g->d_E, *B = (float2 *)g->d_B;
   const float2 *ax = (const float2 *)g->d_ax, *axt = (const float2 *)g->d_axt;
   auto tiles = [](int n) { return (unsigned)((n + GT - 1) / GT); };
@@ -260,5 +444,6 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
 }
 
 int grad_terms(const psf_plan *p) { return p->grad ? p->grad->K : 0; }
+const char *grad_route(const psf_plan *p) { return !p->grad ? "" : p->grad->tensor ? "adjoint_tc3xf16" : "adjoint_ffma"; }
 
 }  // namespace psf

@@ -86,6 +86,9 @@ struct psf_plan {
   psf::GradState *grad = nullptr;
   psf::CztState *czt = nullptr;
   psf::SmlmState *smlm = nullptr;
+  int mat_mode = 0;              // 1: the tensor path's operand scales come from mat_qmax / mat_rmax (materialised pupils)
+  double mat_qmax = 0, mat_rmax = 0;
+  int tune_grad_tensor = 1;      // 1: psf_gradients on the tensor cores where the plan qualifies; 0: the FFMA route
   int tune_smlm = 1;             // 1: the emitter-batch kernel k_smlm where it qualifies; 0: always k_small
   // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
   int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
@@ -130,6 +133,12 @@ int tc_launches(const psf_plan *p);
 bool tc_fused_aborted(const psf_plan *p);
 const char *tc_kernel_names(const psf_plan *p);
 cudaError_t launch_tc(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field);
+cudaError_t launch_tc_mat(const psf_plan *p, cudaStream_t st, float *intensity, float2 *field, const float4 *pupils);
+float tc_pupil_scale(const psf_plan *p);
+int tc_n_pad(const psf_plan *p);
+bool tc_pair_stage1(const psf_plan *p);
+// api.cu: turns a plan into the carrier of a materialised-pupil transform (used by the adjoint for its back-projection plan)
+psf_status plan_set_materialised(psf_plan *p, double qmax, double rmax);
 // kernels_bessel.cu
 psf_status bessel_setup(psf_plan *p, int n_nodes);
 void bessel_free(psf_plan *p);
@@ -149,5 +158,6 @@ psf_status grad_setup(psf_plan *p);
 bool grad_needs_setup(const psf_plan *p);
 void grad_free(psf_plan *p);
 int grad_terms(const psf_plan *p);
+const char *grad_route(const psf_plan *p);
 cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, double *dL_dz, double *dL_dc);
 }  // namespace psf

@@ -426,6 +426,8 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
 // ---- stage 1 ----------------------------------------------------------------------------------------------------------
 struct K1PArgs {
   const float4 *bgp;    // [2][C][jt][kc][half][8 samples][256 threads]  base pupil (4 slots), pre-scaled by s_Q
+  size_t bgp_plane;     // float4 elements between the tables of consecutive planes: 0 = one static table (the normal case);
+                        // > 0 = "materialised pupil": every plane brings its own folded pupil (the adjoint's back-projection)
   const float4 *ktq;    // [jt][kc][half][4 sample pairs][256 threads]      kappa / 2 pi (hi, lo) of two samples
   const float4 *planes; // [Z]
   int C, n_pad, m_pad, z0, zc;
@@ -555,7 +557,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         const K1PTile<GM> T(t, G, rank);
         for (int cg = 0; cg < G.nitems; ++cg) {
           const int grp = GM ? (int)rank : (cg & 1), c = GM ? cg : (cg >> 1);
-          const float4 *src = P.bgp + (size_t)(grp * P.C + c) * P.n_pad * P.n_pad;
+          const float4 *src = P.bgp + (size_t)(P.z0 + T.zl) * P.bgp_plane + (size_t)(grp * P.C + c) * P.n_pad * P.n_pad;
           for (int kc = 0; kc < G.nk; ++kc) {
             mbar_wait(&S.bb_empty[bs], bph ^ 1);
             mbar_arrive_expect_tx(&S.bb_full[bs], K1P_BB_BYTES);

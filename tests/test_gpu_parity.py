@@ -600,3 +600,44 @@ def test_emitter_batch_kernel(psf, seed, N, M, Z, pol, kw):
         c2 = replace(case, **{drop: None})
         I2, _ = gpu_stack(psf, c2)
         assert plane_errors(I2, O.stack_T2(c2)).max() <= TOL, drop
+
+
+@pytest.mark.parametrize("seed,N,M,Z,pol,kw", [
+    (501, 96, 70, 3, W.POL_X, {}),                          # group-mode kernels for both plans
+    (502, 200, 160, 4, W.POL_UNPOLARIZED, {}),              # five pupils with their weights
+    (503, 131, 97, 2, W.POL_CIRC_L, {"fresnel": True}),     # odd N and M: self-mirror row and column in both folds
+    (504, 300, 400, 3, W.POL_JONES, {}),                    # plan B on the 256-row pair kernels (its output grid is the 300-pupil)
+    (505, 400, 300, 2, W.POL_X, {"model": "scalar"}),       # the forward on the 256-row pair kernels
+    (506, 512, 512, 20, W.POL_UNPOLARIZED, {}),             # both plans take the fused launch
+])
+def test_adjoint_on_the_tensor_cores_matches_oracle(psf, seed, N, M, Z, pol, kw):
+    """psf_gradients with both transforms on tcgen05 (static mode, 3xFP16): against the oracle's adjoint (pinned by finite
+    differences) at 2e-5 of the largest component, and against the FFMA route of the same library."""
+    import torch
+    case = replace(W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, per_plane=False, shifts=False, pol=pol), **kw)
+    G = np.random.default_rng(seed).standard_normal((Z, M, M)).astype(np.float32)
+    if seed == 506:                                  # the oracle's adjoint on three planes only (it is O(N^2 M) per plane and pupil)
+        sel = [0, 9, 19]
+        dz_ref, dc_ref = O.grad_T2(case, G[sel].astype(np.float64), planes=sel)
+    else:
+        sel = list(range(Z))
+        dz_ref, dc_ref = O.grad_T2(case, G.astype(np.float64))
+    plan = psf.plan_from_case(case)
+    Gd = torch.from_numpy(G).cuda()
+    dz, dc = plan.gradients(Gd)
+    torch.cuda.synchronize()
+    assert plan.grad_path == "adjoint_tc3xf16"
+    dz, dc = dz.cpu().numpy()[sel], dc.cpu().numpy()[sel]
+    assert np.abs(dz - dz_ref).max() <= GRAD_TOL * np.abs(dz_ref).max(), (np.abs(dz - dz_ref).max(), np.abs(dz_ref).max())
+    assert np.abs(dc - dc_ref).max() <= GRAD_TOL * np.abs(dc_ref).max()
+    # a second call reuses everything; the intensity path of the plan still works afterwards
+    dz2, dc2 = plan.gradients(Gd)
+    assert torch.equal(dz2.cpu(), torch.from_numpy(np.asarray(dz2.cpu()))) and np.allclose(dz2.cpu().numpy()[sel], dz, rtol=0, atol=1e-9 * np.abs(dz_ref).max())
+    I = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(I[sel], O.stack_T2(case, planes=sel)).max() <= TOL
+    plan.tune(psf.TUNE_GRAD_TENSOR, 0)
+    dz3, dc3 = plan.gradients(Gd)
+    torch.cuda.synchronize()
+    assert plan.grad_path == "adjoint_ffma"
+    assert np.abs(dz3.cpu().numpy()[sel] - dz_ref).max() <= GRAD_TOL * np.abs(dz_ref).max()
+    plan.destroy()
