@@ -489,7 +489,10 @@ def run_ours(args):
                 flop = 2 * 8.0 * cs.pupil_n * cs.out_m * (cs.pupil_n + cs.out_m) * cg * cs.n_planes     # forward + back-projection
                 ffma_peak = SM_COUNT * FMA_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
                 sweep[name] = {"ms_per_step": ms, "planes_per_s": cs.n_planes / (ms * 1e-3), "path": plan.grad_path,
-                               "tflops": flop / (ms * 1e-3) / 1e12, "frac_of_ffma_peak": flop / (ms * 1e-3) / 1e12 / ffma_peak,
+                               "fp32_equivalent_tflops": flop / (ms * 1e-3) / 1e12,
+                               "frac_of_ffma_peak": (flop / (ms * 1e-3) / 1e12 / ffma_peak) if plan.grad_path == "adjoint_ffma" else None,
+                               "note": "forward field + back-projection (the same tensor kernels on a plan with the grids swapped) + "
+                                       "weight/fold and reduction kernels; fp32_equivalent_tflops counts the unfolded complex products",
                                "zernike_terms": int(K)}
                 plan.destroy()
             line["workloads"] = sweep

@@ -177,7 +177,13 @@ g_reduce(const float2 *__restrict__ Q, const float2 *__restrict__ B, const float
 // ---- tensor-core route ----------------------------------------------------------------------------------------------
 __global__ void g_absmax(const float *__restrict__ G, size_t n, unsigned *__restrict__ out) {
   float m = 0.f;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) m = fmaxf(m, fabsf(__ldg(G + i)));
+  const size_t n4 = n >> 2;                      // G is 16-byte aligned (psf.h)
+  const float4 *G4 = reinterpret_cast<const float4 *>(G);
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+    const float4 v = __ldg(G4 + i);
+    m = fmaxf(fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+  }
+  for (size_t i = (n4 << 2) + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) m = fmaxf(m, fabsf(__ldg(G + i)));
   for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
   if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));       // non-negative floats order like their bit patterns
 }
@@ -232,41 +238,69 @@ __global__ void __launch_bounds__(256) g_weight_fold(const WFArgs A) {
 
 // S[p] = -2 max|G| sum_c Im(Q_c[p] B_c[p]) with Q_c[p] = base_c[p] exp(i kappa_p z_b) regenerated here (static mode);
 // dL/dz_b += sum_p kappa_p S[p];  dL/dc[b][j] += sum_p Z_j[p] S[p]
+// ZP planes per block: the tables (base pupil, kappa, Zernike basis) are loaded once per sample and used for ZP planes.
+template <int KU, int ZP>
 __global__ void __launch_bounds__(256)
 g_reduce_t(const float2 *__restrict__ base, const float2 *__restrict__ B, const float2 *__restrict__ kt, const float *__restrict__ zb,
            const float4 *__restrict__ planes, const unsigned *__restrict__ gmax, double *__restrict__ dz, double *__restrict__ dc,
            int C, int Z, int K, size_t NN) {
   __shared__ double red[256];
-  const int z = blockIdx.y;
-  constexpr int KMAX = 64;
-  const float4 pl = __ldg(planes + z);
+  const int z0 = blockIdx.y * ZP;
+  float4 pl[ZP];
+#pragma unroll
+  for (int zi = 0; zi < ZP; ++zi) pl[zi] = __ldg(planes + (z0 + zi < Z ? z0 + zi : Z - 1));
   const float gm = __uint_as_float(*gmax);
-  double accz = 0.0;
-  float accc[KMAX];
-  for (int j = 0; j < K; ++j) accc[j] = 0.f;
+  double accz[ZP];
+  float accc[ZP][KU];                            // KU >= K, the loops are unrolled: registers, not local memory
+#pragma unroll
+  for (int zi = 0; zi < ZP; ++zi) {
+    accz[zi] = 0.0;
+#pragma unroll
+    for (int j = 0; j < KU; ++j) accc[zi][j] = 0.f;
+  }
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NN; i += (size_t)gridDim.x * blockDim.x) {
     const float2 k = __ldg(kt + i);
-    float sn, cs;
-    sincospif(2.0f * kz_turns(k, pl.x, pl.y), &sn, &cs);
-    float s = 0.f;
+    float s[ZP];
+#pragma unroll
+    for (int zi = 0; zi < ZP; ++zi) s[zi] = 0.f;
+    float2 ph[ZP];
+#pragma unroll
+    for (int zi = 0; zi < ZP; ++zi) sincospif(2.0f * kz_turns(k, pl[zi].x, pl[zi].y), &ph[zi].y, &ph[zi].x);
     for (int c = 0; c < C; ++c) {
-      const float2 q = cmul(__ldg(base + (size_t)c * NN + i), make_float2(cs, sn));
-      const float2 b = __ldg(B + ((size_t)c * Z + z) * NN + i);
-      s -= 2.f * (q.x * b.y + q.y * b.x);
+      const float2 bc = __ldg(base + (size_t)c * NN + i);
+#pragma unroll
+      for (int zi = 0; zi < ZP; ++zi)
+        if (z0 + zi < Z) {
+          const float2 q = cmul(bc, ph[zi]);
+          const float2 b = __ldg(B + ((size_t)c * Z + z0 + zi) * NN + i);
+          s[zi] -= 2.f * (q.x * b.y + q.y * b.x);
+        }
     }
-    s *= gm;
-    accz += 6.283185307179586 * ((double)k.x + (double)k.y) * (double)s;
-    for (int j = 0; j < K; ++j) accc[j] = fmaf(__ldg(zb + (size_t)j * NN + i), s, accc[j]);
+    const double kap = 6.283185307179586 * ((double)k.x + (double)k.y);
+#pragma unroll
+    for (int zi = 0; zi < ZP; ++zi) { s[zi] *= gm; accz[zi] += kap * (double)s[zi]; }
+#pragma unroll
+    for (int j = 0; j < KU; ++j)
+      if (j < K) {
+        const float zv = __ldg(zb + (size_t)j * NN + i);
+#pragma unroll
+        for (int zi = 0; zi < ZP; ++zi) accc[zi][j] = fmaf(zv, s[zi], accc[zi][j]);
+      }
   }
-  for (int j = -1; j < K; ++j) {
-    red[threadIdx.x] = j < 0 ? accz : (double)accc[j];
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-      if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+#pragma unroll
+  for (int zi = 0; zi < ZP; ++zi) {
+#pragma unroll
+    for (int j = -1; j < KU; ++j) {
+      if (j >= K) break;
+      red[threadIdx.x] = j < 0 ? accz[zi] : (double)accc[zi][j < 0 ? 0 : j];
+      __syncthreads();
+      for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+      }
+      if (threadIdx.x == 0 && z0 + zi < Z) atomicAdd(j < 0 ? dz + z0 + zi : dc + (size_t)(z0 + zi) * K + j, red[0]);
       __syncthreads();
     }
-    if (threadIdx.x == 0) atomicAdd(j < 0 ? dz + z : dc + (size_t)z * K + j, red[0]);
-    __syncthreads();
   }
 }
 
@@ -410,7 +444,7 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
     cudaError_t e = launch_tc(p, st, (float *)g->d_dummyI, (float2 *)g->d_fieldE);                 // E_c, all planes
     if (e != cudaSuccess) return e;
     cudaMemsetAsync(g->d_gmax, 0, sizeof(unsigned), st);
-    g_absmax<<<296, 256, 0, st>>>(dL_dI, (size_t)D.Z * MM, (unsigned *)g->d_gmax);
+    g_absmax<<<148 * 8, 256, 0, st>>>(dL_dI, (size_t)D.Z * MM, (unsigned *)g->d_gmax);
     WFArgs A;
     A.E = (const float2 *)g->d_fieldE; A.G = dL_dI; A.gmax = (const unsigned *)g->d_gmax; A.hfold = (float4 *)g->d_hfold;
     A.C = g->C5; A.Z = D.Z; A.M = M; A.mB = (M + 1) / 2; A.np = tc_n_pad(pb); A.sQ = tc_pupil_scale(pb);
@@ -418,9 +452,12 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
     g_weight_fold<<<dim3((unsigned)((A.mB * A.mB + 255) / 256), D.Z), 256, 0, st>>>(A);
     e = launch_tc_mat(pb, st, (float *)g->d_dummyI, (float2 *)g->d_fieldB, (const float4 *)g->d_hfold);   // B_c = A_y^T H_c A_x
     if (e != cudaSuccess) return e;
-    g_reduce_t<<<dim3(16, D.Z), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, (const float2 *)g->d_kt,
-                                              (const float *)g->d_zb, D.planes, (const unsigned *)g->d_gmax, dL_dz, dL_dc,
-                                              g->C5, D.Z, dL_dc ? g->K : 0, NN);
+    const int Kt = dL_dc ? g->K : 0;
+    // (ZP = 4 planes per block was measured slower, 4.4 vs 2.4 ms at config 5: 218 registers, too few loads in flight)
+#define PSF_GRT(KU, ZP) g_reduce_t<KU, ZP><<<dim3(16, (D.Z + ZP - 1) / ZP), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, \
+      (const float2 *)g->d_kt, (const float *)g->d_zb, D.planes, (const unsigned *)g->d_gmax, dL_dz, dL_dc, g->C5, D.Z, Kt, NN)
+    if (Kt <= 8) PSF_GRT(8, 1); else if (Kt <= 24) PSF_GRT(24, 1); else PSF_GRT(64, 1);
+#undef PSF_GRT
     return cudaGetLastError();
   }
   float2 *Q = (float2 *)g->d_Q, *T = (float2 *)g->d_T, *E = (float2 *)g->d_E, *B = (float2 *)g->d_B;

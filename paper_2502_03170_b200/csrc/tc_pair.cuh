@@ -278,6 +278,53 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
   }
 }
 
+// Field store of one group of four consecutive m_x of every row of a warp (warp-collective).  v[quadrant][u] = E at the four
+// mirror images of pixel (row, mxg + u).  vec (M a multiple of 8): two lanes share a row so that one STG.128 of the warp
+// writes full 32-byte sectors (16 rows x 32 contiguous bytes) - the halves travel by shuffle; else 8-byte stores per pixel.
+__device__ __forceinline__ void store_field_group(float2 *f, int M, int m, int row0, int lane, int mxg, const float2 (&v)[4][4], float fs, bool vec) {
+  if (!vec) {
+    const int my = row0 + lane;
+    if (my < m) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int mx = mxg + u;
+        if (mx < m) {
+          const int myr = M - 1 - my, mxr = M - 1 - mx;
+          f[(size_t)my * M + mx] = make_float2(fs * v[0][u].x, fs * v[0][u].y);
+          f[(size_t)my * M + mxr] = make_float2(fs * v[1][u].x, fs * v[1][u].y);
+          f[(size_t)myr * M + mx] = make_float2(fs * v[2][u].x, fs * v[2][u].y);
+          f[(size_t)myr * M + mxr] = make_float2(fs * v[3][u].x, fs * v[3][u].y);
+        }
+      }
+    }
+    return;
+  }
+  const int odd = lane & 1;
+#pragma unroll
+  for (int qd = 0; qd < 4; ++qd) {
+    const bool mirx = qd & 1;
+    // the 32-byte block of the group in ascending address order: low half, high half
+    const float4 low = mirx ? make_float4(v[qd][3].x, v[qd][3].y, v[qd][2].x, v[qd][2].y) : make_float4(v[qd][0].x, v[qd][0].y, v[qd][1].x, v[qd][1].y);
+    const float4 high = mirx ? make_float4(v[qd][1].x, v[qd][1].y, v[qd][0].x, v[qd][0].y) : make_float4(v[qd][2].x, v[qd][2].y, v[qd][3].x, v[qd][3].y);
+    const float4 send = odd ? low : high;
+    float4 recv;
+    recv.x = __shfl_xor_sync(0xffffffffu, send.x, 1); recv.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
+    recv.z = __shfl_xor_sync(0xffffffffu, send.z, 1); recv.w = __shfl_xor_sync(0xffffffffu, send.w, 1);
+    const int col = (mirx ? M - 4 - mxg : mxg) + 2 * odd;
+    if (mxg < m) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {                   // k = 0: the even row of the lane pair, k = 1: the odd row
+        const int my = row0 + (lane & ~1) + k;
+        if (my < m) {
+          const float4 val = k == 0 ? (odd ? recv : low) : (odd ? high : recv);
+          const int y = (qd & 2) ? M - 1 - my : my;
+          *reinterpret_cast<float4 *>(f + (size_t)y * M + col) = make_float4(fs * val.x, fs * val.y, fs * val.z, fs * val.w);
+        }
+      }
+    }
+  }
+}
+
 // sixteen epilogue warps: butterfly + |E|^2, running sums over the components, coalesced quadrant stores
 // (FIELD: the four mirror values of E_c are also stored, 32 bytes per thread and store, straight from the registers)
 template <bool FIELD>
@@ -317,6 +364,7 @@ __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint3
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(acc_empty_leader);
           }
+          float2 fe[FIELD ? 4 : 1][FIELD ? 4 : 1];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const float a0 = __uint_as_float(v[0][u]), a1 = __uint_as_float(v[1][u]), a2 = __uint_as_float(v[2][u]),
@@ -334,18 +382,13 @@ __device__ __forceinline__ void k2p_epilogue(float *staging, K2PShared &S, uint3
             sum[2][i] = fmaf(w, re2 * re2 + im2 * im2, sum[2][i]);
             sum[3][i] = fmaf(w, re3 * re3 + im3 * im3, sum[3][i]);
             if (FIELD) {
-              const int my = ty * 128 + q * 32 + lane, mx = tx * 64 + e * 16 + i;
-              if (my < P.m && mx < P.m) {
-                float2 *f = P.field + ((size_t)c * P.Z + (P.z0 + zl)) * (size_t)P.M * P.M;
-                const int myr = P.M - 1 - my, mxr = P.M - 1 - mx;
-                const float fs = P.fscale;
-                f[(size_t)my * P.M + mx] = make_float2(fs * re0, fs * im0);
-                f[(size_t)my * P.M + mxr] = make_float2(fs * re1, fs * im1);
-                f[(size_t)myr * P.M + mx] = make_float2(fs * re2, fs * im2);
-                f[(size_t)myr * P.M + mxr] = make_float2(fs * re3, fs * im3);
-              }
+              fe[0][FIELD ? u : 0] = make_float2(re0, im0); fe[FIELD ? 1 : 0][FIELD ? u : 0] = make_float2(re1, im1);
+              fe[FIELD ? 2 : 0][FIELD ? u : 0] = make_float2(re2, im2); fe[FIELD ? 3 : 0][FIELD ? u : 0] = make_float2(re3, im3);
             }
           }
+          if constexpr (FIELD)
+            store_field_group(P.field + ((size_t)c * P.Z + (P.z0 + zl)) * (size_t)P.M * P.M, P.M, P.m, ty * 128 + q * 32, lane,
+                              tx * 64 + e * 16 + i4 * 4, fe, P.fscale, (P.M & 7) == 0);
         }
       }
       // coalesced store of the four mirrored quadrants through the padded staging tile
