@@ -236,70 +236,78 @@ __global__ void __launch_bounds__(256) g_weight_fold(const WFArgs A) {
   }
 }
 
-// S[p] = -2 max|G| sum_c Im(Q_c[p] B_c[p]) with Q_c[p] = base_c[p] exp(i kappa_p z_b) regenerated here (static mode);
-// dL/dz_b += sum_p kappa_p S[p];  dL/dc[b][j] += sum_p Z_j[p] S[p]
-// ZP planes per block: the tables (base pupil, kappa, Zernike basis) are loaded once per sample and used for ZP planes.
-template <int KU, int ZP>
+// Pupil-side sensitivity S[z][p] = -2 max|G| sum_c Im(Q_c[p] B_c[p]), Q_c[p] = base_c[p] exp(i kappa_p z) regenerated here.
 __global__ void __launch_bounds__(256)
-g_reduce_t(const float2 *__restrict__ base, const float2 *__restrict__ B, const float2 *__restrict__ kt, const float *__restrict__ zb,
-           const float4 *__restrict__ planes, const unsigned *__restrict__ gmax, double *__restrict__ dz, double *__restrict__ dc,
-           int C, int Z, int K, size_t NN) {
-  __shared__ double red[256];
-  const int z0 = blockIdx.y * ZP;
-  float4 pl[ZP];
-#pragma unroll
-  for (int zi = 0; zi < ZP; ++zi) pl[zi] = __ldg(planes + (z0 + zi < Z ? z0 + zi : Z - 1));
-  const float gm = __uint_as_float(*gmax);
-  double accz[ZP];
-  float accc[ZP][KU];                            // KU >= K, the loops are unrolled: registers, not local memory
-#pragma unroll
-  for (int zi = 0; zi < ZP; ++zi) {
-    accz[zi] = 0.0;
-#pragma unroll
-    for (int j = 0; j < KU; ++j) accc[zi][j] = 0.f;
+g_dphi(const float2 *__restrict__ base, const float2 *__restrict__ B, const float2 *__restrict__ kt, const float4 *__restrict__ planes,
+       const unsigned *__restrict__ gmax, float *__restrict__ S, int C, int Z, size_t NN) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int z = blockIdx.y;
+  if (i >= NN) return;
+  const float4 pl = __ldg(planes + z);
+  float sn, cs;
+  sincospif(2.0f * kz_turns(__ldg(kt + i), pl.x, pl.y), &sn, &cs);
+  float s = 0.f;
+  for (int c = 0; c < C; ++c) {
+    const float2 q = cmul(__ldg(base + (size_t)c * NN + i), make_float2(cs, sn));
+    const float2 b = __ldg(B + ((size_t)c * Z + z) * NN + i);
+    s -= 2.f * (q.x * b.y + q.y * b.x);
   }
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NN; i += (size_t)gridDim.x * blockDim.x) {
-    const float2 k = __ldg(kt + i);
-    float s[ZP];
-#pragma unroll
-    for (int zi = 0; zi < ZP; ++zi) s[zi] = 0.f;
-    float2 ph[ZP];
-#pragma unroll
-    for (int zi = 0; zi < ZP; ++zi) sincospif(2.0f * kz_turns(k, pl[zi].x, pl[zi].y), &ph[zi].y, &ph[zi].x);
-    for (int c = 0; c < C; ++c) {
-      const float2 bc = __ldg(base + (size_t)c * NN + i);
-#pragma unroll
-      for (int zi = 0; zi < ZP; ++zi)
-        if (z0 + zi < Z) {
-          const float2 q = cmul(bc, ph[zi]);
-          const float2 b = __ldg(B + ((size_t)c * Z + z0 + zi) * NN + i);
-          s[zi] -= 2.f * (q.x * b.y + q.y * b.x);
-        }
+  S[(size_t)z * NN + i] = s * __uint_as_float(*gmax);
+}
+
+// dL/dz_b = sum_p kappa_p S[b][p],  dL/dc[b][j] = sum_p Z_j[p] S[b][p]: a skinny product [Z x N^2] . [N^2 x (K + 1)].
+// Block = 16 planes x one chunk of 4096 samples, in tiles of 256 samples through shared memory; thread = (plane, j mod 16);
+// fp32 sums inside a tile, fp64 across tiles, one atomicAdd per (block, plane, j).
+constexpr int SR_ZT = 16, SR_TILE = 256, SR_CHUNK = 4096, SR_PITCH = SR_TILE + 1, SR_JMAX = 5;
+__global__ void __launch_bounds__(256)
+g_sred(const float *__restrict__ S, const float2 *__restrict__ kt, const float *__restrict__ zb, double *__restrict__ dz,
+       double *__restrict__ dc, int Z, int K, size_t NN) {
+  extern __shared__ float sr_smem[];
+  float *Ss = sr_smem;                         // [SR_ZT][SR_PITCH]
+  float *Ws = sr_smem + SR_ZT * SR_PITCH;      // [K + 1][SR_PITCH]: row 0 = kappa, row 1 + j = Z_j
+  const int KW = K + 1;
+  const int z0 = blockIdx.y * SR_ZT;
+  const int tz = threadIdx.x >> 4, tj = threadIdx.x & 15;
+  double acc[SR_JMAX] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  const size_t i0 = (size_t)blockIdx.x * SR_CHUNK;
+  for (int t = 0; t < SR_CHUNK / SR_TILE; ++t) {
+    const size_t ib = i0 + (size_t)t * SR_TILE;
+    if (ib >= NN) break;
+    __syncthreads();
+    for (int e = threadIdx.x; e < SR_ZT * SR_TILE; e += 256) {
+      const int zz = e / SR_TILE, ii = e % SR_TILE;
+      Ss[zz * SR_PITCH + ii] = (z0 + zz < Z && ib + ii < NN) ? __ldg(S + (size_t)(z0 + zz) * NN + ib + ii) : 0.f;
     }
-    const double kap = 6.283185307179586 * ((double)k.x + (double)k.y);
-#pragma unroll
-    for (int zi = 0; zi < ZP; ++zi) { s[zi] *= gm; accz[zi] += kap * (double)s[zi]; }
-#pragma unroll
-    for (int j = 0; j < KU; ++j)
-      if (j < K) {
-        const float zv = __ldg(zb + (size_t)j * NN + i);
-#pragma unroll
-        for (int zi = 0; zi < ZP; ++zi) accc[zi][j] = fmaf(zv, s[zi], accc[zi][j]);
+    for (int e = threadIdx.x; e < KW * SR_TILE; e += 256) {
+      const int jj = e / SR_TILE, ii = e % SR_TILE;
+      float w = 0.f;
+      if (ib + ii < NN) {
+        if (jj == 0) { const float2 k = __ldg(kt + ib + ii); w = 6.283185307179586f * (k.x + k.y); }
+        else w = __ldg(zb + (size_t)(jj - 1) * NN + ib + ii);
       }
+      Ws[jj * SR_PITCH + ii] = w;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < SR_JMAX; ++u) {
+      const int j = tj + 16 * u;
+      if (j < KW) {
+        float a = 0.f;
+        const float *sr = Ss + tz * SR_PITCH, *wr = Ws + j * SR_PITCH;
+#pragma unroll 8
+        for (int ii = 0; ii < SR_TILE; ++ii) a = fmaf(sr[ii], wr[ii], a);
+        acc[u] += (double)a;
+      }
+    }
   }
+  if (z0 + tz < Z) {
 #pragma unroll
-  for (int zi = 0; zi < ZP; ++zi) {
-#pragma unroll
-    for (int j = -1; j < KU; ++j) {
-      if (j >= K) break;
-      red[threadIdx.x] = j < 0 ? accz[zi] : (double)accc[zi][j < 0 ? 0 : j];
-      __syncthreads();
-      for (int o = 128; o > 0; o >>= 1) {
-        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
-        __syncthreads();
+    for (int u = 0; u < SR_JMAX; ++u) {
+      const int j = tj + 16 * u;
+      if (j < KW) {
+        if (j == 0) atomicAdd(dz + z0 + tz, acc[u]);
+        else if (dc) atomicAdd(dc + (size_t)(z0 + tz) * K + (j - 1), acc[u]);
       }
-      if (threadIdx.x == 0 && z0 + zi < Z) atomicAdd(j < 0 ? dz + z0 + zi : dc + (size_t)(z0 + zi) * K + j, red[0]);
-      __syncthreads();
     }
   }
 }
@@ -402,6 +410,7 @@ psf_status grad_setup(psf_plan *p) {
             cudaMalloc(&g->d_fieldB, (size_t)C5 * D.Z * NN * sizeof(float2)) == cudaSuccess &&
             cudaMalloc(&g->d_hfold, hf * sizeof(float4)) == cudaSuccess && cudaMemset(g->d_hfold, 0, hf * sizeof(float4)) == cudaSuccess &&
             cudaMalloc(&g->d_dummyI, big * sizeof(float)) == cudaSuccess && cudaMalloc(&g->d_gmax, sizeof(unsigned)) == cudaSuccess) {
+          cudaFuncSetAttribute(g_sred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((SR_ZT + 65) * SR_PITCH * sizeof(float)));
           g->tensor = true;
           g->planB = pb;
           g->C5 = C5;
@@ -453,11 +462,13 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
     e = launch_tc_mat(pb, st, (float *)g->d_dummyI, (float2 *)g->d_fieldB, (const float4 *)g->d_hfold);   // B_c = A_y^T H_c A_x
     if (e != cudaSuccess) return e;
     const int Kt = dL_dc ? g->K : 0;
-    // (ZP = 4 planes per block was measured slower, 4.4 vs 2.4 ms at config 5: 218 registers, too few loads in flight)
-#define PSF_GRT(KU, ZP) g_reduce_t<KU, ZP><<<dim3(16, (D.Z + ZP - 1) / ZP), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, \
-      (const float2 *)g->d_kt, (const float *)g->d_zb, D.planes, (const unsigned *)g->d_gmax, dL_dz, dL_dc, g->C5, D.Z, Kt, NN)
-    if (Kt <= 8) PSF_GRT(8, 1); else if (Kt <= 24) PSF_GRT(24, 1); else PSF_GRT(64, 1);
-#undef PSF_GRT
+    // sensitivity S (fp32, in the dummy-intensity buffer, free by now), then the skinny product against kappa and the basis
+    float *S = (float *)g->d_dummyI;
+    g_dphi<<<dim3((unsigned)((NN + 255) / 256), D.Z), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, (const float2 *)g->d_kt,
+                                                                   D.planes, (const unsigned *)g->d_gmax, S, g->C5, D.Z, NN);
+    const size_t sr_bytes = (size_t)(SR_ZT + Kt + 1) * SR_PITCH * sizeof(float);
+    g_sred<<<dim3((unsigned)((NN + SR_CHUNK - 1) / SR_CHUNK), (D.Z + SR_ZT - 1) / SR_ZT), 256, sr_bytes, st>>>(
+        S, (const float2 *)g->d_kt, (const float *)g->d_zb, dL_dz, Kt ? dL_dc : nullptr, D.Z, Kt, NN);
     return cudaGetLastError();
   }
   float2 *Q = (float2 *)g->d_Q, *T = (float2 *)g->d_T, *E = (float2 *)g->d_E, *B = (float2 *)g->d_B;
