@@ -95,6 +95,7 @@ struct psf_plan {
   int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
   int tune_fused = 1;            // 1: both stages in one launch (k12_fused) where eligible; 0: always two launches
   int tune_k1p_handoff = 0;      // k1_pair: 0 plain remote arrive, 1 .release.cluster arrive per producer warp of the non-leader CTA
+  int tune_k1p_asplit = 1;       // k1_pair: 1 = the TMA-written table half of a stage buffer is released right behind its own stage
   int tune_k1p_defer = 1;        // k1_pair: K = 16 steps of the next stage issued before a stage buffer is released
   cudaEvent_t done_ev = nullptr; // recorded on the caller's stream after the last launch of every compute call: table
                                  // refreshes wait for it before they overwrite tables a launch in flight may still read

@@ -477,6 +477,8 @@ struct K1PArgs {
   float f1;             // epilogue factor s_T / (s_Q s_X)
   int handoff;          // how the non-leader CTA's producer warps signal the leader's barrier: 0 plain arrive, 1 cluster-scope release
   int defer;            // K = 16 steps of the next stage issued before a stage buffer is released (0 = released right behind its own stage)
+  int asplit;           // 1: the table half of a stage buffer (refilled by TMA, no hazard) has its own barrier and is released right
+                        // behind its own stage; only the producer-written half waits for the deferred release
 };
 
 constexpr int K1P_NST = 2;
@@ -492,6 +494,7 @@ constexpr int K1P_QY = 64;                                        // q_y per til
 
 struct K1PShared {
   uint64_t full[K1P_NST], empty[K1P_NST], acc_full[2], acc_empty[2];
+  uint64_t a_empty[K1P_NST];                                // table half of a stage buffer (asplit)
   uint64_t bb_full[K1P_BB_SLOTS], bb_empty[K1P_BB_SLOTS];   // base-pupil ring: bulk copy -> producers -> free
   uint32_t tmem_slot;
 };
@@ -546,7 +549,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
         for (int cg = 0; cg < G.nitems; ++cg) {
           const int row = GM ? (int)rank * P.m_pad + mt * 128 : (cg & 1) * P.m_pad + mt * 256 + (int)rank * 128;
           for (int kc = 0; kc < G.nk; ++kc) {
-            mbar_wait(&S.empty[st], ph ^ 1);
+            mbar_wait(P.asplit ? &S.a_empty[st] : &S.empty[st], ph ^ 1);
             const uint32_t s = smem_u32(smem + st * P_STAGE);
             if (leader) mbar_arrive_expect_tx(&S.full[st], 4 * TILE16K);
             tma2_load_2d(s, &map_xhi, full_leader[st], kc * 64, row);
@@ -580,6 +583,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
               // waits for those, which gives the peer that much tensor time of slack.
               if (k == P.defer - 1 && pending >= 0) { umma2_commit(&S.empty[pending]); pending = -1; }
             }
+            if (P.asplit) umma2_commit(&S.a_empty[st]);          // the TMA-written table tiles: free as soon as these UMMAs are done
             if (P.defer == 0) umma2_commit(&S.empty[st]);
             else pending = st;
             if (++st == K1P_NST) { st = 0; ph ^= 1; }
@@ -814,6 +818,7 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
     for (int i = 0; i < K1P_NST; ++i) {
       mbar_init(&S.full[i], 1 + 2 * K1P_PRODUCER_WARPS);  // the leader's expect_tx arrive + every producer warp of the pair
       mbar_init(&S.empty[i], 1);
+      mbar_init(&S.a_empty[i], 1);
     }
     for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S.bb_full[i], 1); mbar_init(&S.bb_empty[i], K1P_PRODUCER_WARPS); }
     for (int i = 0; i < 2; ++i) { mbar_init(&S.acc_full[i], 1); mbar_init(&S.acc_empty[i], 8); }
@@ -875,7 +880,7 @@ k12_fused(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ C
 
   if (threadIdx.x == 0) {
     if (stage1) {
-      for (int i = 0; i < K1P_NST; ++i) { mbar_init(&S1.full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&S1.empty[i], 1); }
+      for (int i = 0; i < K1P_NST; ++i) { mbar_init(&S1.full[i], 1 + 2 * K1P_PRODUCER_WARPS); mbar_init(&S1.empty[i], 1); mbar_init(&S1.a_empty[i], 1); }
       for (int i = 0; i < K1P_BB_SLOTS; ++i) { mbar_init(&S1.bb_full[i], 1); mbar_init(&S1.bb_empty[i], K1P_PRODUCER_WARPS); }
       for (int i = 0; i < 2; ++i) { mbar_init(&S1.acc_full[i], 1); mbar_init(&S1.acc_empty[i], 8); }
     } else {
