@@ -39,8 +39,12 @@ __device__ __forceinline__ void sincos_turns(float t, float &sn, float &cs) {
   cs = __cosf(x);
 }
 
-template <int MQ, bool PER_PLANE, bool FIELD>
+// STRIPS > 1 (static mode, short stacks): a plane is split over STRIPS CTAs by m_x strip; each regenerates the folded pupil
+// (cheap) and does its share of both products, so that a 16-plane stack occupies 64 SMs instead of 16.
+template <int MQ, bool PER_PLANE, bool FIELD, int STRIPS>
 __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const DevPlan P, float *__restrict__ I, float2 *__restrict__ field) {
+  constexpr int MXS = MQ / STRIPS;               // m_x columns of this CTA
+  const int mx_base = blockIdx.y * MXS;
   extern __shared__ __align__(16) uint8_t smem_raw[];
   SmallSmem<MQ, PER_PLANE> &S = *reinterpret_cast<SmallSmem<MQ, PER_PLANE> *>(smem_raw);
   const int tid = threadIdx.x;
@@ -103,8 +107,9 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
     }
   }
 
-  constexpr int PASS1 = MQ / 16;                 // stage-1 passes over m_x groups of 4 (4 groups per pass)
-  constexpr int PASS2 = (MQ / 2) * (MQ / 2) / 64;  // stage-2 passes over 2 x 2 pixel tiles (64 tiles per pass)
+  constexpr int PASS1 = MXS >= 16 ? MXS / 16 : 1;  // stage-1 passes over m_x groups of 4 (4 groups per pass)
+  constexpr int G1 = MXS >= 16 ? 4 : MXS / 4;      // m_x groups per pass (a strip of 8 columns keeps half of the threads busy here)
+  constexpr int PASS2 = (MQ / 2) * (MXS / 2) / 64; // stage-2 passes over 2 x 2 pixel tiles (64 tiles per pass)
   float inten[PASS2][2][4];
 #pragma unroll
   for (int p = 0; p < PASS2; ++p)
@@ -166,7 +171,9 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
       const int qy = tid >> 2;
 #pragma unroll
       for (int p = 0; p < PASS1; ++p) {
-        const int mx0 = ((tid & 3) + 4 * p) * 4;
+        if ((tid & 3) >= G1) break;
+        const int lx0 = ((tid & 3) + 4 * p) * 4;     // column inside the strip
+        const int mx0 = mx_base + lx0;
         float acc[8][4];
 #pragma unroll
         for (int j = 0; j < 8; ++j)
@@ -193,8 +200,8 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
         }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          *reinterpret_cast<float4 *>(&S.Ts[qy][(mx0 + i) * 4]) = make_float4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
-          *reinterpret_cast<float4 *>(&S.Ts[qy][MQ * 4 + (mx0 + i) * 4]) = make_float4(acc[4][i], acc[5][i], acc[6][i], acc[7][i]);
+          *reinterpret_cast<float4 *>(&S.Ts[qy][(lx0 + i) * 4]) = make_float4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
+          *reinterpret_cast<float4 *>(&S.Ts[qy][MXS * 4 + (lx0 + i) * 4]) = make_float4(acc[4][i], acc[5][i], acc[6][i], acc[7][i]);
         }
       }
     }
@@ -206,7 +213,7 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
 #pragma unroll
     for (int p = 0; p < PASS2; ++p) {
       const int tile = (tid >> 1) + 64 * p;
-      const int my0 = (tile / (MQ / 2)) * 2, mx0 = (tile % (MQ / 2)) * 2;
+      const int my0 = (tile / (MXS / 2)) * 2, lx0 = (tile % (MXS / 2)) * 2, mx0 = mx_base + lx0;
       float acc[8][2][2];
 #pragma unroll
       for (int j = 0; j < 8; ++j) acc[j][0][0] = acc[j][0][1] = acc[j][1][0] = acc[j][1][1] = 0.f;
@@ -215,10 +222,10 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
         const int qy = 2 * kk + kh;
         const float2 yc = *reinterpret_cast<const float2 *>(&S.Xc[qy][my0]);
         const float2 ys = *reinterpret_cast<const float2 *>(&S.Xs[qy][my0]);
-        const float4 t00 = *reinterpret_cast<const float4 *>(&S.Ts[qy][mx0 * 4]);            // chains 0-3, mx0
-        const float4 t01 = *reinterpret_cast<const float4 *>(&S.Ts[qy][mx0 * 4 + 4]);        // chains 0-3, mx0 + 1
-        const float4 t10 = *reinterpret_cast<const float4 *>(&S.Ts[qy][MQ * 4 + mx0 * 4]);   // chains 4-7
-        const float4 t11 = *reinterpret_cast<const float4 *>(&S.Ts[qy][MQ * 4 + mx0 * 4 + 4]);
+        const float4 t00 = *reinterpret_cast<const float4 *>(&S.Ts[qy][lx0 * 4]);            // chains 0-3, mx0
+        const float4 t01 = *reinterpret_cast<const float4 *>(&S.Ts[qy][lx0 * 4 + 4]);        // chains 0-3, mx0 + 1
+        const float4 t10 = *reinterpret_cast<const float4 *>(&S.Ts[qy][MXS * 4 + lx0 * 4]);   // chains 4-7
+        const float4 t11 = *reinterpret_cast<const float4 *>(&S.Ts[qy][MXS * 4 + lx0 * 4 + 4]);
         const float lo0[4] = {t00.x, t00.y, t00.z, t00.w}, lo1[4] = {t01.x, t01.y, t01.z, t01.w};
         const float hi0[4] = {t10.x, t10.y, t10.z, t10.w}, hi1[4] = {t11.x, t11.y, t11.z, t11.w};
 #pragma unroll
@@ -275,7 +282,7 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
 #pragma unroll
   for (int p = 0; p < PASS2; ++p) {
     const int tile = (tid >> 1) + 64 * p;
-    const int my = (tile / (MQ / 2)) * 2 + (tid & 1), mx0 = (tile % (MQ / 2)) * 2;
+    const int my = (tile / (MXS / 2)) * 2 + (tid & 1), mx0 = mx_base + (tile % (MXS / 2)) * 2;
 #pragma unroll
     for (int ix = 0; ix < 2; ++ix) {
       const int mx = mx0 + ix;
@@ -290,20 +297,22 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
   }
 }
 
-template <int MQ, bool PP, bool FIELD>
+template <int MQ, bool PP, bool FIELD, int STRIPS = 1>
 cudaError_t launch_one(const DevPlan &P, cudaStream_t st, float *intensity, float2 *field) {
-  k_small<MQ, PP, FIELD><<<P.Z, SM_THREADS, (int)sizeof(SmallSmem<MQ, PP>), st>>>(P, intensity, field);
+  k_small<MQ, PP, FIELD, STRIPS><<<dim3(P.Z, STRIPS), SM_THREADS, (int)sizeof(SmallSmem<MQ, PP>), st>>>(P, intensity, field);
   return cudaGetLastError();
 }
 
-template <int MQ, bool PP, bool FIELD>
+template <int MQ, bool PP, bool FIELD, int STRIPS = 1>
 cudaError_t set_attr() {
-  return cudaFuncSetAttribute(k_small<MQ, PP, FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem<MQ, PP>));
+  return cudaFuncSetAttribute(k_small<MQ, PP, FIELD, STRIPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem<MQ, PP>));
 }
 
 template <int MQ>
 cudaError_t launch_mq(const DevPlan &P, cudaStream_t st, float *intensity, float2 *field) {
   if (P.per_plane) return field ? launch_one<MQ, true, true>(P, st, intensity, field) : launch_one<MQ, true, false>(P, st, intensity, field);
+  if (MQ == 32 && !field && P.Z * 4 <= 148) return launch_one<32, false, false, 4>(P, st, intensity, field);   // short static stacks: m_x strips
+  if (MQ == 32 && !field && P.Z * 2 <= 148) return launch_one<32, false, false, 2>(P, st, intensity, field);
   return field ? launch_one<MQ, false, true>(P, st, intensity, field) : launch_one<MQ, false, false>(P, st, intensity, field);
 }
 
@@ -318,7 +327,8 @@ cudaError_t small_setup() {
   if ((e = set_attr<16, false, false>()) != cudaSuccess || (e = set_attr<16, false, true>()) != cudaSuccess ||
       (e = set_attr<16, true, false>()) != cudaSuccess || (e = set_attr<16, true, true>()) != cudaSuccess ||
       (e = set_attr<32, false, false>()) != cudaSuccess || (e = set_attr<32, false, true>()) != cudaSuccess ||
-      (e = set_attr<32, true, false>()) != cudaSuccess || (e = set_attr<32, true, true>()) != cudaSuccess)
+      (e = set_attr<32, true, false>()) != cudaSuccess || (e = set_attr<32, true, true>()) != cudaSuccess ||
+      (e = set_attr<32, false, false, 2>()) != cudaSuccess || (e = set_attr<32, false, false, 4>()) != cudaSuccess)
     return e;
   return cudaSuccess;
 }
