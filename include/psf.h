@@ -193,10 +193,14 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_K1P_ASPLIT    : 1 (default) = in the stage-1 pair kernel the TMA-written table half of a stage buffer has its own barrier and
  *                            is released right behind its own stage (only the producer-written half needs the deferred release);
  *                            0 = one barrier for both halves (round 1);
+ *   PSF_TUNE_FUSED_WINDOW  : 1 = the fused launch carries a persisting L2 access-policy window over its ring scratch (the library then
+ *                            raises the device's cudaLimitPersistingL2CacheSize to the ring size); 0 (default) = none - measured, the
+ *                            window doubles the DRAM writes and gains no time (profiles/r2_fused_cfg5.md);
  *   PSF_TUNE_GRAD_TENSOR   : 1 (default) = psf_gradients runs its two transforms on the tensor cores where the plan is on the 3xFP16
  *                            path in static mode; 0 = the fp32 FFMA route of round 1. */
 enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
-       PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7, PSF_TUNE_K1P_ASPLIT = 8 };
+       PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7, PSF_TUNE_K1P_ASPLIT = 8,
+       PSF_TUNE_FUSED_WINDOW = 9 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

@@ -521,6 +521,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_GRAD_TENSOR) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_GRAD_TENSOR: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_grad_tensor = (int)value;
+    } else if (knob == PSF_TUNE_FUSED_WINDOW) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_FUSED_WINDOW: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_fused_window = (int)value;
     } else if (knob == PSF_TUNE_K1P_ASPLIT) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_ASPLIT: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_asplit = (int)value;

@@ -93,6 +93,7 @@ struct psf_plan {
   // psf_plan_tune knobs (tests and A/B runs; defaults = the library's own choice)
   int tune_pair_mask = 3;        // ANDed with the plan's choice: bit 0 = stage 1 on CTA pairs, bit 1 = stage 2
   int tune_scratch_mb = 0;       // > 0: budget of the tensor path's T^T scratch in MB (several launch pairs per stack)
+  int tune_fused_window = 0;     // 1: the fused launch carries a persisting L2 access-policy window over its ring (measured: no gain, more DRAM writes)
   int tune_fused = 1;            // 1: both stages in one launch (k12_fused) where eligible; 0: always two launches
   int tune_k1p_handoff = 0;      // k1_pair: 0 plain remote arrive, 1 .release.cluster arrive per producer warp of the non-leader CTA
   int tune_k1p_asplit = 1;       // k1_pair: 1 = the TMA-written table half of a stage buffer is released right behind its own stage
