@@ -237,11 +237,13 @@ def e2e_workload(torch, plan, case, device, steps, warmup):
     out = torch.empty((case.n_planes, case.out_m, case.out_m), dtype=torch.float32, device=dev)
     host = torch.empty(out.shape, dtype=torch.float32, pin_memory=True)
     h2d = 0
-    times = []
+    times, refresh = [], []
     for i in range(warmup + steps):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         plan.set_zernike(case.zernike, case.noll_first)
+        if i >= warmup:
+            refresh.append(time.perf_counter() - t0)
         h2d = plan.last_upload_bytes
         if case.shifts_um is not None:
             plan.set_shifts(case.shifts_um)
@@ -278,7 +280,7 @@ def e2e_workload(torch, plan, case, device, steps, warmup):
     torch.cuda.synchronize(dev)
     piped = (time.perf_counter() - t0) / steps
     return {"s_per_step": statistics.mean(times), "s_per_step_streamed": piped, "h2d": int(h2d), "d2h": int(out.numel() * 4),
-            "checksum": float(host.double().sum())}
+            "set_zernike_ms": 1e3 * statistics.median(refresh), "checksum": float(host.double().sum())}
 
 
 def oracle_sample(case, budget_planes):
@@ -413,10 +415,21 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                     "streamed_value": voxels / world / e2e["s_per_step_streamed"] * world,
-                    "note": "value: each step serial (host table refresh + upload, kernels, device->host copy); "
+                    "set_zernike_ms": e2e["set_zernike_ms"],
+                    "note": "value: each step serial (psf_set_zernike = coefficient upload + table refresh, on the device for "
+                            "3xFP16 pair plans; kernels; device->host copy); "
                             "streamed_value: same steps with the copy of step i overlapping step i+1 (two pinned buffers)"},
             "gpu_launches": int(res["launches"]) * args.steps,
             "roofline": roofline}
+    if path == "tc3xf16" and case.zernike is not None and case.shifts_um is None:
+        # A/B of the table refresh: the same call with the device-side refresh switched off (host fp64 tables + upload)
+        res["plan"].tune(psf.TUNE_DEVICE_REFRESH, 0)
+        ts = []
+        for _ in range(6):
+            t0 = time.perf_counter()
+            res["plan"].set_zernike(case.zernike, case.noll_first)
+            ts.append(time.perf_counter() - t0)
+        line["e2e"]["set_zernike_host_path_ms"] = 1e3 * statistics.median(ts[1:])
     res["plan"].destroy()
 
     if rank == 0 and world == 1:

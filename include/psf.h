@@ -182,9 +182,9 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_TC_SCRATCH_MB : budget in MB of the stage-1 -> stage-2 scratch (default 0 = 4096): a smaller value splits a
  *                            stack into several launch pairs;
  *   PSF_TUNE_K1P_HANDOFF   : stage-1 pair kernel, how the non-leader CTA's producer warps signal the leader's barrier:
- *                            0 plain remote arrive, 1 cluster-scope release per warp, 2 relay threads (default);
- *   PSF_TUNE_K1P_DEFER     : 1 (default) = producer-written operand slots are released one full stage late; 0 = at once
- *                            (the A/B setting of profiles/r2*_race_k1_pair.md; unsafe);
+ *                            0 (default) plain remote arrive, 1 cluster-scope release per warp;
+ *   PSF_TUNE_K1P_DEFER     : producer-written operand slots are released that many K-steps (three UMMAs each) after the stage's
+ *                            last UMMA: 1 (default), 0 = at once (the A/B setting of profiles/r2_race_k1_pair.md; unsafe), up to 4;
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
  *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;
@@ -197,10 +197,14 @@ int psf_grad_terms(const psf_plan *plan);
  *                            raises the device's cudaLimitPersistingL2CacheSize to the ring size); 0 (default) = none - measured, the
  *                            window doubles the DRAM writes and gains no time (profiles/r2_fused_cfg5.md);
  *   PSF_TUNE_GRAD_TENSOR   : 1 (default) = psf_gradients runs its two transforms on the tensor cores where the plan is on the 3xFP16
- *                            path in static mode; 0 = the fp32 FFMA route of round 1. */
+ *                            path in static mode; 0 = the fp32 FFMA route of round 1;
+ *   PSF_TUNE_DEVICE_REFRESH: 1 (default) = on a plan that runs the 3xFP16 pair kernels, psf_set_zernike (shared coefficients) and
+ *                            psf_set_phase_mask recompute the phase, the fold and the operand scales on the device from resident
+ *                            fp64 copies of the static pupil and the Zernike basis (same arithmetic, same order as the host path);
+ *                            0 = the host path (fp64 on the host cores + upload of the folded tables). */
 enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
        PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7, PSF_TUNE_K1P_ASPLIT = 8,
-       PSF_TUNE_FUSED_WINDOW = 9 };
+       PSF_TUNE_FUSED_WINDOW = 9, PSF_TUNE_DEVICE_REFRESH = 10 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

@@ -91,6 +91,7 @@ psf_status upload_static(psf_plan *p) {
   std::vector<cplx> &base_z = p->h_base;
   apply_shared_zernike(hp, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis,
                        p->phase_mask.empty() ? nullptr : p->phase_mask.data(), base_z);
+  p->host_base_stale = false;
   const int N = d.pupil_n, n = (N + 1) / 2, C = hp.C;
   const size_t NN = (size_t)N * N, nn = (size_t)n * n;
   DevPlan &P = p->dp;
@@ -250,6 +251,14 @@ psf_status alloc_scratch(psf_plan *p) {
   return PSF_OK;
 }
 
+// cudaMemcpy from pageable host memory returns once the data is staged; the DMA to the device may still be in flight, ordered
+// only against the legacy stream and blocking streams.  The caller's stream may be non-blocking, so every call that uploads
+// tables ends with this fence.
+psf_status uploads_fence(psf_plan *p) {
+  if (cudaStreamSynchronize(cudaStreamLegacy) != cudaSuccess) { p->err = "cudaStreamSynchronize after the table uploads failed"; return PSF_ERR_CUDA; }
+  return PSF_OK;
+}
+
 psf_status refresh(psf_plan *p) {
   if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
   if (tc_fused_aborted(p)) {
@@ -258,9 +267,33 @@ psf_status refresh(psf_plan *p) {
   }
   p->upload_bytes = 0;
   ++p->table_version;
+  ++p->static_version;
   psf_status s = upload_static(p);
   if (s != PSF_OK) return s;
-  return alloc_scratch(p);     // C is fixed per plan, but keep the scratch consistent with it
+  if ((s = alloc_scratch(p)) != PSF_OK) return s;     // C is fixed per plan, but keep the scratch consistent with it
+  return uploads_fence(p);
+}
+
+// A change of the shared pupil phase only (shared Zernike coefficients, phase mask) on a plan whose tables are already in place:
+// plans on the 3xFP16 pair kernels redo the phase, the fold and the operand scales on the device (tc_refresh_device, ~0.1 ms
+// instead of 2.5 ms of host work and an 11 MB upload at config 5); every other plan takes the host path.
+psf_status refresh_phase(psf_plan *p) {
+  if (!p->tune_dev_refresh || !tc_refresh_device_ok(p) || p->desc.precision == PSF_PREC_CZT_FFT) return refresh(p);
+  if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+  if (tc_fused_aborted(p)) {
+    p->err = "an earlier psf_compute of this plan (fused launch) gave up waiting for a stage-1 / stage-2 dependency: its stack is invalid";
+    return PSF_ERR_CUDA;
+  }
+  const int Kneed = (int)p->zern_shared.size();
+  if (Kneed > 0 && (p->zb_first != p->noll_first || p->zb_K != Kneed)) {
+    build_zernike_basis(p->hp0, p->noll_first, Kneed, p->zbasis);
+    p->zb_first = p->noll_first;
+    p->zb_K = Kneed;
+  }
+  p->upload_bytes = 0;
+  ++p->table_version;
+  p->host_base_stale = true;
+  return tc_refresh_device(p);
 }
 
 void free_all(psf_plan *p) {
@@ -281,6 +314,14 @@ void free_all(psf_plan *p) {
 }  // namespace
 
 namespace psf {
+const std::vector<cplx> &host_base(psf_plan *p) {
+  if (p->host_base_stale) {
+    apply_shared_zernike(p->hp0, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis,
+                         p->phase_mask.empty() ? nullptr : p->phase_mask.data(), p->h_base);
+    p->host_base_stale = false;      // h_bfold stays behind: only upload_static reads it, right after rebuilding it
+  }
+  return p->h_base;
+}
 psf_status plan_set_materialised(psf_plan *p, double qmax, double rmax) {
   p->mat_mode = 1;
   p->mat_qmax = qmax;
@@ -339,7 +380,7 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out) {
   build_host_pupil(p->desc, nullptr, 1, 0, p->hp0);
   const bool czt = p->desc.precision == PSF_PREC_CZT_FFT;
   if (!czt) build_dft_phase(p->desc, p->phi);
-  if ((s = refresh(p)) != PSF_OK || (!czt && (s = upload_dft(p)) != PSF_OK)) {
+  if ((s = refresh(p)) != PSF_OK || (!czt && (s = upload_dft(p)) != PSF_OK) || (s = uploads_fence(p)) != PSF_OK) {
     g_create_err = p->err;
     free_all(p);
     delete p;
@@ -375,8 +416,9 @@ psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int
     if (per_plane) { p->zern_rows.assign(coeffs, coeffs + cnt); p->K_rows = n_coeffs; }
     else p->zern_shared.assign(coeffs, coeffs + n_coeffs);
   }
+  const int was_per_plane = p->dp.per_plane;
   p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;
-  return refresh(p);
+  return (was_per_plane || p->dp.per_plane) ? refresh(p) : refresh_phase(p);
   });
 }
 
@@ -391,7 +433,8 @@ psf_status psf_set_phase_mask(psf_plan *p, const float *w0_rad) {
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
   p->phase_mask.clear();
   if (w0_rad) p->phase_mask.assign(w0_rad, w0_rad + NN);
-  return refresh(p);
+  ++p->phase_mask_version;
+  return refresh_phase(p);
   });
 }
 
@@ -455,7 +498,8 @@ psf_status psf_spherical_prepare(psf_plan *p, int n_nodes) {
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
   if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
-  return bessel_setup(p, n_nodes);
+  psf_status sb = bessel_setup(p, n_nodes);
+  return sb != PSF_OK ? sb : uploads_fence(p);
   });
 }
 
@@ -487,7 +531,9 @@ psf_status psf_gradients(psf_plan *p, void *cuda_stream, const float *dL_dI, dou
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
   if (grad_needs_setup(p) && wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+  const bool setup = grad_needs_setup(p);
   psf_status s = grad_setup(p);               // first call, or the tables changed: (re)build the adjoint's copies
+  if (s == PSF_OK && setup) s = uploads_fence(p);
   if (s != PSF_OK) return s;
   if (dL_dc && grad_terms(p) == 0) { p->err = "dL_dc asked for, but no Zernike terms are set"; return PSF_ERR_STATE; }
   e = launch_grad(p, (cudaStream_t)cuda_stream, dL_dI, dL_dz, dL_dc);
@@ -530,6 +576,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_SMLM) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_SMLM: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_smlm = (int)value;
+    } else if (knob == PSF_TUNE_DEVICE_REFRESH) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_DEVICE_REFRESH: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_dev_refresh = (int)value;
     } else if (knob == PSF_TUNE_K1P_HANDOFF) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_handoff = (int)value;

@@ -39,6 +39,9 @@ struct GradState {
   void *d_axt = nullptr;      // float2 [N][M]      its transpose
   void *d_Q = nullptr, *d_T = nullptr, *d_E = nullptr, *d_B = nullptr;   // per-pass scratch
   long long version = -1;     // table version these copies were made from
+  long long static_version = -1;   // the plan's static version at the last full setup
+  int zb_first = 0;           // first Noll index of d_zb
+  const float2 *base5 = nullptr;   // what g_dphi reads: d_base5, or the tensor path's own device copy after a device-side refresh
   // tensor-core route
   bool tensor = false;
   psf_plan *planB = nullptr;  // the back-projection plan (sizes swapped), owned
@@ -337,6 +340,32 @@ psf_status grad_setup(psf_plan *p) {
   const int N = D.N, M = D.M;
   const size_t NN = (size_t)N * N, MM = (size_t)M * M, MN = (size_t)M * N;
   if (p->grad && p->grad->version == p->table_version) return PSF_OK;
+  if (p->grad && p->grad->tensor && p->grad->static_version == p->static_version) {
+    // only the shared pupil phase changed since the last full setup (device-side refresh): the back-projection plan, the
+    // scratch and every static table stand; what moves is the unfolded pupil and, if the term list changed, the basis
+    GradState *g = p->grad;
+    const int K = (int)p->zern_shared.size();
+    if (K != g->K || (K > 0 && p->zb_first != g->zb_first)) {
+      std::vector<float> zb((size_t)K * NN);
+      for (size_t i = 0; i < zb.size(); ++i) zb[i] = (float)p->zbasis[i];
+      if (g->d_zb) { cudaFree(g->d_zb); g->d_zb = nullptr; }
+      if (K > 0 && (cudaMalloc(&g->d_zb, zb.size() * sizeof(float)) != cudaSuccess ||
+                    cudaMemcpy(g->d_zb, zb.data(), zb.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)) {
+        p->err = "gradients: basis upload failed";
+        grad_free(p);
+        return PSF_ERR_ALLOC;
+      }
+      g->K = K;
+      g->zb_first = p->zb_first;
+    }
+    g->base5 = tc_device_pupil(p);
+    if (!g->base5) {                       // cannot happen while static_version stands, but stay correct if it does
+      grad_free(p);
+      return grad_setup(p);
+    }
+    g->version = p->table_version;
+    return PSF_OK;
+  }
   grad_free(p);
   GradState *g = new GradState();
   p->grad = g;
@@ -349,7 +378,7 @@ psf_status grad_setup(psf_plan *p) {
   for (int c = 0; c < g->Cg; ++c) g->w[c] = unpol ? 0.5f : 1.0f;
   std::vector<float2> base((size_t)g->Cg * NN);
   for (int c = 0; c < g->Cg; ++c) {
-    const cplx *src = p->h_base.data() + (size_t)(unpol ? pick[c] : c) * NN;
+    const cplx *src = host_base(p).data() + (size_t)(unpol ? pick[c] : c) * NN;
     for (size_t i = 0; i < NN; ++i) base[(size_t)c * NN + i] = make_float2((float)src[i].real(), (float)src[i].imag());
   }
   std::vector<float2> kt(NN);
@@ -360,6 +389,8 @@ psf_status grad_setup(psf_plan *p) {
     kt[i] = make_float2(hi, (float)(t - (double)hi));
   }
   g->K = p->zern_shared.empty() ? p->K_rows : (int)p->zern_shared.size();
+  g->zb_first = p->zb_first;
+  g->static_version = p->static_version;
   std::vector<float> zb((size_t)g->K * NN);
   for (size_t i = 0; i < zb.size(); ++i) zb[i] = (float)p->zbasis[i];
   std::vector<float2> ax(MN), axt(MN);
@@ -388,7 +419,7 @@ psf_status grad_setup(psf_plan *p) {
     std::vector<float2> base5((size_t)C5 * NN);
     for (int c = 0; c < C5; ++c) {
       double l1 = 0.0;
-      const cplx *src = p->h_base.data() + (size_t)c * NN;
+      const cplx *src = host_base(p).data() + (size_t)c * NN;
       for (size_t i = 0; i < NN; ++i) { l1 += std::abs(src[i]); base5[(size_t)c * NN + i] = make_float2((float)src[i].real(), (float)src[i].imag()); }
       hmax = std::max(hmax, hp.weight[c] * l1);                 // |H_c| = w_c |G / max G| |E_c| <= w_c sum_p |base_c[p]|
     }
@@ -412,6 +443,7 @@ psf_status grad_setup(psf_plan *p) {
             cudaMalloc(&g->d_dummyI, big * sizeof(float)) == cudaSuccess && cudaMalloc(&g->d_gmax, sizeof(unsigned)) == cudaSuccess) {
           cudaFuncSetAttribute(g_sred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((SR_ZT + 65) * SR_PITCH * sizeof(float)));
           g->tensor = true;
+          g->base5 = (const float2 *)g->d_base5;
           g->planB = pb;
           g->C5 = C5;
           for (int c = 0; c < C5; ++c) g->w5[c] = (float)hp.weight[c];
@@ -464,7 +496,7 @@ cudaError_t launch_grad(const psf_plan *p, cudaStream_t st, const float *dL_dI, 
     const int Kt = dL_dc ? g->K : 0;
     // sensitivity S (fp32, in the dummy-intensity buffer, free by now), then the skinny product against kappa and the basis
     float *S = (float *)g->d_dummyI;
-    g_dphi<<<dim3((unsigned)((NN + 255) / 256), D.Z), 256, 0, st>>>((const float2 *)g->d_base5, (const float2 *)g->d_fieldB, (const float2 *)g->d_kt,
+    g_dphi<<<dim3((unsigned)((NN + 255) / 256), D.Z), 256, 0, st>>>(g->base5, (const float2 *)g->d_fieldB, (const float2 *)g->d_kt,
                                                                    D.planes, (const unsigned *)g->d_gmax, S, g->C5, D.Z, NN);
     const size_t sr_bytes = (size_t)(SR_ZT + Kt + 1) * SR_PITCH * sizeof(float);
     g_sred<<<dim3((unsigned)((NN + SR_CHUNK - 1) / SR_CHUNK), (D.Z + SR_ZT - 1) / SR_ZT), 256, sr_bytes, st>>>(

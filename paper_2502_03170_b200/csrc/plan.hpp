@@ -101,6 +101,10 @@ struct psf_plan {
   cudaEvent_t done_ev = nullptr; // recorded on the caller's stream after the last launch of every compute call: table
                                  // refreshes wait for it before they overwrite tables a launch in flight may still read
   long long table_version = 0;   // bumped by every table refresh (psf_set_*): derived copies check it
+  long long static_version = 0;  // bumped by every full (host) refresh: a device-side refresh of the shared phase leaves it alone
+  long long phase_mask_version = 0;   // bumped by psf_set_phase_mask (device copies of the mask check it)
+  bool host_base_stale = false;  // the last refresh ran on the device (tc_refresh_device): h_base / h_bfold are behind; see host_base()
+  int tune_dev_refresh = 1;      // 1: shared-phase changes of a 3xFP16 pair plan are refreshed on the device; 0: always the host path
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)
 };
 
@@ -139,6 +143,10 @@ cudaError_t launch_tc_mat(const psf_plan *p, cudaStream_t st, float *intensity, 
 float tc_pupil_scale(const psf_plan *p);
 int tc_n_pad(const psf_plan *p);
 bool tc_pair_stage1(const psf_plan *p);
+bool tc_refresh_device_ok(const psf_plan *p);
+psf_status tc_refresh_device(psf_plan *p);
+const float2 *tc_device_pupil(const psf_plan *p);
+const std::vector<cplx> &host_base(psf_plan *p);   // h_base, recomputed first if a device-side refresh left it behind
 // api.cu: turns a plan into the carrier of a materialised-pupil transform (used by the adjoint for its back-projection plan)
 psf_status plan_set_materialised(psf_plan *p, double qmax, double rmax);
 // kernels_bessel.cu

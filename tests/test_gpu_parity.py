@@ -641,3 +641,63 @@ def test_adjoint_on_the_tensor_cores_matches_oracle(psf, seed, N, M, Z, pol, kw)
     assert plan.grad_path == "adjoint_ffma"
     assert np.abs(dz3.cpu().numpy()[sel] - dz_ref).max() <= GRAD_TOL * np.abs(dz_ref).max()
     plan.destroy()
+
+
+@pytest.mark.parametrize("seed,N,M,pol", [(301, 300, 400, W.POL_UNPOLARIZED),    # pair kernels, five pupils, n_pad = 192
+                                          (302, 255, 256, W.POL_CIRC_L),        # odd N (self-mirror row and column), group mode
+                                          (303, 128, 128, W.POL_X)])            # group mode + k2_res
+def test_device_side_refresh_of_the_shared_phase(psf, seed, N, M, pol):
+    """psf_set_zernike (shared) / psf_set_phase_mask on a 3xFP16 pair plan recompute the phase (Eq. 18), the fold and
+    the operand scales on the device (tc_refresh_device).  Every state must match the oracle, and the host refresh of the same
+    plan (PSF_TUNE_DEVICE_REFRESH = 0) to the last bits: same fp64 arithmetic in the same order."""
+    import torch
+    rng = np.random.default_rng(seed)
+    base = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=3, per_plane=False, shifts=False, pol=pol)
+    plan = psf.plan_from_case(base, precision="3xf16")
+    assert plan.path == "tc3xf16" and plan.kernel_names[0].startswith("k1_pair")
+    vortex = (0.7 * _vortex(N)).astype(np.float32)
+    states = [
+        replace(base, zernike=(0.3 * rng.standard_normal(9)).astype(np.float32), noll_first=4),       # same K or new K: basis upload
+        replace(base, zernike=(0.2 * rng.standard_normal(15)).astype(np.float32), noll_first=2),      # K and first index change
+        replace(base, zernike=(0.2 * rng.standard_normal(15)).astype(np.float32), noll_first=2, phase_mask=vortex),
+        replace(base, zernike=None, phase_mask=vortex),                                               # mask only
+        replace(base, zernike=None, phase_mask=None),                                                 # everything cleared
+        replace(base, zernike=np.array([2.5, -1.5, 0.8], np.float32), noll_first=4),                  # large phases: scales move
+        replace(base, zernike=np.array([-1.0, 0.5, 2.0], np.float32), noll_first=4),                  # same terms, new values
+    ]
+
+    def apply(case):
+        plan.set_phase_mask(case.phase_mask)
+        plan.set_zernike(case.zernike, case.noll_first)
+
+    for k, case in enumerate(states):
+        apply(case)
+        if k == 6:                                            # same K, same basis: the coefficients are all that is uploaded
+            assert plan.last_upload_bytes < 4096, plan.last_upload_bytes
+        a = plan.compute().cpu().numpy()
+        assert plane_errors(a.astype(np.float64), O.stack_T2(case)).max() <= TOL, (k, "device refresh")
+        plan.tune(psf.TUNE_DEVICE_REFRESH, 0)                 # rebuilds everything on the host
+        assert plan.last_upload_bytes > 100000
+        b = plan.compute().cpu().numpy()
+        plan.tune(psf.TUNE_DEVICE_REFRESH, 1)
+        torch.cuda.synchronize()
+        # device libm against glibc in fp64: the rounded fp32 tables may differ in a last bit here and there
+        assert np.abs(a - b).max() <= 2e-6 * b.max(), (k, np.abs(a - b).max() / b.max())
+    # the adjoint across device-side refreshes: the first call builds its state from the host copy of the pupil (brought up to
+    # date first), later calls only re-point at the refreshed device pupil (and re-upload the basis when the term list changes)
+    G = torch.from_numpy(rng.standard_normal((3, M, M)).astype(np.float32)).cuda()
+    got = []
+    for case in (states[0], states[1], states[2], states[5], states[6]):
+        apply(case)
+        dz, dc = plan.gradients(G)
+        assert plan.grad_path == "adjoint_tc3xf16"
+        got.append((dz.cpu().numpy(), dc.cpu().numpy()))
+    plan.tune(psf.TUNE_DEVICE_REFRESH, 0)
+    for (dz, dc), case in zip(got, (states[0], states[1], states[2], states[5], states[6])):
+        apply(case)
+        dz0, dc0 = plan.gradients(G)
+        dz0, dc0 = dz0.cpu().numpy(), dc0.cpu().numpy()
+        assert dc.shape == dc0.shape == (3, len(case.zernike))
+        assert np.allclose(dz, dz0, rtol=0, atol=1e-5 * np.abs(dz0).max())
+        assert np.allclose(dc, dc0, rtol=0, atol=1e-5 * np.abs(dc0).max())
+    plan.destroy()
