@@ -115,6 +115,7 @@ def roofline_record(case, res, ms_per_step, peaks, traffic_rows):
                 "kernel_ms_per_launch": dur_ms, "launches_per_step": launches_dom,
                 "algorithmic_tflops": flop_dom / launches_dom / (dur_ms * 1e-3) / 1e12, "peak_source": peak_note,
                 "stage_ms_per_step": [float(stage_ms[0]), float(stage_ms[1])],
+                "kernel_times_from": res.get("profile_pass"),
                 # compulsory HBM traffic = the intensity stack: reported for every workload, the binding
                 # bound only where the flop are few (the small-M batched regime)
                 "hbm_gbs": out_bytes / (ms_per_step * 1e-3) / 1e9,
@@ -188,7 +189,13 @@ def time_workload(torch, psf, case, device, steps, warmup, flush, profile=True):
     dev = torch.device("cuda", device)
     out = torch.empty((case.n_planes, case.out_m, case.out_m), dtype=torch.float32, device=dev)
     stream = torch.cuda.current_stream(dev)
-    if profile:
+    # Per-kernel durations come from psf_profile_enable (an event record behind every launch).  On a one-kernel path that is
+    # free, so the timed steps carry it; on a two-kernel path the record sits between the kernels (and switches the
+    # programmatic dependent launch of stage 2 off), so the steps are timed without it and a second pass of the same
+    # steps, profiled, gives the split.
+    multi = plan.launches_per_compute > 1
+    inline = profile and not multi
+    if inline:
         plan.profile_enable(True)
     for _ in range(warmup):
         plan.compute(out)
@@ -201,16 +208,32 @@ def time_workload(torch, psf, case, device, steps, warmup, flush, profile=True):
         ev[i][0].record(stream)
         plan.compute(out)
         ev[i][1].record(stream)
-        if profile:
+        if inline:
             torch.cuda.synchronize(dev)
             ms, ln = plan.profile_read()
             stage_ms += np.array(ms)
             stage_launches += np.array(ln)
     torch.cuda.synchronize(dev)
     step_ms = [a.elapsed_time(b) for a, b in ev]
+    psteps = steps
+    if profile and multi:
+        psteps = min(steps, 10)
+        plan.profile_enable(True)
+        plan.compute(out)
+        for i in range(psteps):
+            flush.fill_(float(i % 251))
+            plan.compute(out)
+            torch.cuda.synchronize(dev)
+            ms, ln = plan.profile_read()
+            stage_ms += np.array(ms)
+            stage_launches += np.array(ln)
+        plan.profile_enable(False)
+    steps = psteps
     res = {"plan": plan, "out": out, "step_ms": step_ms, "stage_ms": stage_ms / max(steps, 1),
            "stage_launches": stage_launches // max(steps, 1), "path": plan.path,
-           "launches": plan.launches_per_compute, "kernels": plan.kernel_names}
+           "launches": plan.launches_per_compute, "kernels": plan.kernel_names,
+           "profile_pass": "none" if not profile else ("separate pass of %d profiled steps behind the timed steps" % psteps if multi
+                                                        else "inside the timed steps")}
     return res
 
 
@@ -507,6 +530,23 @@ def run_ours(args):
                                "note": "forward field + back-projection (the same tensor kernels on a plan with the grids swapped) + "
                                        "weight/fold and reduction kernels; fp32_equivalent_tflops counts the unfolded complex products",
                                "zernike_terms": int(K)}
+                # one iteration of a fit: new shared coefficients in, stack and gradients out (wall clock, one sync at the end),
+                # with the table refresh on the device (default) and on the host (PSF_TUNE_DEVICE_REFRESH = 0)
+                out = torch.empty((cs.n_planes, cs.out_m, cs.out_m), dtype=torch.float32, device=dev)
+                rng = np.random.default_rng(7)
+                for mode, key in ((1, "fit_iteration_ms"), (0, "fit_iteration_host_refresh_ms")):
+                    plan.tune(psf.TUNE_DEVICE_REFRESH, mode)
+                    its = []
+                    for i in range(2 + 5):
+                        coef = (cs.zernike + 0.01 * rng.standard_normal(K)).astype(np.float32)
+                        torch.cuda.synchronize(dev)
+                        t0 = time.perf_counter()
+                        plan.set_zernike(coef, cs.noll_first)
+                        plan.compute(out)
+                        plan.gradients(G, K)
+                        torch.cuda.synchronize(dev)
+                        its.append(time.perf_counter() - t0)
+                    sweep[name][key] = 1e3 * statistics.median(its[2:])
                 plan.destroy()
             line["workloads"] = sweep
     if rank == 0:

@@ -201,10 +201,14 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_DEVICE_REFRESH: 1 (default) = on a plan that runs the 3xFP16 pair kernels, psf_set_zernike (shared coefficients) and
  *                            psf_set_phase_mask recompute the phase, the fold and the operand scales on the device from resident
  *                            fp64 copies of the static pupil and the Zernike basis (same arithmetic, same order as the host path);
- *                            0 = the host path (fp64 on the host cores + upload of the folded tables). */
+ *                            0 = the host path (fp64 on the host cores + upload of the folded tables);
+ *   PSF_TUNE_PDL           : 1 (default) = on the two-kernel tensor path the stage-2 kernel is a programmatic dependent launch of
+ *                            stage 1: its CTAs take the SMs stage 1 leaves, run their prologue (barriers, TMEM, table loads) and
+ *                            wait (griddepcontrol.wait) for the stage-1 grid to complete before the first read of its output;
+ *                            0 = plain stream order. */
 enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
        PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7, PSF_TUNE_K1P_ASPLIT = 8,
-       PSF_TUNE_FUSED_WINDOW = 9, PSF_TUNE_DEVICE_REFRESH = 10 };
+       PSF_TUNE_FUSED_WINDOW = 9, PSF_TUNE_DEVICE_REFRESH = 10, PSF_TUNE_PDL = 11 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

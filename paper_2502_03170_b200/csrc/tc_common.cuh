@@ -48,6 +48,13 @@ __device__ __forceinline__ void tcgen05_fence_before() { asm volatile("tcgen05.f
 __device__ __forceinline__ void tcgen05_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
 // ---- TMA -----------------------------------------------------------------------------------------------------------
+// Programmatic dependent launch: a stage-2 kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization becomes
+// resident (on SMs the stage-1 grid has left) once every stage-1 CTA has issued pdl_trigger(), runs its prologue (barriers,
+// TMEM, table loads) and then blocks in pdl_wait() until the stage-1 grid has completed and its stores are visible.  Both are
+// no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ void prefetch_tmap(const void *tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)tmap) : "memory");
 }

@@ -219,6 +219,7 @@ __device__ __forceinline__ void k2p_feed(uint8_t *smem, K2PShared &S, uint32_t t
       int st = 0, ph = 0;
       uint32_t full_leader[K2P_NST];
       for (int i = 0; i < K2P_NST; ++i) full_leader[i] = mapa(smem_u32(&full[i]), 0);
+      if (!FUSED) tc::pdl_wait();                          // two-kernel path: T^T is the stage-1 grid's output
       for (int t = cid; t < ntiles; t += ncl) {
         const int typ = t % tiles_yp;
         int r = t / tiles_yp;
@@ -813,6 +814,7 @@ k1_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
   __shared__ K1PShared S;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
+  if (threadIdx.x == 0) tc::pdl_trigger();                 // the stage-2 grid may take the SMs this grid leaves (it waits for our completion)
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < K1P_NST; ++i) {

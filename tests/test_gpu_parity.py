@@ -701,3 +701,26 @@ def test_device_side_refresh_of_the_shared_phase(psf, seed, N, M, pol):
         assert np.allclose(dz, dz0, rtol=0, atol=1e-5 * np.abs(dz0).max())
         assert np.allclose(dc, dc0, rtol=0, atol=1e-5 * np.abs(dc0).max())
     plan.destroy()
+
+
+@pytest.mark.parametrize("seed,N,M,pol,fused", [(311, 128, 128, W.POL_CIRC_L, 1),      # k1_pair<gm> -> k2_res
+                                                (312, 300, 400, W.POL_UNPOLARIZED, 0),  # k1_pair -> k2_pair
+                                                (313, 200, 200, W.POL_X, 1)])           # k1_pair<gm> -> k2_res, ragged
+def test_programmatic_dependent_launch_of_stage_two_changes_no_bit(psf, seed, N, M, pol, fused):
+    """On the two-kernel tensor path the stage-2 kernel is a programmatic dependent launch of stage 1 (its prologue overlaps the
+    stage-1 tail; griddepcontrol.wait orders its first read of T^T behind the completed stage-1 grid).  Same bits as the
+    plain stream order, call after call, and within the bar of the oracle."""
+    import torch
+    case = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=5, per_plane=False, shifts=False, pol=pol)
+    plan = psf.plan_from_case(case, precision="3xf16")
+    plan.tune(psf.TUNE_TC_FUSED, fused)
+    assert len(plan.kernel_names) == 2
+    plan.tune(psf.TUNE_PDL, 0)
+    ref = plan.compute().clone()
+    assert plane_errors(ref.cpu().numpy().astype(np.float64), O.stack_T2(case)).max() <= TOL
+    plan.tune(psf.TUNE_PDL, 1)
+    out = torch.empty_like(ref)
+    for _ in range(200):                       # back to back: stage 1 of call i + 1 follows stage 2 of call i in plain stream order
+        plan.compute(out)
+    assert torch.equal(out, ref)
+    plan.destroy()
