@@ -474,6 +474,18 @@ def run_ours(args):
                                "path": r["path"], "kernels": r["kernels"], "launches": r["launches"],
                                "roofline": roofline_record(cs, r, ms, peaks, traffic_rows),
                                "cpu_baseline": cpu_baseline(cs, c, ORACLE_PLANES_SWEEP)}
+                if cs.shifts_um is not None and cs.zernike is not None and cs.zernike.ndim == 2:
+                    # emitter batch: what new per-emitter coefficients and positions cost before the next psf_compute
+                    tz, tsft = [], []
+                    for _ in range(6):
+                        t0 = time.perf_counter()
+                        r["plan"].set_zernike(cs.zernike, cs.noll_first)
+                        t1 = time.perf_counter()
+                        r["plan"].set_shifts(cs.shifts_um)
+                        tz.append(t1 - t0)
+                        tsft.append(time.perf_counter() - t1)
+                    sweep[name]["set_zernike_rows_ms"] = 1e3 * statistics.median(tz[1:])
+                    sweep[name]["set_shifts_ms"] = 1e3 * statistics.median(tsft[1:])
                 if c == 1:      # launch-rate view of the tiny stack: 100 calls back to back between two events
                     sweep[name]["loop100_ms_per_call"] = loop_ms_per_call(torch, r["plan"], r["out"], local)
                 r["plan"].destroy()

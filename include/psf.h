@@ -123,7 +123,11 @@ psf_status psf_plan_create(const psf_plan_desc *desc, psf_plan **out);
 /* Zernike phase W = sum_{i<n_coeffs} coeffs[i] * Z_{noll_first+i}, radians, Noll-normalised (Eq. 18).
  * per_plane == 0: coeffs[n_coeffs] shared by all planes (folded into the static pupil);
  * per_plane == 1: coeffs[n_planes][n_coeffs], row b for plane b (evaluated in the pupil producer).
- * coeffs == NULL or n_coeffs == 0 clears the Zernike term.  coeffs is host memory, copied. */
+ * coeffs == NULL or n_coeffs == 0 clears the Zernike term.  coeffs is host memory, copied.
+ * Cost: a change of the term list, or of the mode, rebuilds and uploads the plan's tables (host, fp64).  Two cases are cheap,
+ * as they are the inner loop of a fit: new shared values on a plan that runs the 3xFP16 pair kernels are folded into the
+ * operand tables on the device (K doubles uploaded, two small launches; see PSF_TUNE_DEVICE_REFRESH), and new per-plane rows for
+ * the terms already set upload the rows only (2 * n_planes * n_coeffs floats).  psf_last_upload_bytes reports what a call moved. */
 psf_status psf_set_zernike(psf_plan *plan, const float *coeffs, int noll_first, int n_coeffs, int per_plane);
 
 /* Free phase mask W_0 of PAPER.md:176 Eq. 18 (vortex ramp, half-moon, measured wavefront ...): w0_rad is host
@@ -132,7 +136,9 @@ psf_status psf_set_zernike(psf_plan *plan, const float *coeffs, int noll_first, 
 psf_status psf_set_phase_mask(psf_plan *plan, const float *w0_rad);
 
 /* Per-plane lateral emitter position (x_b, y_b): plane b becomes I(x - x_b, y - y_b; z_b), applied as the pupil
- * tilt phase -k (s_x x_b + s_y y_b).  xy_um is host [n_planes][2]; NULL clears. */
+ * tilt phase -k (s_x x_b + s_y y_b).  xy_um is host [n_planes][2]; NULL clears.  Setting shifts for the first time (or
+ * clearing them) switches the plan between static and per-plane mode and rebuilds its tables; new values where shifts are
+ * already set upload the plane table only (16 bytes per plane). */
 psf_status psf_set_shifts(psf_plan *plan, const float *xy_um);
 
 /* Enqueue the whole stack on `cuda_stream`:

@@ -77,6 +77,43 @@ psf_status upload_ffma_tables(psf_plan *p) {
   return PSF_OK;
 }
 
+// Plane table: defocus (hi, lo) and the tilt of the lateral shift, per plane / emitter.
+psf_status upload_planes(psf_plan *p) {
+  const psf_plan_desc &d = p->desc;
+  DevPlan &P = p->dp;
+  std::vector<float4> planes(d.n_planes);
+  const double tscale = d.NA / d.wavelength_um;   // k s_max / 2 pi
+  P.has_shift = p->shifts.empty() ? 0 : 1;
+  for (int b = 0; b < d.n_planes; ++b) {
+    float zh, zl;
+    split2(p->z[b], zh, zl);
+    float tx = 0.f, ty = 0.f;
+    if (P.has_shift) { tx = (float)(tscale * (double)p->shifts[2 * b]); ty = (float)(tscale * (double)p->shifts[2 * b + 1]); }
+    planes[b] = make_float4(zh, zl, tx, ty);
+  }
+  psf_status s = upload(p, &p->d_planes, &p->cap_planes, planes);
+  if (s != PSF_OK) return s;
+  P.planes = (const float4 *)p->d_planes;
+  return PSF_OK;
+}
+
+// Per-plane Zernike rows: as given (the tiled FFMA kernels, the adjoint) and in the parity-sorted term order p->zorder
+// (k_small, k_smlm).
+psf_status upload_coef_rows(psf_plan *p) {
+  const int K = p->K_rows, Z = p->desc.n_planes;
+  std::vector<float> coefq(p->zern_rows.size(), 0.f);
+  for (int k = 0; k < K; ++k) {
+    const int j = p->zorder[k];
+    for (int b = 0; b < Z; ++b) coefq[(size_t)b * K + k] = p->zern_rows[(size_t)b * K + j];
+  }
+  psf_status s;
+  if ((s = upload(p, &p->d_coef, &p->cap_coef, p->zern_rows)) != PSF_OK) return s;
+  if ((s = upload(p, &p->d_coefq, &p->cap_coefq, coefq)) != PSF_OK) return s;
+  p->dp.coef = (const float *)p->d_coef;
+  p->dp.coefq = (const float *)p->d_coefq;
+  return PSF_OK;
+}
+
 // Folds the static pupil about both axes into the four parity classes and uploads every static table.
 psf_status upload_static(psf_plan *p) {
   const psf_plan_desc &d = p->desc;
@@ -161,9 +198,7 @@ psf_status upload_static(psf_plan *p) {
     std::vector<float> zb((size_t)K * NN, 0.f);
     for (size_t i = 0; i < zb.size(); ++i) zb[i] = (float)(p->zbasis[i] / twopi);
     if ((s = upload(p, &p->d_zb, &p->cap_zb, zb)) != PSF_OK) return s;
-    if ((s = upload(p, &p->d_coef, &p->cap_coef, p->zern_rows)) != PSF_OK) return s;
     P.zb = (const float *)p->d_zb;
-    P.coef = (const float *)p->d_coef;
     P.K = K;
     // folded, parity-sorted copy for the fused small-grid kernel: Z_j(-x, y) = +-Z_j(x, y), Z_j(x, -y) = +-Z_j(x, y)
     //   m = 0: even/even;  cos(m phi): even in y, odd in x iff m odd;  sin(m phi): odd in y, odd in x iff m even
@@ -177,17 +212,16 @@ psf_status upload_static(psf_plan *p) {
         const int yo = (kind == 2) ? 1 : 0;
         if (xo + 2 * yo == cls) { order.push_back(j); P.zcnt[cls]++; }
       }
-    std::vector<float> zbq((size_t)K * nn, 0.f), coefq(p->zern_rows.size(), 0.f);
+    p->zorder = order;
+    std::vector<float> zbq((size_t)K * nn, 0.f);
     for (int k = 0; k < K; ++k) {
       const int j = order[k];
       for (int qy = 0; qy < n; ++qy)
         for (int qx = 0; qx < n; ++qx) zbq[(size_t)k * nn + (size_t)qy * n + qx] = (float)(p->zbasis[(size_t)j * NN + (size_t)qy * N + qx] / twopi);
-      for (int b = 0; b < d.n_planes; ++b) coefq[(size_t)b * K + k] = p->zern_rows[(size_t)b * K + j];
     }
     if ((s = upload(p, &p->d_zbq, &p->cap_zbq, zbq)) != PSF_OK) return s;
-    if ((s = upload(p, &p->d_coefq, &p->cap_coefq, coefq)) != PSF_OK) return s;
+    if ((s = upload_coef_rows(p)) != PSF_OK) return s;
     P.zbq = (const float *)p->d_zbq;
-    P.coefq = (const float *)p->d_coefq;
     // the emitter-batch kernel for small grids (falls back to k_small when the plan does not qualify)
     smlm_free(p);
     if (p->tune_smlm && small_eligible(p) && d.precision != PSF_PREC_CZT_FFT && (s = smlm_setup(p, zbq)) != PSF_OK) return s;
@@ -196,19 +230,7 @@ psf_status upload_static(psf_plan *p) {
     for (int i = 0; i < 4; ++i) P.zcnt[i] = 0;
     smlm_free(p);
   }
-  // plane table
-  std::vector<float4> planes(d.n_planes);
-  const double tscale = d.NA / d.wavelength_um;   // k s_max / 2 pi
-  P.has_shift = p->shifts.empty() ? 0 : 1;
-  for (int b = 0; b < d.n_planes; ++b) {
-    float zh, zl;
-    split2(p->z[b], zh, zl);
-    float tx = 0.f, ty = 0.f;
-    if (P.has_shift) { tx = (float)(tscale * (double)p->shifts[2 * b]); ty = (float)(tscale * (double)p->shifts[2 * b + 1]); }
-    planes[b] = make_float4(zh, zl, tx, ty);
-  }
-  if ((s = upload(p, &p->d_planes, &p->cap_planes, planes)) != PSF_OK) return s;
-  P.planes = (const float4 *)p->d_planes;
+  if ((s = upload_planes(p)) != PSF_OK) return s;
   // path: tensor cores for the static (shared-pupil) mode when asked for or when the problem is large enough
   const psf_precision prec = d.precision;
   const bool want_tc = prec != PSF_PREC_FP32 && !P.per_plane && (prec == PSF_PREC_3XTF32 || prec == PSF_PREC_3XF16 || tc_eligible(p));
@@ -408,6 +430,15 @@ psf_status psf_set_zernike(psf_plan *p, const float *coeffs, int noll_first, int
       if (!std::isfinite(coeffs[i])) { p->err = "non-finite Zernike coefficient"; return PSF_ERR_INVALID_ARG; }
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  // new per-plane rows for the terms already set: only the two coefficient tables change (no table refresh, derived state stands)
+  if (per_plane && coeffs && n_coeffs > 0 && p->dp.per_plane && p->K_rows == n_coeffs && p->noll_first == noll_first &&
+      p->zern_shared.empty() && (int)p->zorder.size() == n_coeffs && (p->path == 0 || p->path == 3)) {
+    if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+    p->zern_rows.assign(coeffs, coeffs + cnt);
+    p->upload_bytes = 0;
+    psf_status s = upload_coef_rows(p);
+    return s != PSF_OK ? s : uploads_fence(p);
+  }
   p->zern_shared.clear();
   p->zern_rows.clear();
   p->K_rows = 0;
@@ -446,6 +477,14 @@ psf_status psf_set_shifts(psf_plan *p, const float *xy_um) {
       if (!std::isfinite(xy_um[i])) { p->err = "non-finite shift"; return PSF_ERR_INVALID_ARG; }
   cudaError_t e = cudaSetDevice(p->device);
   if (e != cudaSuccess) { p->err = cudaGetErrorString(e); return PSF_ERR_CUDA; }
+  // new shifts where shifts are already set: only the plane table changes
+  if (xy_um && !p->shifts.empty() && p->dp.per_plane && (p->path == 0 || p->path == 3)) {
+    if (wait_inflight(p) != cudaSuccess) { p->err = "cudaEventSynchronize (launches in flight) failed"; return PSF_ERR_CUDA; }
+    p->shifts.assign(xy_um, xy_um + 2 * (size_t)p->dp.Z);
+    p->upload_bytes = 0;
+    psf_status s = upload_planes(p);
+    return s != PSF_OK ? s : uploads_fence(p);
+  }
   p->shifts.clear();
   if (xy_um) p->shifts.assign(xy_um, xy_um + 2 * (size_t)p->dp.Z);
   p->dp.per_plane = (p->K_rows > 0 || !p->shifts.empty()) ? 1 : 0;

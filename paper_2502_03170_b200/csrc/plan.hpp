@@ -58,6 +58,7 @@ struct psf_plan {
   std::vector<float> zern_shared;
   int noll_first = 4;
   std::vector<float> zern_rows;  // [Z][K]
+  std::vector<int> zorder;       // parity-sorted order of the K per-plane terms (the coefq / zbq tables)
   int K_rows = 0;
   std::vector<float> shifts;     // [Z][2]
   std::vector<float> phase_mask; // [N][N] radians (psf_set_phase_mask), empty = none

@@ -724,3 +724,38 @@ def test_programmatic_dependent_launch_of_stage_two_changes_no_bit(psf, seed, N,
         plan.compute(out)
     assert torch.equal(out, ref)
     plan.destroy()
+
+
+@pytest.mark.parametrize("seed,N,M,Z", [(321, 64, 32, 40),      # k_smlm (emitter batches)
+                                        (322, 37, 33, 5),       # k_small, odd sizes
+                                        (323, 90, 70, 4)])      # tiled FFMA kernels in per-plane mode
+def test_new_per_plane_rows_and_shifts_only_move_their_own_tables(psf, seed, N, M, Z):
+    """psf_set_zernike (per-plane rows, same terms) and psf_set_shifts (shifts already set) upload the coefficient rows / the
+    plane table and nothing else; the stack and the adjoint must follow the new values."""
+    import torch
+    a = W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z)
+    b = W.small_random_case(seed + 50, pupil_n=N, out_m=M, n_planes=Z)
+    b = replace(a, zernike=b.zernike, shifts_um=b.shifts_um)
+    assert a.zernike.shape == b.zernike.shape and a.noll_first == b.noll_first
+    plan = psf.plan_from_case(a)
+    kernels = plan.kernel_names
+    assert plane_errors(plan.compute().cpu().numpy().astype(np.float64), O.stack_T2(a)).max() <= TOL
+    plan.set_zernike(b.zernike, b.noll_first)
+    assert plan.last_upload_bytes == 2 * b.zernike.nbytes                 # the rows, as given and in the parity-sorted order
+    plan.set_shifts(b.shifts_um)
+    assert plan.last_upload_bytes == 16 * Z                               # the plane table
+    assert plan.kernel_names == kernels
+    I = plan.compute().cpu().numpy().astype(np.float64)
+    assert plane_errors(I, O.stack_T2(b)).max() <= TOL
+    # same values through a fresh plan: same bits (the tables are the same)
+    fresh = psf.plan_from_case(b)
+    assert np.array_equal(fresh.compute().cpu().numpy(), I.astype(np.float32))
+    G = torch.from_numpy(np.random.default_rng(seed).standard_normal((Z, M, M)).astype(np.float32)).cuda()
+    dz, dc = plan.gradients(G)
+    dz0, dc0 = fresh.gradients(G)
+    torch.cuda.synchronize()
+    # (the adjoint's reduction adds fp64 partial sums with atomics: equal to rounding, not to the bit)
+    assert np.allclose(dz.cpu().numpy(), dz0.cpu().numpy(), rtol=1e-9, atol=1e-9 * float(dz0.abs().max()))
+    assert np.allclose(dc.cpu().numpy(), dc0.cpu().numpy(), rtol=1e-9, atol=1e-9 * float(dc0.abs().max()))
+    fresh.destroy()
+    plan.destroy()
