@@ -613,7 +613,7 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_ASPLIT: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_asplit = (int)value;
     } else if (knob == PSF_TUNE_SMLM) {
-      if (value < 0 || value > 1) { p->err = "PSF_TUNE_SMLM: 0..1"; return PSF_ERR_INVALID_ARG; }
+      if (value < 0 || value > 2) { p->err = "PSF_TUNE_SMLM: 0..2"; return PSF_ERR_INVALID_ARG; }
       p->tune_smlm = (int)value;
     } else if (knob == PSF_TUNE_PDL) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_PDL: 0..1"; return PSF_ERR_INVALID_ARG; }
@@ -702,7 +702,7 @@ long long psf_last_upload_bytes(const psf_plan *p) { return p ? p->upload_bytes 
 const char *psf_kernel_names(psf_plan *p) {
   if (!p) return "";
   try {
-    if (p->path == 3) p->kernel_names = p->smlm ? "k_smlm" : "k_small";
+    if (p->path == 3) p->kernel_names = p->smlm ? (smlm_on_tensor_cores(p) ? "k_smlm_tc" : "k_smlm") : "k_small";
     else if (p->path == 4) p->kernel_names = "czt_rows,czt_cols";
     else if ((p->path == 1 || p->path == 2) && p->tc) p->kernel_names = tc_kernel_names(p);
     else p->kernel_names = "k1_stage1,k2_stage2";

@@ -22,8 +22,11 @@
 #include <cmath>
 #include <complex>
 
+#include <cuda_fp16.h>
+
 #include "plan.hpp"
 #include "pupil_gen.cuh"
+#include "tc_common.cuh"
 
 namespace psf {
 
@@ -37,6 +40,11 @@ struct SmlmState {
   void *d_zbp = nullptr;       // [K][32][32] float folded basis / 2 pi, terms sorted by parity class, zero padded
   int smem = 0, mq = 16;
   long long version = -1;
+  // tensor-core variant (k_smlm_tc): m <= 16, precision AUTO / 3xFP16
+  bool tc = false;
+  void *d_xy = nullptr;        // 4096 bytes: the cos | sin table as the UMMA B operand (fp16 hi | lo rows, swizzled)
+  int smem_tc = 0, lanes_tc = 0;
+  float sQ = 1.f, f1 = 1.f, fs2 = 1.f;
 };
 
 namespace {
@@ -288,6 +296,291 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, 
   }
 }
 
+// ---- k_smlm_tc: the same emitter batch with both DFT stages on tcgen05 (3xFP16 split), SURVEY 8 / round-1 review item 5 option B ----
+// Per emitter and component the folded pupil is the A operand of stage 1: two tiles (x-parity b) of 128 rows = (a, re/im) x 32 q_y,
+// K = 32 q_x, against the shared cos (b = e) or sin (b = o) table as B (N = 16 m_x); the accumulator D1[(a, ri, q_y)][m_x] comes
+// back through registers as the A operand of stage 2, rows = (class, re/im, m_x) = 128, K = 32 q_y - each warp reads its TMEM
+// quarter (one chain, lane = q_y) and the 32 lanes write 32 consecutive K positions of a row, so the transposition costs
+// nothing - against the same table (cos rows | sin rows, N = 32: a chain uses the half that matches its y-parity).  A row
+// of every operand is 128 bytes = [hi(32 k) | lo(32 k)] fp16, SWIZZLE_128B, so x = hi + lo on both sides is three K = 32
+// products picked by the K offsets of the descriptors.  A lane (128 threads = the four TMEM quarters) does everything for
+// its emitter - generate, issue, drain, issue, combine - and LANES lanes interleave on the SM.
+constexpr int ST_TILE = 16384;                 // [128 rows][128 B]
+constexpr int ST_LANE_BYTES = 3 * ST_TILE;     // A1 (two parity tiles) + A2 (later the F exchange buffer)
+constexpr int ST_XY = 4096;                    // [32 rows][128 B]: rows 0..15 cos, 16..31 sin
+constexpr int ST_FCH = 16 * 16 + 16;           // floats per chain in the F buffer (padded: the re / im halves of a warp hit different banks)
+constexpr float ST_XSCALE = 256.f;
+
+struct SmlmTcArgs {
+  const float2 *bcls;
+  const uint4 *xy;            // the table, fp16 hi | lo, already swizzled: 4096 bytes
+  const float2 *ktp;
+  const float *zbp;
+  int ncls, K;
+  int comp_start[6];
+  int cls_ab[12];
+  float sQ;                   // operand scale of the folded pupil
+  float f1;                   // s_T / (s_Q s_X): D1 -> stage-2 operand
+  float fs2;                  // (1 / (s_T s_X))^2: |D2|^2 -> |F|^2
+};
+
+template <int LANES>
+__global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan P, const SmlmTcArgs A, float *__restrict__ I) {
+  using namespace tc;
+  constexpr uint32_t IDESC1 = umma_idesc_f16(128, 16), IDESC2 = umma_idesc_f16(128, 32);
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t *xy = smem;
+  float2 *kts = reinterpret_cast<float2 *>(smem + ST_XY + LANES * ST_LANE_BYTES);
+  float2 *bcl = kts + SL_NQ * SL_NQ;
+  float *zbs = reinterpret_cast<float *>(bcl + (size_t)A.ncls * SL_NQ * SL_NQ);
+  float *cf_all = zbs + (size_t)A.K * SL_NQ * SL_NQ;
+  __shared__ uint64_t mbar[LANES];
+  __shared__ uint32_t tmem_slot;
+  const int lane_id = threadIdx.x / SL_THREADS, lt = threadIdx.x % SL_THREADS;
+  const int warp = lt >> 5, l = lt & 31;
+  uint8_t *A1 = smem + ST_XY + lane_id * ST_LANE_BYTES, *A2 = A1 + 2 * ST_TILE;
+  float *Fb = reinterpret_cast<float *>(A2);
+  float *cfs = cf_all + lane_id * 16;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < LANES; ++i) mbar_init(&mbar[i], 1);
+    fence_barrier_init();
+  }
+  if (threadIdx.x < 32) tmem_alloc(&tmem_slot, 512);
+  for (int i = threadIdx.x; i < ST_XY / 16; i += blockDim.x) reinterpret_cast<uint4 *>(xy)[i] = __ldg(A.xy + i);
+  for (int i = threadIdx.x; i < SL_NQ * SL_NQ; i += blockDim.x) kts[i] = __ldg(A.ktp + i);
+  for (int i = threadIdx.x; i < A.ncls * SL_NQ * SL_NQ; i += blockDim.x) bcl[i] = __ldg(A.bcls + i);
+  for (int i = threadIdx.x; i < A.K * SL_NQ * SL_NQ; i += blockDim.x) zbs[i] = __ldg(A.zbp + i);
+  fence_proxy_async_smem();                    // the table is read by the async proxy
+  tcgen05_fence_before();
+  __syncthreads();
+  tcgen05_fence_after();
+  const uint32_t tmem = tmem_slot + lane_id * 128;      // this lane's columns: D1(c, b) at c * 32 + b * 16, D2(c) over them
+  const uint32_t tq = tmem + ((uint32_t)(warp * 32) << 16);
+
+  const int m = P.m, M = P.M, N = P.N, K = A.K;
+  // generation: a thread owns two adjacent q_x at four q_y; the half-warps sit four rows apart (different swizzle phase)
+  const int qxp = lt & 15, qx0 = 2 * qxp, qyb = warp + 4 * ((lt >> 4) & 1);
+  uint32_t ph = 0;
+
+  for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
+    const float4 pl = __ldg(P.planes + b);
+    sl_bar(lane_id);                                     // the previous emitter's reads of cfs are done
+    if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
+    sl_bar(lane_id);
+
+    // ---- phase 0: parity transform Phi_g of the emitter's phasor field at the thread's 8 folded samples ----
+    // (term loops outermost, the thread's 8 samples inside: 8 independent FMA chains per shared-memory round trip)
+    float2 phi[8][4];
+    {
+      float pcl[8][4];
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int f = (qyb + 8 * (r >> 1)) * SL_NQ + qx0 + (r & 1);
+        pcl[r][0] = kz_turns(kts[f], pl.x, pl.y);
+        pcl[r][1] = pcl[r][2] = pcl[r][3] = 0.f;
+      }
+      int j = 0;
+#pragma unroll
+      for (int cls = 0; cls < 4; ++cls)
+        for (int e = j + P.zcnt[cls]; j < e; ++j) {
+          const float cj = cfs[j];
+          const float *zb = zbs + j * (SL_NQ * SL_NQ) + qyb * SL_NQ + qx0;
+#pragma unroll
+          for (int rr = 0; rr < 4; ++rr) {
+            const float2 z2 = *reinterpret_cast<const float2 *>(zb + 8 * rr * SL_NQ);
+            pcl[2 * rr][cls] = fmaf(cj, z2.x, pcl[2 * rr][cls]);
+            pcl[2 * rr + 1][cls] = fmaf(cj, z2.y, pcl[2 * rr + 1][cls]);
+          }
+        }
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int qy = qyb + 8 * (r >> 1), qx = qx0 + (r & 1);
+        if (P.has_shift) {
+          const float ux = (float)(2 * qx + 1 - N) / (float)N, uy = (float)(2 * qy + 1 - N) / (float)N;
+          pcl[r][1] = fmaf(-ux, pl.z, pcl[r][1]);
+          pcl[r][2] = fmaf(-uy, pl.w, pcl[r][2]);
+        }
+        float2 e[4];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+          for (int bb = 0; bb < 2; ++bb) {
+            const float sx = bb ? -1.f : 1.f, sy = a ? -1.f : 1.f;
+            sl_sincos_turns(pcl[r][0] + sx * pcl[r][1] + sy * pcl[r][2] + sx * sy * pcl[r][3], e[a * 2 + bb].y, e[a * 2 + bb].x);
+          }
+        const float2 s01 = make_float2(e[0].x + e[1].x, e[0].y + e[1].y), d01 = make_float2(e[0].x - e[1].x, e[0].y - e[1].y);
+        const float2 s23 = make_float2(e[2].x + e[3].x, e[2].y + e[3].y), d23 = make_float2(e[2].x - e[3].x, e[2].y - e[3].y);
+        phi[r][0] = make_float2(s01.x + s23.x, s01.y + s23.y);
+        phi[r][1] = make_float2(d01.x + d23.x, d01.y + d23.y);
+        phi[r][2] = make_float2(s01.x - s23.x, s01.y - s23.y);
+        phi[r][3] = make_float2(d01.x - d23.x, d01.y - d23.y);
+      }
+    }
+
+    float inten[2][4];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) inten[i][q] = 0.f;
+
+    for (int c = 0; c < P.C; ++c) {
+      // ---- Q_g = sum_ab B_ab Phi_(g xor ab), scaled, split, into the two stage-1 operand tiles ----
+#pragma unroll
+      for (int rr = 0; rr < 4; ++rr) {
+        const int qy = qyb + 8 * rr;
+        float2 o[2][4];
+        o[0][0] = o[0][1] = o[0][2] = o[0][3] = o[1][0] = o[1][1] = o[1][2] = o[1][3] = make_float2(0.f, 0.f);
+        for (int ci = A.comp_start[c]; ci < A.comp_start[c + 1]; ++ci) {
+          const float4 b2 = *reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + qy * SL_NQ + qx0]);
+          const float2 bv[2] = {make_float2(b2.x, b2.y), make_float2(b2.z, b2.w)};
+          const int x = A.cls_ab[ci];                    // Phi index = g xor ab; static register indices in every branch
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int r = 2 * rr + e;
+            switch (x) {
+              case 0: o[e][0] = cfma(bv[e], phi[r][0], o[e][0]); o[e][1] = cfma(bv[e], phi[r][1], o[e][1]); o[e][2] = cfma(bv[e], phi[r][2], o[e][2]); o[e][3] = cfma(bv[e], phi[r][3], o[e][3]); break;
+              case 1: o[e][0] = cfma(bv[e], phi[r][1], o[e][0]); o[e][1] = cfma(bv[e], phi[r][0], o[e][1]); o[e][2] = cfma(bv[e], phi[r][3], o[e][2]); o[e][3] = cfma(bv[e], phi[r][2], o[e][3]); break;
+              case 2: o[e][0] = cfma(bv[e], phi[r][2], o[e][0]); o[e][1] = cfma(bv[e], phi[r][3], o[e][1]); o[e][2] = cfma(bv[e], phi[r][0], o[e][2]); o[e][3] = cfma(bv[e], phi[r][1], o[e][3]); break;
+              default: o[e][0] = cfma(bv[e], phi[r][3], o[e][0]); o[e][1] = cfma(bv[e], phi[r][2], o[e][1]); o[e][2] = cfma(bv[e], phi[r][1], o[e][2]); o[e][3] = cfma(bv[e], phi[r][0], o[e][3]); break;
+            }
+          }
+        }
+        // class g = 2 a + xb -> tile xb, rows (2 a + ri) * 32 + qy; the pair (qx0, qx0 + 1) is one 32-bit word of the row
+        const uint32_t sw = (uint32_t)(qy & 7);
+        const uint32_t off_hi = ((((uint32_t)qxp >> 2) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
+        const uint32_t off_lo = (((((uint32_t)qxp >> 2) + 4u) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          const uint32_t tile = smem_u32(A1) + (uint32_t)(g & 1) * ST_TILE;
+          uint32_t hi, lo;
+          split_f16x2(A.sQ * o[0][g].x, A.sQ * o[1][g].x, hi, lo);
+          uint32_t row = (uint32_t)(((g >> 1) * 2 + 0) * 32 + qy) * 128u;
+          st_shared_u32(tile + row + off_hi, hi);
+          st_shared_u32(tile + row + off_lo, lo);
+          split_f16x2(A.sQ * o[0][g].y, A.sQ * o[1][g].y, hi, lo);
+          row = (uint32_t)(((g >> 1) * 2 + 1) * 32 + qy) * 128u;
+          st_shared_u32(tile + row + off_hi, hi);
+          st_shared_u32(tile + row + off_lo, lo);
+        }
+      }
+      fence_proxy_async_smem();
+      tcgen05_fence_before();                            // (the previous component's TMEM reads of this lane are behind us)
+      sl_bar(lane_id);
+      if (lt == 0) {
+        tcgen05_fence_after();
+#pragma unroll
+        for (int xb = 0; xb < 2; ++xb) {
+          const uint32_t d = tmem + c * 32 + xb * 16;
+          const uint32_t a = smem_u32(A1) + xb * ST_TILE, t = smem_u32(xy) + xb * 2048;
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const uint32_t o = k * 32;
+            umma_f16(d, umma_desc_sw128(a + 64 + o), umma_desc_sw128(t + o), IDESC1, k == 0 ? 0u : 1u);   // lo x hi
+            umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + 64 + o), IDESC1, 1u);                 // hi x lo
+            umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + o), IDESC1, 1u);                      // hi x hi
+          }
+        }
+        umma_commit(&mbar[lane_id]);
+      }
+      mbar_wait(&mbar[lane_id], ph);
+      ph ^= 1;
+      tcgen05_fence_after();
+
+      // ---- drain D1: warp = chain (a, ri) of tile xb, lane = q_y; write T^T rows (class, ri, m_x), K = q_y ----
+#pragma unroll
+      for (int xb = 0; xb < 2; ++xb) {
+        uint32_t v[16];
+        tmem_ld_32x32b_x16(tq + c * 32 + xb * 16, v);
+        tmem_ld_wait();
+        const int chain8 = (((warp >> 1) * 2 + xb) * 2) + (warp & 1);
+        // lane pairs exchange so that each lane owns two adjacent q_y of one row: even lanes row mxa, odd lanes row mxa + 4
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int mxa = (j & 3) + 8 * (j >> 2), mxb = mxa + 4;
+          const float va = A.f1 * __uint_as_float(v[mxa]), vb = A.f1 * __uint_as_float(v[mxb]);
+          const float send = (l & 1) ? va : vb;
+          const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
+          const float p0 = (l & 1) ? recv : va, p1 = (l & 1) ? vb : recv;      // (q_y even, q_y odd) of the lane's row
+          const int mx = (l & 1) ? mxb : mxa;
+          uint32_t hi, lo;
+          split_f16x2(p0, p1, hi, lo);
+          const uint32_t row = (uint32_t)(chain8 * 16 + mx);
+          const uint32_t w = (uint32_t)(l >> 1);                               // 32-bit word of the hi half: q_y pair
+          const uint32_t base = smem_u32(A2) + row * 128u;
+          st_shared_u32(base + ((((w >> 2)) ^ (row & 7u)) << 4) + ((w & 3u) << 2), hi);
+          st_shared_u32(base + ((((w >> 2) + 4u) ^ (row & 7u)) << 4) + ((w & 3u) << 2), lo);
+        }
+      }
+      fence_proxy_async_smem();
+      tcgen05_fence_before();
+      sl_bar(lane_id);
+      if (lt == 0) {
+        tcgen05_fence_after();
+        const uint32_t d = tmem + c * 32;
+        const uint32_t a = smem_u32(A2), t = smem_u32(xy);
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const uint32_t o = k * 32;
+          umma_f16(d, umma_desc_sw128(a + 64 + o), umma_desc_sw128(t + o), IDESC2, k == 0 ? 0u : 1u);
+          umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + 64 + o), IDESC2, 1u);
+          umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + o), IDESC2, 1u);
+        }
+        umma_commit(&mbar[lane_id]);
+      }
+      mbar_wait(&mbar[lane_id], ph);
+      ph ^= 1;
+      tcgen05_fence_after();
+
+      // ---- D2: warp = class (re rows 0..15, im rows 16..31 of the quarter), lane = (ri, m_x); its y-parity picks the column half ----
+      {
+        uint32_t v[16];
+        tmem_ld_32x32b_x16(tq + c * 32 + (warp >> 1) * 16, v);
+        tmem_ld_wait();
+        float *dst = Fb + (warp * 2 + (l >> 4)) * ST_FCH + (l & 15);
+#pragma unroll
+        for (int my = 0; my < 16; ++my) dst[my * 16] = __uint_as_float(v[my]);
+      }
+      tcgen05_fence_before();
+      sl_bar(lane_id);
+      // ---- butterfly + |E|^2 at the thread's two pixels of the quadrant ----
+      const float w = P.weight[c] * A.fs2;
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int px = lt + SL_THREADS * i;                // = my * 16 + mx
+        const float a0 = Fb[0 * ST_FCH + px], a1 = Fb[1 * ST_FCH + px], a2 = Fb[2 * ST_FCH + px], a3 = Fb[3 * ST_FCH + px];
+        const float a4 = Fb[4 * ST_FCH + px], a5 = Fb[5 * ST_FCH + px], a6 = Fb[6 * ST_FCH + px], a7 = Fb[7 * ST_FCH + px];
+        const float re0 = a0 - a3 - a5 - a6, im0 = a1 + a2 + a4 - a7;
+        const float re1 = a0 + a3 - a5 + a6, im1 = a1 - a2 + a4 + a7;
+        const float re2 = a0 - a3 + a5 + a6, im2 = a1 + a2 - a4 + a7;
+        const float re3 = a0 + a3 + a5 - a6, im3 = a1 - a2 - a4 - a7;
+        inten[i][0] = fmaf(w, re0 * re0 + im0 * im0, inten[i][0]);
+        inten[i][1] = fmaf(w, re1 * re1 + im1 * im1, inten[i][1]);
+        inten[i][2] = fmaf(w, re2 * re2 + im2 * im2, inten[i][2]);
+        inten[i][3] = fmaf(w, re3 * re3 + im3 * im3, inten[i][3]);
+      }
+      // (the next write of this buffer - the drain of the next component - is behind two more lane barriers)
+    }
+
+    float *Ib = I + (size_t)b * M * M;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int px = lt + SL_THREADS * i, my = px >> 4, mx = px & 15;
+      if (my < m && mx < m) {
+        const int myr = M - 1 - my;
+        Ib[(size_t)my * M + mx] = inten[i][0];
+        Ib[(size_t)my * M + (M - 1 - mx)] = inten[i][1];
+        Ib[(size_t)myr * M + mx] = inten[i][2];
+        Ib[(size_t)myr * M + (M - 1 - mx)] = inten[i][3];
+      }
+    }
+  }
+  tcgen05_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) tmem_dealloc(tmem_slot, 512);
+}
+
 template <int MQ, int LANES>
 cudaError_t sl_launch(const psf_plan *p, const SmlmState *t, const SmlmArgs &A, cudaStream_t st, float *intensity) {
   const int per = (p->dp.Z + LANES - 1) / LANES;
@@ -311,7 +604,7 @@ bool sl_up(void **d, const std::vector<T> &h, long long *acc) {
 void smlm_free(psf_plan *p) {
   SmlmState *t = p->smlm;
   if (!t) return;
-  void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp};
+  void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp, t->d_xy};
   for (void *b : bufs)
     if (b) cudaFree(b);
   delete t;
@@ -401,11 +694,79 @@ psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted) {
   }
   if (e != cudaSuccess) { p->err = std::string("smlm: cudaFuncSetAttribute: ") + cudaGetErrorString(e); smlm_free(p); return PSF_ERR_CUDA; }
   t->version = p->table_version;
+  // ---- tensor-core variant: both DFT stages on tcgen05 (3xFP16), where the quadrant fits one 16-column tile ----
+  const psf_precision prec = p->desc.precision;
+  if (p->tune_smlm == 1 && m <= 16 && (prec == PSF_PREC_AUTO || prec == PSF_PREC_3XF16)) {
+    // operand scales from phase-independent bounds: |Phi_g| <= 4, |Q_g| <= 4 sum_ab |B_ab|, |T| <= sum_qx |Q|
+    double qmax = 0.0, rmax = 0.0;
+    for (int c = 0; c < C; ++c)
+      for (int qy = 0; qy < n; ++qy) {
+        double rs = 0.0;
+        for (int qx = 0; qx < n; ++qx) {
+          double a = 0.0;
+          for (int ci = t->comp_start[c]; ci < t->comp_start[c + 1]; ++ci) {
+            const float2 v = bcls[(size_t)ci * SL_NQ * SL_NQ + (size_t)qy * SL_NQ + qx];
+            a += std::sqrt((double)v.x * v.x + (double)v.y * v.y);
+          }
+          a *= 4.0;
+          qmax = std::max(qmax, a);
+          rs += a;
+        }
+        rmax = std::max(rmax, rs);
+      }
+    auto pow2 = [](double v, double limit) { return v > 0 ? std::exp2(std::floor(std::log2(limit / v))) : 1.0; };
+    const double sQ = pow2(qmax, 16384.0), sT = pow2(rmax, 32768.0), sX = (double)ST_XSCALE;
+    t->sQ = (float)sQ;
+    t->f1 = (float)(sT / (sQ * sX));
+    t->fs2 = (float)((1.0 / (sT * sX)) * (1.0 / (sT * sX)));
+    std::vector<__half> xy((size_t)ST_XY / 2, __float2half_rn(0.f));
+    for (int row = 0; row < 32; ++row) {
+      const int mi = row & 15;
+      if (mi >= m) continue;
+      for (int q = 0; q < n; ++q) {
+        const double ph = p->phi[(size_t)mi * n + q];
+        const double v = sX * ((row >> 4) ? std::sin(ph) : std::cos(ph));
+        const __half hi = __float2half_rn((float)v);
+        const __half lo = __float2half_rn((float)(v - (double)__half2float(hi)));
+        const int bh = 2 * q, bl = 64 + 2 * q;          // byte offsets in the 128-byte row, before the swizzle
+        const int ph_hi = row * 128 + ((((bh >> 4) ^ (row & 7)) << 4) | (bh & 15));
+        const int ph_lo = row * 128 + ((((bl >> 4) ^ (row & 7)) << 4) | (bl & 15));
+        xy[ph_hi / 2] = hi;
+        xy[ph_lo / 2] = lo;
+      }
+    }
+    const size_t fixed_tc = (size_t)ST_XY + (size_t)SL_NQ * SL_NQ * 8 + (size_t)ncls * SL_NQ * SL_NQ * 8 + (size_t)K * SL_NQ * SL_NQ * 4 + 1024 + 256;
+    const int lanes_tc = (fixed_tc + 3 * (size_t)ST_LANE_BYTES <= limit) ? 3 : (fixed_tc + 2 * (size_t)ST_LANE_BYTES <= limit) ? 2 : 0;
+    if (lanes_tc && sl_up(&t->d_xy, xy, &p->upload_bytes)) {
+      t->lanes_tc = lanes_tc;
+      t->smem_tc = (int)(fixed_tc + lanes_tc * (size_t)ST_LANE_BYTES);
+      e = lanes_tc == 3 ? cudaFuncSetAttribute(k_smlm_tc<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem_tc)
+                        : cudaFuncSetAttribute(k_smlm_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem_tc);
+      if (e != cudaSuccess) { p->err = std::string("smlm: cudaFuncSetAttribute (tensor variant): ") + cudaGetErrorString(e); smlm_free(p); return PSF_ERR_CUDA; }
+      t->tc = true;
+    }
+  }
   return PSF_OK;
 }
 
+bool smlm_on_tensor_cores(const psf_plan *p) { return p->smlm && p->smlm->tc; }
+
 cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity) {
   const SmlmState *t = p->smlm;
+  if (t->tc) {
+    SmlmTcArgs T;
+    T.bcls = (const float2 *)t->d_bcls; T.xy = (const uint4 *)t->d_xy; T.ktp = (const float2 *)t->d_ktp; T.zbp = (const float *)t->d_zbp;
+    T.ncls = t->ncls; T.K = t->K;
+    for (int i = 0; i < 6; ++i) T.comp_start[i] = t->comp_start[i];
+    for (int i = 0; i < 12; ++i) T.cls_ab[i] = t->cls_ab[i];
+    T.sQ = t->sQ; T.f1 = t->f1; T.fs2 = t->fs2;
+    const int L = t->lanes_tc, per = (p->dp.Z + L - 1) / L;
+    const int grid = per < p->sm_count ? per : p->sm_count;
+    if (L == 3) k_smlm_tc<3><<<grid, SL_THREADS * 3, t->smem_tc, st>>>(p->dp, T, intensity);
+    else k_smlm_tc<2><<<grid, SL_THREADS * 2, t->smem_tc, st>>>(p->dp, T, intensity);
+    prof_mark(p, st, 0);
+    return cudaGetLastError();
+  }
   SmlmArgs A;
   A.bcls = (const float2 *)t->d_bcls; A.xd = (const float2 *)t->d_xd; A.ktp = (const float2 *)t->d_ktp; A.zbp = (const float *)t->d_zbp;
   A.ncls = t->ncls; A.K = t->K;

@@ -159,6 +159,7 @@ cudaError_t launch_bessel(const psf_plan *p, cudaStream_t st, float *intensity);
 psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted);
 void smlm_free(psf_plan *p);
 cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity);
+bool smlm_on_tensor_cores(const psf_plan *p);
 // kernels_czt.cu
 bool czt_supported(const psf_plan *p, std::string &why);
 psf_status czt_setup(psf_plan *p);
