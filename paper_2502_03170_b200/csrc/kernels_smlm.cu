@@ -42,6 +42,7 @@ struct SmlmState {
   long long version = -1;
   // tensor-core variant (k_smlm_tc): m <= 16, precision AUTO / 3xFP16
   bool tc = false;
+  void *d_bcls_tc = nullptr;   // the class tables times the operand scale s_Q
   void *d_xy = nullptr;        // 4096 bytes: the cos | sin table as the UMMA B operand (fp16 hi | lo rows, swizzled)
   int smem_tc = 0, lanes_tc = 0;
   float sQ = 1.f, f1 = 1.f, fs2 = 1.f;
@@ -312,14 +313,13 @@ constexpr int ST_FCH = 16 * 16 + 16;           // floats per chain in the F buff
 constexpr float ST_XSCALE = 256.f;
 
 struct SmlmTcArgs {
-  const float2 *bcls;
+  const float2 *bcls;         // class tables, pre-scaled by s_Q
   const uint4 *xy;            // the table, fp16 hi | lo, already swizzled: 4096 bytes
   const float2 *ktp;
   const float *zbp;
   int ncls, K;
   int comp_start[6];
   int cls_ab[12];
-  float sQ;                   // operand scale of the folded pupil
   float f1;                   // s_T / (s_Q s_X): D1 -> stage-2 operand
   float fs2;                  // (1 / (s_T s_X))^2: |D2|^2 -> |F|^2
 };
@@ -329,13 +329,13 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   using namespace tc;
   constexpr uint32_t IDESC1 = umma_idesc_f16(128, 16), IDESC2 = umma_idesc_f16(128, 32);
   extern __shared__ uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // (pointer arithmetic: the compiler keeps the shared address space)
   uint8_t *xy = smem;
   float2 *kts = reinterpret_cast<float2 *>(smem + ST_XY + LANES * ST_LANE_BYTES);
   float2 *bcl = kts + SL_NQ * SL_NQ;
   float *zbs = reinterpret_cast<float *>(bcl + (size_t)A.ncls * SL_NQ * SL_NQ);
   float *cf_all = zbs + (size_t)A.K * SL_NQ * SL_NQ;
-  __shared__ uint64_t mbar[LANES];
+  __shared__ uint64_t mbar1[LANES], mbar2[LANES];
   __shared__ uint32_t tmem_slot;
   const int lane_id = threadIdx.x / SL_THREADS, lt = threadIdx.x % SL_THREADS;
   const int warp = lt >> 5, l = lt & 31;
@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   float *cfs = cf_all + lane_id * 16;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < LANES; ++i) mbar_init(&mbar[i], 1);
+    for (int i = 0; i < LANES; ++i) { mbar_init(&mbar1[i], 2); mbar_init(&mbar2[i], 1); }
     fence_barrier_init();
   }
   if (threadIdx.x < 32) tmem_alloc(&tmem_slot, 512);
@@ -362,7 +362,17 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   const int m = P.m, M = P.M, N = P.N, K = A.K;
   // generation: a thread owns two adjacent q_x at four q_y; the half-warps sit four rows apart (different swizzle phase)
   const int qxp = lt & 15, qx0 = 2 * qxp, qyb = warp + 4 * ((lt >> 4) & 1);
-  uint32_t ph = 0;
+  uint32_t ph1 = 0, ph2 = 0;
+  // operand addresses of the thread's stores: the swizzle phase (q_y & 7) and the word inside the row do not change over the 4 q_y
+  const uint32_t sw = (uint32_t)(qyb & 7);
+  const uint32_t off_hi = ((((uint32_t)qxp >> 2) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
+  const uint32_t off_lo = (((((uint32_t)qxp >> 2) + 4u) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
+  // drain stores: row = chain8 * 16 + m_x with m_x = mxa + 4 (lane & 1); the row's swizzle phase is m_x & 7 = (j & 3) + 4 (lane & 1)
+  const uint32_t a2_base = smem_u32(A2) + (uint32_t)((((warp >> 1) * 4 + (warp & 1)) * 16 + 4 * (l & 1)) * 128) + (((uint32_t)(l >> 1) & 3u) << 2);
+  uint32_t a2_sw[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) a2_sw[k] = ((((uint32_t)l >> 3) ^ (uint32_t)(k + 4 * (l & 1))) << 4);
+  const uint32_t a1_hi = smem_u32(A1) + (uint32_t)qyb * 128u + off_hi, a1_lo = smem_u32(A1) + (uint32_t)qyb * 128u + off_lo;
 
   for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
     const float4 pl = __ldg(P.planes + b);
@@ -425,68 +435,102 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
 #pragma unroll
       for (int q = 0; q < 4; ++q) inten[i][q] = 0.f;
 
+    // second half of a component: D2 -> F buffer -> butterfly + |E|^2.  Runs one component behind the first half, so that the
+    // stage-2 product of component c is in flight while the operands of c + 1 are generated, and the stage-1 product of c + 1
+    // while this runs.
+    auto finish = [&](int cc) {
+      mbar_wait(&mbar2[lane_id], ph2);
+      ph2 ^= 1;
+      tcgen05_fence_after();
+
+      // ---- D2: warp = class (re rows 0..15, im rows 16..31 of the quarter), lane = (ri, m_x); its y-parity picks the column half ----
+      {
+        uint32_t v[16];
+        tmem_ld_32x32b_x16(tq + cc * 32 + (warp >> 1) * 16, v);
+        tmem_ld_wait();
+        float *dst = Fb + (warp * 2 + (l >> 4)) * ST_FCH + (l & 15);
+#pragma unroll
+        for (int my = 0; my < 16; ++my) dst[my * 16] = __uint_as_float(v[my]);
+      }
+      tcgen05_fence_before();
+      sl_bar(lane_id);
+      // ---- butterfly + |E|^2 at the thread's two pixels of the quadrant ----
+      const float w = P.weight[cc] * A.fs2;
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int px = lt + SL_THREADS * i;                // = my * 16 + mx
+        const float a0 = Fb[0 * ST_FCH + px], a1 = Fb[1 * ST_FCH + px], a2 = Fb[2 * ST_FCH + px], a3 = Fb[3 * ST_FCH + px];
+        const float a4 = Fb[4 * ST_FCH + px], a5 = Fb[5 * ST_FCH + px], a6 = Fb[6 * ST_FCH + px], a7 = Fb[7 * ST_FCH + px];
+        const float re0 = a0 - a3 - a5 - a6, im0 = a1 + a2 + a4 - a7;
+        const float re1 = a0 + a3 - a5 + a6, im1 = a1 - a2 + a4 + a7;
+        const float re2 = a0 - a3 + a5 + a6, im2 = a1 + a2 - a4 + a7;
+        const float re3 = a0 + a3 + a5 - a6, im3 = a1 - a2 - a4 - a7;
+        inten[i][0] = fmaf(w, re0 * re0 + im0 * im0, inten[i][0]);
+        inten[i][1] = fmaf(w, re1 * re1 + im1 * im1, inten[i][1]);
+        inten[i][2] = fmaf(w, re2 * re2 + im2 * im2, inten[i][2]);
+        inten[i][3] = fmaf(w, re3 * re3 + im3 * im3, inten[i][3]);
+      }
+    };
+
     for (int c = 0; c < P.C; ++c) {
       // ---- Q_g = sum_ab B_ab Phi_(g xor ab), scaled, split, into the two stage-1 operand tiles ----
+      const int c0 = A.comp_start[c], c1 = A.comp_start[c + 1];
 #pragma unroll
       for (int rr = 0; rr < 4; ++rr) {
-        const int qy = qyb + 8 * rr;
         float2 o[2][4];
         o[0][0] = o[0][1] = o[0][2] = o[0][3] = o[1][0] = o[1][1] = o[1][2] = o[1][3] = make_float2(0.f, 0.f);
-        for (int ci = A.comp_start[c]; ci < A.comp_start[c + 1]; ++ci) {
-          const float4 b2 = *reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + qy * SL_NQ + qx0]);
+        for (int ci = c0; ci < c1; ++ci) {
+          const float4 b2 = *reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + (qyb + 8 * rr) * SL_NQ + qx0]);
           const float2 bv[2] = {make_float2(b2.x, b2.y), make_float2(b2.z, b2.w)};
-          const int x = A.cls_ab[ci];                    // Phi index = g xor ab; static register indices in every branch
+          const int x = A.cls_ab[ci];                    // Phi index = g xor x
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
             const int r = 2 * rr + e;
-            switch (x) {
-              case 0: o[e][0] = cfma(bv[e], phi[r][0], o[e][0]); o[e][1] = cfma(bv[e], phi[r][1], o[e][1]); o[e][2] = cfma(bv[e], phi[r][2], o[e][2]); o[e][3] = cfma(bv[e], phi[r][3], o[e][3]); break;
-              case 1: o[e][0] = cfma(bv[e], phi[r][1], o[e][0]); o[e][1] = cfma(bv[e], phi[r][0], o[e][1]); o[e][2] = cfma(bv[e], phi[r][3], o[e][2]); o[e][3] = cfma(bv[e], phi[r][2], o[e][3]); break;
-              case 2: o[e][0] = cfma(bv[e], phi[r][2], o[e][0]); o[e][1] = cfma(bv[e], phi[r][3], o[e][1]); o[e][2] = cfma(bv[e], phi[r][0], o[e][2]); o[e][3] = cfma(bv[e], phi[r][1], o[e][3]); break;
-              default: o[e][0] = cfma(bv[e], phi[r][3], o[e][0]); o[e][1] = cfma(bv[e], phi[r][2], o[e][1]); o[e][2] = cfma(bv[e], phi[r][1], o[e][2]); o[e][3] = cfma(bv[e], phi[r][0], o[e][3]); break;
-            }
+            // branch-free selection: the four targets are a permutation of phi[r][0..3] by xor with x
+            const bool x1 = x & 1, x2 = x & 2;
+            const float2 q0 = x1 ? phi[r][1] : phi[r][0], q1 = x1 ? phi[r][0] : phi[r][1];
+            const float2 q2 = x1 ? phi[r][3] : phi[r][2], q3 = x1 ? phi[r][2] : phi[r][3];
+            o[e][0] = cfma(bv[e], x2 ? q2 : q0, o[e][0]);
+            o[e][1] = cfma(bv[e], x2 ? q3 : q1, o[e][1]);
+            o[e][2] = cfma(bv[e], x2 ? q0 : q2, o[e][2]);
+            o[e][3] = cfma(bv[e], x2 ? q1 : q3, o[e][3]);
           }
         }
         // class g = 2 a + xb -> tile xb, rows (2 a + ri) * 32 + qy; the pair (qx0, qx0 + 1) is one 32-bit word of the row
-        const uint32_t sw = (uint32_t)(qy & 7);
-        const uint32_t off_hi = ((((uint32_t)qxp >> 2) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
-        const uint32_t off_lo = (((((uint32_t)qxp >> 2) + 4u) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
-          const uint32_t tile = smem_u32(A1) + (uint32_t)(g & 1) * ST_TILE;
+          const uint32_t rel = (uint32_t)(g & 1) * ST_TILE + (uint32_t)(((g >> 1) * 2) * 32 + 8 * rr) * 128u;
           uint32_t hi, lo;
-          split_f16x2(A.sQ * o[0][g].x, A.sQ * o[1][g].x, hi, lo);
-          uint32_t row = (uint32_t)(((g >> 1) * 2 + 0) * 32 + qy) * 128u;
-          st_shared_u32(tile + row + off_hi, hi);
-          st_shared_u32(tile + row + off_lo, lo);
-          split_f16x2(A.sQ * o[0][g].y, A.sQ * o[1][g].y, hi, lo);
-          row = (uint32_t)(((g >> 1) * 2 + 1) * 32 + qy) * 128u;
-          st_shared_u32(tile + row + off_hi, hi);
-          st_shared_u32(tile + row + off_lo, lo);
+          split_f16x2(o[0][g].x, o[1][g].x, hi, lo);
+          st_shared_u32(a1_hi + rel, hi);
+          st_shared_u32(a1_lo + rel, lo);
+          split_f16x2(o[0][g].y, o[1][g].y, hi, lo);
+          st_shared_u32(a1_hi + rel + 32 * 128, hi);
+          st_shared_u32(a1_lo + rel + 32 * 128, lo);
         }
       }
       fence_proxy_async_smem();
       tcgen05_fence_before();                            // (the previous component's TMEM reads of this lane are behind us)
       sl_bar(lane_id);
-      if (lt == 0) {
+      if (l == 0 && warp < 2) {                          // one issuing thread per accumulator tile: warp 0 -> x-even, warp 1 -> x-odd
         tcgen05_fence_after();
+        const int xb = warp;
+        const uint32_t d = tmem + c * 32 + xb * 16;
+        const uint32_t a = smem_u32(A1) + xb * ST_TILE, t = smem_u32(xy) + xb * 2048;
 #pragma unroll
-        for (int xb = 0; xb < 2; ++xb) {
-          const uint32_t d = tmem + c * 32 + xb * 16;
-          const uint32_t a = smem_u32(A1) + xb * ST_TILE, t = smem_u32(xy) + xb * 2048;
-#pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const uint32_t o = k * 32;
-            umma_f16(d, umma_desc_sw128(a + 64 + o), umma_desc_sw128(t + o), IDESC1, k == 0 ? 0u : 1u);   // lo x hi
-            umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + 64 + o), IDESC1, 1u);                 // hi x lo
-            umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + o), IDESC1, 1u);                      // hi x hi
-          }
+        for (int k = 0; k < 2; ++k) {
+          const uint32_t o = k * 32;
+          umma_f16(d, umma_desc_sw128(a + 64 + o), umma_desc_sw128(t + o), IDESC1, k == 0 ? 0u : 1u);   // lo x hi
+          umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + 64 + o), IDESC1, 1u);                 // hi x lo
+          umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + o), IDESC1, 1u);                      // hi x hi
         }
-        umma_commit(&mbar[lane_id]);
+        umma_commit(&mbar1[lane_id]);
       }
-      mbar_wait(&mbar[lane_id], ph);
-      ph ^= 1;
+      if (c > 0) finish(c - 1);
+      mbar_wait(&mbar1[lane_id], ph1);
+      ph1 ^= 1;
       tcgen05_fence_after();
+      if (c > 0) sl_bar(lane_id);                        // every warp is done reading the F buffer, which the drain overwrites
 
       // ---- drain D1: warp = chain (a, ri) of tile xb, lane = q_y; write T^T rows (class, ri, m_x), K = q_y ----
 #pragma unroll
@@ -494,8 +538,8 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
         uint32_t v[16];
         tmem_ld_32x32b_x16(tq + c * 32 + xb * 16, v);
         tmem_ld_wait();
-        const int chain8 = (((warp >> 1) * 2 + xb) * 2) + (warp & 1);
         // lane pairs exchange so that each lane owns two adjacent q_y of one row: even lanes row mxa, odd lanes row mxa + 4
+        const uint32_t dbase = a2_base + (uint32_t)xb * (2 * 16 * 128);        // chain8 = ((a 2 + xb) 2 + ri)
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const int mxa = (j & 3) + 8 * (j >> 2), mxb = mxa + 4;
@@ -503,14 +547,11 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
           const float send = (l & 1) ? va : vb;
           const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
           const float p0 = (l & 1) ? recv : va, p1 = (l & 1) ? vb : recv;      // (q_y even, q_y odd) of the lane's row
-          const int mx = (l & 1) ? mxb : mxa;
           uint32_t hi, lo;
           split_f16x2(p0, p1, hi, lo);
-          const uint32_t row = (uint32_t)(chain8 * 16 + mx);
-          const uint32_t w = (uint32_t)(l >> 1);                               // 32-bit word of the hi half: q_y pair
-          const uint32_t base = smem_u32(A2) + row * 128u;
-          st_shared_u32(base + ((((w >> 2)) ^ (row & 7u)) << 4) + ((w & 3u) << 2), hi);
-          st_shared_u32(base + ((((w >> 2) + 4u) ^ (row & 7u)) << 4) + ((w & 3u) << 2), lo);
+          const uint32_t addr = dbase + (uint32_t)mxa * 128u + a2_sw[j & 3];
+          st_shared_u32(addr, hi);
+          st_shared_u32(addr ^ 0x40u, lo);                                     // the lo half sits four 16-byte chunks on: bit 6 after the swizzle
         }
       }
       fence_proxy_async_smem();
@@ -527,41 +568,10 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
           umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + 64 + o), IDESC2, 1u);
           umma_f16(d, umma_desc_sw128(a + o), umma_desc_sw128(t + o), IDESC2, 1u);
         }
-        umma_commit(&mbar[lane_id]);
+        umma_commit(&mbar2[lane_id]);
       }
-      mbar_wait(&mbar[lane_id], ph);
-      ph ^= 1;
-      tcgen05_fence_after();
-
-      // ---- D2: warp = class (re rows 0..15, im rows 16..31 of the quarter), lane = (ri, m_x); its y-parity picks the column half ----
-      {
-        uint32_t v[16];
-        tmem_ld_32x32b_x16(tq + c * 32 + (warp >> 1) * 16, v);
-        tmem_ld_wait();
-        float *dst = Fb + (warp * 2 + (l >> 4)) * ST_FCH + (l & 15);
-#pragma unroll
-        for (int my = 0; my < 16; ++my) dst[my * 16] = __uint_as_float(v[my]);
-      }
-      tcgen05_fence_before();
-      sl_bar(lane_id);
-      // ---- butterfly + |E|^2 at the thread's two pixels of the quadrant ----
-      const float w = P.weight[c] * A.fs2;
-#pragma unroll
-      for (int i = 0; i < 2; ++i) {
-        const int px = lt + SL_THREADS * i;                // = my * 16 + mx
-        const float a0 = Fb[0 * ST_FCH + px], a1 = Fb[1 * ST_FCH + px], a2 = Fb[2 * ST_FCH + px], a3 = Fb[3 * ST_FCH + px];
-        const float a4 = Fb[4 * ST_FCH + px], a5 = Fb[5 * ST_FCH + px], a6 = Fb[6 * ST_FCH + px], a7 = Fb[7 * ST_FCH + px];
-        const float re0 = a0 - a3 - a5 - a6, im0 = a1 + a2 + a4 - a7;
-        const float re1 = a0 + a3 - a5 + a6, im1 = a1 - a2 + a4 + a7;
-        const float re2 = a0 - a3 + a5 + a6, im2 = a1 + a2 - a4 + a7;
-        const float re3 = a0 + a3 + a5 - a6, im3 = a1 - a2 - a4 - a7;
-        inten[i][0] = fmaf(w, re0 * re0 + im0 * im0, inten[i][0]);
-        inten[i][1] = fmaf(w, re1 * re1 + im1 * im1, inten[i][1]);
-        inten[i][2] = fmaf(w, re2 * re2 + im2 * im2, inten[i][2]);
-        inten[i][3] = fmaf(w, re3 * re3 + im3 * im3, inten[i][3]);
-      }
-      // (the next write of this buffer - the drain of the next component - is behind two more lane barriers)
     }
+    finish(P.C - 1);
 
     float *Ib = I + (size_t)b * M * M;
 #pragma unroll
@@ -604,7 +614,7 @@ bool sl_up(void **d, const std::vector<T> &h, long long *acc) {
 void smlm_free(psf_plan *p) {
   SmlmState *t = p->smlm;
   if (!t) return;
-  void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp, t->d_xy};
+  void *bufs[] = {t->d_bcls, t->d_xd, t->d_ktp, t->d_zbp, t->d_xy, t->d_bcls_tc};
   for (void *b : bufs)
     if (b) cudaFree(b);
   delete t;
@@ -737,7 +747,9 @@ psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted) {
     }
     const size_t fixed_tc = (size_t)ST_XY + (size_t)SL_NQ * SL_NQ * 8 + (size_t)ncls * SL_NQ * SL_NQ * 8 + (size_t)K * SL_NQ * SL_NQ * 4 + 1024 + 256;
     const int lanes_tc = (fixed_tc + 3 * (size_t)ST_LANE_BYTES <= limit) ? 3 : (fixed_tc + 2 * (size_t)ST_LANE_BYTES <= limit) ? 2 : 0;
-    if (lanes_tc && sl_up(&t->d_xy, xy, &p->upload_bytes)) {
+    std::vector<float2> bcls_s(bcls.size());
+    for (size_t i = 0; i < bcls.size(); ++i) bcls_s[i] = make_float2((float)(sQ * bcls[i].x), (float)(sQ * bcls[i].y));   // power of two: exact
+    if (lanes_tc && sl_up(&t->d_xy, xy, &p->upload_bytes) && sl_up(&t->d_bcls_tc, bcls_s, &p->upload_bytes)) {
       t->lanes_tc = lanes_tc;
       t->smem_tc = (int)(fixed_tc + lanes_tc * (size_t)ST_LANE_BYTES);
       e = lanes_tc == 3 ? cudaFuncSetAttribute(k_smlm_tc<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->smem_tc)
@@ -755,11 +767,11 @@ cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity) {
   const SmlmState *t = p->smlm;
   if (t->tc) {
     SmlmTcArgs T;
-    T.bcls = (const float2 *)t->d_bcls; T.xy = (const uint4 *)t->d_xy; T.ktp = (const float2 *)t->d_ktp; T.zbp = (const float *)t->d_zbp;
+    T.bcls = (const float2 *)t->d_bcls_tc; T.xy = (const uint4 *)t->d_xy; T.ktp = (const float2 *)t->d_ktp; T.zbp = (const float *)t->d_zbp;
     T.ncls = t->ncls; T.K = t->K;
     for (int i = 0; i < 6; ++i) T.comp_start[i] = t->comp_start[i];
     for (int i = 0; i < 12; ++i) T.cls_ab[i] = t->cls_ab[i];
-    T.sQ = t->sQ; T.f1 = t->f1; T.fs2 = t->fs2;
+    T.f1 = t->f1; T.fs2 = t->fs2;
     const int L = t->lanes_tc, per = (p->dp.Z + L - 1) / L;
     const int grid = per < p->sm_count ? per : p->sm_count;
     if (L == 3) k_smlm_tc<3><<<grid, SL_THREADS * 3, t->smem_tc, st>>>(p->dp, T, intensity);
