@@ -194,8 +194,9 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
  *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;
- *   PSF_TUNE_SMLM          : 1 (default) = small grids in per-plane mode (emitter batches) run the emitter-batch kernel k_smlm where
- *                            the plan qualifies; 0 = always k_small;
+ *   PSF_TUNE_SMLM          : 1 (default) = small grids in per-plane mode (emitter batches) run the emitter-batch kernels where the plan
+ *                            qualifies: k_smlm_tc (tcgen05; output half-size <= 16, precision AUTO or 3XF16), else k_smlm (fp32 FMA);
+ *                            2 = k_smlm, never the tensor-core variant; 0 = always k_small;
  *   PSF_TUNE_K1P_ASPLIT    : 1 (default) = in the stage-1 pair kernel the TMA-written table half of a stage buffer has its own barrier and
  *                            is released right behind its own stage (only the producer-written half needs the deferred release);
  *                            0 = one barrier for both halves (round 1);
@@ -225,7 +226,9 @@ const char *psf_last_error(const psf_plan *plan);
 int psf_launches_per_compute(const psf_plan *plan);
 
 /* Name of the kernel path the plan selected (static string): "ffma" (fp32 FFMA tiles), "ffma_fused" (small grids: the
- * whole path in one CTA per plane), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision), "czt_fft" (chirp-Z by FFT). */
+ * whole path in one kernel, fp32 FMA: k_small, k_smlm), "fused_tc3xf16" (emitter batches on small grids: the whole path in one
+ * kernel with both DFT stages on tcgen05, 3xFP16 split: k_smlm_tc), "tc3xtf32", "tc3xf16" (tcgen05 tensor cores, split precision,
+ * one kernel per stage or both in k12_fused), "czt_fft" (chirp-Z by FFT). */
 const char *psf_path_name(const psf_plan *plan);
 
 /* Comma-separated names of the kernels one psf_compute of this plan launches, in launch order (stage 1, stage 2; one

@@ -655,7 +655,7 @@ int psf_launches_per_compute(const psf_plan *p) {
   return (p->path >= 1 && p->tc) ? tc_launches(p) : ffma_launches(p);
 }
 
-const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 4 ? "czt_fft" : p->path == 3 ? "ffma_fused" : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
+const char *psf_path_name(const psf_plan *p) { return !p ? "ffma" : p->path == 4 ? "czt_fft" : p->path == 3 ? (smlm_on_tensor_cores(p) ? "fused_tc3xf16" : "ffma_fused") : p->path == 2 ? "tc3xf16" : p->path == 1 ? "tc3xtf32" : "ffma"; }
 
 psf_status psf_profile_enable(psf_plan *p, int enable) {
   if (!p) return PSF_ERR_INVALID_ARG;

@@ -392,10 +392,12 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
         pcl[r][1] = pcl[r][2] = pcl[r][3] = 0.f;
       }
       int j = 0;
+      float cnext = cfs[0];
 #pragma unroll
       for (int cls = 0; cls < 4; ++cls)
         for (int e = j + P.zcnt[cls]; j < e; ++j) {
-          const float cj = cfs[j];
+          const float cj = cnext;
+          cnext = cfs[j + 1];                              // (one past the row at the end: the buffer has 16 floats)
           const float *zb = zbs + j * (SL_NQ * SL_NQ) + qyb * SL_NQ + qx0;
 #pragma unroll
           for (int rr = 0; rr < 4; ++rr) {
@@ -482,19 +484,20 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
         for (int ci = c0; ci < c1; ++ci) {
           const float4 b2 = *reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + (qyb + 8 * rr) * SL_NQ + qx0]);
           const float2 bv[2] = {make_float2(b2.x, b2.y), make_float2(b2.z, b2.w)};
-          const int x = A.cls_ab[ci];                    // Phi index = g xor x
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int r = 2 * rr + e;
-            // branch-free selection: the four targets are a permutation of phi[r][0..3] by xor with x
-            const bool x1 = x & 1, x2 = x & 2;
-            const float2 q0 = x1 ? phi[r][1] : phi[r][0], q1 = x1 ? phi[r][0] : phi[r][1];
-            const float2 q2 = x1 ? phi[r][3] : phi[r][2], q3 = x1 ? phi[r][2] : phi[r][3];
-            o[e][0] = cfma(bv[e], x2 ? q2 : q0, o[e][0]);
-            o[e][1] = cfma(bv[e], x2 ? q3 : q1, o[e][1]);
-            o[e][2] = cfma(bv[e], x2 ? q0 : q2, o[e][2]);
-            o[e][3] = cfma(bv[e], x2 ? q1 : q3, o[e][3]);
+          // Phi index = g xor x; x is uniform: one branch per (q_y group, class), static register indices in every arm
+#define SL_ACC(i0, i1, i2, i3)                                                                                     \
+  _Pragma("unroll") for (int e = 0; e < 2; ++e) {                                                                  \
+    const int r = 2 * rr + e;                                                                                      \
+    o[e][0] = cfma(bv[e], phi[r][i0], o[e][0]); o[e][1] = cfma(bv[e], phi[r][i1], o[e][1]);                        \
+    o[e][2] = cfma(bv[e], phi[r][i2], o[e][2]); o[e][3] = cfma(bv[e], phi[r][i3], o[e][3]);                        \
+  }
+          switch (A.cls_ab[ci]) {
+            case 0: SL_ACC(0, 1, 2, 3) break;
+            case 1: SL_ACC(1, 0, 3, 2) break;
+            case 2: SL_ACC(2, 3, 0, 1) break;
+            default: SL_ACC(3, 2, 1, 0) break;
           }
+#undef SL_ACC
         }
         // class g = 2 a + xb -> tile xb, rows (2 a + ri) * 32 + qy; the pair (qx0, qx0 + 1) is one 32-bit word of the row
 #pragma unroll

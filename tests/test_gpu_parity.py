@@ -580,15 +580,25 @@ def test_fused_launch_matches_the_two_kernel_path_bit_for_bit(psf):
     (407, 64, 32, 6, W.POL_X, {"fresnel": True, "envelope_s": 0.7}),
 ])
 def test_emitter_batch_kernel(psf, seed, N, M, Z, pol, kw):
-    """k_smlm (kernels_smlm.cu): per-plane Zernike rows + shifts on small even grids, against the fp64 oracle, and bit-level
-    agreement is not expected with k_small (different association), so both are checked against the oracle."""
+    """The emitter-batch kernels (kernels_smlm.cu): per-plane Zernike rows + shifts on small even grids, against the fp64 oracle.
+    Output quadrants of at most 16 x 16 pixels run k_smlm_tc (both DFT stages on tcgen05, 3xFP16 split), wider ones k_smlm
+    (packed fp32 FMA); PSF_TUNE_SMLM = 2 selects k_smlm everywhere, 0 the one-CTA-per-plane kernel k_small.  The three
+    associate differently, so each is checked against the oracle, not against the others."""
     import torch
     case = replace(W.small_random_case(seed, pupil_n=N, out_m=M, n_planes=Z, pol=pol), **kw)
     ref = O.stack_T2(case)
     plan = psf.plan_from_case(case)
-    assert plan.kernel_names == ["k_smlm"], plan.kernel_names
+    tensor = (M + 1) // 2 <= 16
+    assert plan.kernel_names == (["k_smlm_tc"] if tensor else ["k_smlm"]), plan.kernel_names
     I = plan.compute().cpu().numpy().astype(np.float64)
     assert plane_errors(I, ref).max() <= TOL, plane_errors(I, ref)
+    if tensor:
+        again = plan.compute().cpu().numpy()
+        assert np.array_equal(again, I.astype(np.float32))          # no atomics, no order dependence: same bits call after call
+        plan.tune(psf.TUNE_SMLM, 2)
+        assert plan.kernel_names == ["k_smlm"]
+        I1 = plan.compute().cpu().numpy().astype(np.float64)
+        assert plane_errors(I1, ref).max() <= TOL
     plan.tune(psf.TUNE_SMLM, 0)
     assert plan.kernel_names == ["k_small"]
     I0 = plan.compute().cpu().numpy().astype(np.float64)

@@ -53,7 +53,8 @@ def test_config1_fused_small_grid_kernel(psf):
 
 def test_config4_fused_small_grid_kernel_per_plane_mode(psf):
     """config 4 (96 of its 4096 emitters): k_small, per-plane Zernike rows and shifts."""
-    _check(psf, W.config4().with_planes(np.arange(0, 4096, 43)), "auto", ["k_smlm"])
+    _check(psf, W.config4().with_planes(np.arange(0, 4096, 43)), "auto", ["k_smlm_tc"])
+    _check(psf, W.config4().with_planes(np.arange(0, 4096, 43)), "auto", ["k_smlm"], tune=(psf.TUNE_SMLM, 2))
     _check(psf, W.config4().with_planes(np.arange(0, 4096, 43)), "auto", ["k_small"], tune=(psf.TUNE_SMLM, 0))
 
 
