@@ -108,38 +108,50 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, 
     sl_bar(lane_id);
 
     // ---- phase 0: the parity transform Phi_g of the emitter's phasor field, 8 folded samples per thread, in registers ----
+    // (term loops outermost, the thread's 8 samples inside: 8 independent FMA chains per shared-memory round trip)
     float2 phi[8][4];
+    {
+      float pcl[8][4];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      const int f = lt + SL_THREADS * r;
-      const int qy = f >> 5, qx = f & 31;
-      float pcl[4] = {kz_turns(kts[f], pl.x, pl.y), 0.f, 0.f, 0.f};     // phase parts: even/even, x-odd, y-odd, odd/odd (turns)
-      {
-        int j = 0;
-        for (int e = P.zcnt[0]; j < e; ++j) pcl[0] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[0]);
-        for (int e = j + P.zcnt[1]; j < e; ++j) pcl[1] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[1]);
-        for (int e = j + P.zcnt[2]; j < e; ++j) pcl[2] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[2]);
-        for (int e = j + P.zcnt[3]; j < e; ++j) pcl[3] = fmaf(cfs[j], zbs[j * (SL_NQ * SL_NQ) + f], pcl[3]);
+      for (int r = 0; r < 8; ++r) {
+        pcl[r][0] = kz_turns(kts[lt + SL_THREADS * r], pl.x, pl.y);     // phase parts: even/even, x-odd, y-odd, odd/odd (turns)
+        pcl[r][1] = pcl[r][2] = pcl[r][3] = 0.f;
       }
-      if (P.has_shift) {
-        const float ux = (float)(2 * qx + 1 - N) / (float)N, uy = (float)(2 * qy + 1 - N) / (float)N;
-        pcl[1] = fmaf(-ux, pl.z, pcl[1]);
-        pcl[2] = fmaf(-uy, pl.w, pcl[2]);
-      }
-      float2 e[4];
+      int j = 0;
+      float cnext = cfs[0];
 #pragma unroll
-      for (int a = 0; a < 2; ++a)
+      for (int cls = 0; cls < 4; ++cls)
+        for (int e = j + P.zcnt[cls]; j < e; ++j) {
+          const float cj = cnext;
+          cnext = cfs[j + 1];                              // (one past the row at the end: the buffer has 16 floats)
+          const float *zb = zbs + j * (SL_NQ * SL_NQ) + lt;
 #pragma unroll
-        for (int bb = 0; bb < 2; ++bb) {
-          const float sx = bb ? -1.f : 1.f, sy = a ? -1.f : 1.f;
-          sl_sincos_turns(pcl[0] + sx * pcl[1] + sy * pcl[2] + sx * sy * pcl[3], e[a * 2 + bb].y, e[a * 2 + bb].x);
+          for (int r = 0; r < 8; ++r) pcl[r][cls] = fmaf(cj, zb[SL_THREADS * r], pcl[r][cls]);
         }
-      const float2 s01 = make_float2(e[0].x + e[1].x, e[0].y + e[1].y), d01 = make_float2(e[0].x - e[1].x, e[0].y - e[1].y);
-      const float2 s23 = make_float2(e[2].x + e[3].x, e[2].y + e[3].y), d23 = make_float2(e[2].x - e[3].x, e[2].y - e[3].y);
-      phi[r][0] = make_float2(s01.x + s23.x, s01.y + s23.y);      // sigma = 1
-      phi[r][1] = make_float2(d01.x + d23.x, d01.y + d23.y);      // sigma = s_x
-      phi[r][2] = make_float2(s01.x - s23.x, s01.y - s23.y);      // sigma = s_y
-      phi[r][3] = make_float2(d01.x - d23.x, d01.y - d23.y);      // sigma = s_x s_y
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int f = lt + SL_THREADS * r;
+        const int qy = f >> 5, qx = f & 31;
+        if (P.has_shift) {
+          const float ux = (float)(2 * qx + 1 - N) / (float)N, uy = (float)(2 * qy + 1 - N) / (float)N;
+          pcl[r][1] = fmaf(-ux, pl.z, pcl[r][1]);
+          pcl[r][2] = fmaf(-uy, pl.w, pcl[r][2]);
+        }
+        float2 e[4];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+          for (int bb = 0; bb < 2; ++bb) {
+            const float sx = bb ? -1.f : 1.f, sy = a ? -1.f : 1.f;
+            sl_sincos_turns(pcl[r][0] + sx * pcl[r][1] + sy * pcl[r][2] + sx * sy * pcl[r][3], e[a * 2 + bb].y, e[a * 2 + bb].x);
+          }
+        const float2 s01 = make_float2(e[0].x + e[1].x, e[0].y + e[1].y), d01 = make_float2(e[0].x - e[1].x, e[0].y - e[1].y);
+        const float2 s23 = make_float2(e[2].x + e[3].x, e[2].y + e[3].y), d23 = make_float2(e[2].x - e[3].x, e[2].y - e[3].y);
+        phi[r][0] = make_float2(s01.x + s23.x, s01.y + s23.y);      // sigma = 1
+        phi[r][1] = make_float2(d01.x + d23.x, d01.y + d23.y);      // sigma = s_x
+        phi[r][2] = make_float2(s01.x - s23.x, s01.y - s23.y);      // sigma = s_y
+        phi[r][3] = make_float2(d01.x - d23.x, d01.y - d23.y);      // sigma = s_x s_y
+      }
     }
 
     float inten[PASS2][2][4];
