@@ -349,8 +349,9 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   float *cf_all = zbs + (size_t)A.K * SL_NQ * SL_NQ;
   __shared__ uint64_t mbar1[LANES], mbar2[LANES];
   __shared__ uint32_t tmem_slot;
-  const int lane_id = threadIdx.x / SL_THREADS, lt = threadIdx.x % SL_THREADS;
-  const int warp = lt >> 5, l = lt & 31;
+  // warp-uniform by construction (the broadcast tells the compiler so: addresses and descriptors derived from them stay in uniform registers)
+  const int wu = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+  const int lane_id = wu >> 2, warp = wu & 3, lt = threadIdx.x % SL_THREADS, l = threadIdx.x & 31;
   uint8_t *A1 = smem + ST_XY + lane_id * ST_LANE_BYTES, *A2 = A1 + 2 * ST_TILE;
   float *Fb = reinterpret_cast<float *>(A2);
   float *cfs = cf_all + lane_id * 16;
@@ -527,7 +528,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       fence_proxy_async_smem();
       tcgen05_fence_before();                            // (the previous component's TMEM reads of this lane are behind us)
       sl_bar(lane_id);
-      if (l == 0 && warp < 2) {                          // one issuing thread per accumulator tile: warp 0 -> x-even, warp 1 -> x-odd
+      if (warp < 2 && elect_one()) {                     // one issuing thread per accumulator tile: warp 0 -> x-even, warp 1 -> x-odd
         tcgen05_fence_after();
         const int xb = warp;
         const uint32_t d = tmem + c * 32 + xb * 16;
@@ -572,7 +573,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       fence_proxy_async_smem();
       tcgen05_fence_before();
       sl_bar(lane_id);
-      if (lt == 0) {
+      if (warp == 0 && elect_one()) {
         tcgen05_fence_after();
         const uint32_t d = tmem + c * 32;
         const uint32_t a = smem_u32(A2), t = smem_u32(xy);
