@@ -219,7 +219,7 @@ enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDO
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /
- * psf_host_tables.  Never NULL; valid until the next call on the same plan / thread. */
+ * psf_host_tables / psf_propagate_static.  Never NULL; valid until the next call on the same plan / thread. */
 const char *psf_last_error(const psf_plan *plan);
 
 /* Number of kernel launches one psf_compute call of this plan enqueues (for benchmarking records). */
@@ -249,6 +249,30 @@ psf_status psf_profile_read(psf_plan *plan, float *stage_ms, int *launches);
 
 /* Bytes copied host->device by the last psf_plan_create / psf_set_zernike / psf_set_shifts of this plan. */
 long long psf_last_upload_bytes(const psf_plan *plan);
+
+/* The zoomed Fourier sum of PAPER.md:116 Eq. 9 WITHOUT a plan and without any allocation, for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it; psf_plan_create allocates):
+ *   E_c[z][my][mx] = sum_{py,px} pupil[z][c][py][px] exp(+i k s_max (u_px x_mx + u_py y_my)),   I[z] = sum_c weights[c] |E_c[z]|^2,
+ *   u_p = (2p + 1 - N)/N, x_m = (m - (M-1)/2) pixel_um, k s_max = 2 pi NA / wavelength_um (readings A4, A6, A9).
+ * The caller passes everything: `pupil` = DEVICE float2 [n_planes][n_components][pupil_n][pupil_n] (row = p_y), the complete
+ * pupil field of every plane with every phase, prefactor and quadrature weight in it (e.g. psf_host_tables' base times
+ * exp(i kappa z)), 8-byte aligned; `weights` = HOST float [n_components], read before the call returns; `intensity` = DEVICE
+ * float [n_planes][out_m][out_m], written in stream order.  fp32 complex products (two kernels: rows, then columns with |E|^2
+ * in the epilogue); the row -> column scratch and the DFT table live in a file-scope `static __device__` array of
+ * PSF_STATIC_SCRATCH_BYTES that every GPU using this entry point holds until the process exits.
+ * Limit: (n_components + 1) * out_m * pupil_n * 8 bytes (the table's share rounded up to 256) must fit the array, e.g. three
+ * components at 512 x 512 or five at 256 x 512; n_planes is free (planes go through in passes that fit).  Larger sizes return PSF_ERR_UNSUPPORTED with the byte counts
+ * in psf_last_error(NULL); nothing is launched.  n_components is 1..5.
+ * The call only enqueues kernels on `cuda_stream` (NULL = the legacy default stream) of the CURRENT device: no cudaMalloc, cudaFree,
+ * copy or synchronisation.  The first call on a device looks the array's device address up (cudaGetSymbolAddress, once per
+ * device): make one call outside a stream capture first.
+ * All calls on a device share the array, which keeps the last call's contents (nothing in it needs clearing: every call rewrites
+ * what it reads).  Calls that overlap on the GPU - two streams, or two host threads on one device - race on it: serialise them
+ * (one stream, or events).  Errors: PSF_ERR_INVALID_ARG (NULL / misaligned pointers, non-positive sizes or optics, non-finite
+ * weights), PSF_ERR_UNSUPPORTED (too large), PSF_ERR_CUDA; the message is psf_last_error(NULL) of the calling thread. */
+#define PSF_STATIC_SCRATCH_BYTES (16u << 20)
+psf_status psf_propagate_static(void *cuda_stream, const void *pupil, int n_planes, int n_components, int pupil_n, int out_m,
+                                double NA, double wavelength_um, double pixel_um, const float *weights, float *intensity);
 
 /* Host-only diagnostic (no device needed): the plan-time static pupil in fp64, before folding and rounding.
  *   n_components : out, 3 (coherent input), 5 (unpolarised: the distinct scalar pupils a, b, d, c_x, c_y) or 1 (scalar);

@@ -21,7 +21,8 @@ PREC = {"auto": 0, "3xtf32": 1, "fp32": 2, "3xf16": 3, "czt_fft": 4}
 EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phase_mask", "psf_compute", "psf_plan_destroy",
            "psf_spherical_prepare", "psf_compute_spherical", "psf_gradients",
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
-           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names", "psf_grad_path_name"]
+           "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names", "psf_grad_path_name",
+           "psf_propagate_static"]
 TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER, TUNE_TC_FUSED, TUNE_SMLM, TUNE_GRAD_TENSOR, TUNE_K1P_ASPLIT, TUNE_FUSED_WINDOW, TUNE_DEVICE_REFRESH, TUNE_PDL = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 
 
@@ -103,6 +104,9 @@ def load_library(build_if_missing: bool = True):
                                     C.POINTER(C.c_int), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double), C.POINTER(C.c_ubyte)]
     lib.psf_host_tables.restype = C.c_int
+    lib.psf_propagate_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                         C.c_double, C.POINTER(C.c_float), C.c_void_p]
+    lib.psf_propagate_static.restype = C.c_int
     _lib = lib
     return lib
 
@@ -302,6 +306,37 @@ def plan_from_case(case, device: int = 0, precision: str = "auto") -> PsfPlan:
     if getattr(case, "phase_mask", None) is not None:
         plan.set_phase_mask(case.phase_mask)
     return plan
+
+
+STATIC_SCRATCH_BYTES = 16 << 20
+
+
+def propagate_static(pupil, out_m: int, NA: float, wavelength_um: float, pixel_um: float, weights, intensity, stream=None):
+    """psf_propagate_static: pupil = CUDA complex64 (or float32 [..., 2]) tensor [Z, C, N, N], intensity = CUDA float32 tensor
+    [Z, out_m, out_m] that the CALLER provides (the entry point allocates nothing, and neither does this wrapper)."""
+    import torch
+    lib = load_library()
+    if pupil.dtype == torch.complex64:
+        Z, Cn, N, N2 = pupil.shape
+    else:
+        Z, Cn, N, N2, two = pupil.shape
+        if two != 2 or pupil.dtype != torch.float32:
+            raise ValueError("pupil must be complex64 [Z, C, N, N] or float32 [Z, C, N, N, 2]")
+    if N != N2 or not pupil.is_cuda or not pupil.is_contiguous():
+        raise ValueError("pupil must be a contiguous CUDA tensor [Z, C, N, N]")
+    if tuple(intensity.shape) != (Z, out_m, out_m) or intensity.dtype != torch.float32 or not intensity.is_cuda or \
+            not intensity.is_contiguous() or intensity.device != pupil.device:
+        raise ValueError("intensity must be a contiguous CUDA float32 tensor [Z, out_m, out_m] on the pupil's device")
+    w = np.ascontiguousarray(np.asarray(weights, dtype=np.float32))
+    if w.shape != (Cn,):
+        raise ValueError("weights must have one entry per component")
+    with torch.cuda.device(pupil.device):
+        s = torch.cuda.current_stream(pupil.device) if stream is None else stream
+        st = lib.psf_propagate_static(C.c_void_p(s.cuda_stream), C.c_void_p(pupil.data_ptr()), int(Z), int(Cn), int(N), int(out_m),
+                                      float(NA), float(wavelength_um), float(pixel_um), _fptr(w), C.c_void_p(intensity.data_ptr()))
+    if st != PSF_OK:
+        raise PsfError(st, lib.psf_last_error(None).decode())
+    return intensity
 
 
 def host_tables(case, shared_coeffs=None, noll_first: int = 4):

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpsf_b200.so")
-SOURCES = ["api.cu", "kernels_ffma.cu", "kernels_small.cu", "kernels_smlm.cu", "kernels_tc.cu", "kernels_czt.cu", "kernels_bessel.cu", "kernels_grad.cu", "host_tables.cpp"]
+SOURCES = ["api.cu", "kernels_ffma.cu", "kernels_small.cu", "kernels_smlm.cu", "kernels_tc.cu", "kernels_czt.cu", "kernels_bessel.cu", "kernels_grad.cu", "noalloc.cu", "host_tables.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xcompiler", "-fopenmp", "--shared", "-cudart", "static"]
 

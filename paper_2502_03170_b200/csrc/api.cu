@@ -336,6 +336,9 @@ void free_all(psf_plan *p) {
 }  // namespace
 
 namespace psf {
+// for entry points without a plan in other files (noalloc.cu): the message psf_last_error(NULL) returns on this thread
+void set_thread_error(const char *msg) noexcept { set_err(nullptr, msg); }
+
 const std::vector<cplx> &host_base(psf_plan *p) {
   if (p->host_base_stale) {
     apply_shared_zernike(p->hp0, p->zern_shared.empty() ? nullptr : p->zern_shared.data(), (int)p->zern_shared.size(), p->zbasis,
