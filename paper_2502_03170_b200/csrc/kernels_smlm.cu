@@ -45,7 +45,7 @@ struct SmlmState {
   void *d_bcls_tc = nullptr;   // the class tables times the operand scale s_Q
   void *d_xy = nullptr;        // 4096 bytes: the cos | sin table as the UMMA B operand (fp16 hi | lo rows, swizzled)
   int smem_tc = 0, lanes_tc = 0;
-  float sQ = 1.f, f1 = 1.f, fs2 = 1.f;
+  float sQ = 1.f, fs2 = 1.f;
 };
 
 namespace {
@@ -332,7 +332,6 @@ struct SmlmTcArgs {
   int ncls, K;
   int comp_start[6];
   int cls_ab[12];
-  float f1;                   // s_T / (s_Q s_X): D1 -> stage-2 operand
   float fs2;                  // (1 / (s_T s_X))^2: |D2|^2 -> |F|^2
 };
 
@@ -373,19 +372,20 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   const uint32_t tq = tmem + ((uint32_t)(warp * 32) << 16);
 
   const int m = P.m, M = P.M, N = P.N, K = A.K;
-  // generation: a thread owns two adjacent q_x at four q_y; the half-warps sit four rows apart (different swizzle phase)
-  const int qxp = lt & 15, qx0 = 2 * qxp, qyb = warp + 4 * ((lt >> 4) & 1);
+  // generation: a thread owns four adjacent q_x (8 bytes of a row's hi half, 8 of its lo half) at two q_y, 16 rows apart; the
+  // quarter-warps of a warp sit four rows apart, so a half-warp's 8-byte stores cover all 32 banks once (rows r and r + 4 swizzle
+  // into different halves of the 128-byte row)
+  const int qxq = l & 7, qx0 = 4 * qxq, qyb = warp + 4 * (l >> 3);
   uint32_t ph1 = 0, ph2 = 0;
   // operand addresses of the thread's stores: the swizzle phase (q_y & 7) and the word inside the row do not change over the 4 q_y
   const uint32_t sw = (uint32_t)(qyb & 7);
-  const uint32_t off_hi = ((((uint32_t)qxp >> 2) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
-  const uint32_t off_lo = (((((uint32_t)qxp >> 2) + 4u) ^ sw) << 4) + (((uint32_t)qxp & 3u) << 2);
+  const uint32_t off_hi = ((((uint32_t)qxq >> 1) ^ sw) << 4) + (((uint32_t)qxq & 1u) << 3);     // the lo half sits at off_hi ^ 0x40
   // drain stores: row = chain8 * 16 + m_x with m_x = mxa + 4 (lane & 1); the row's swizzle phase is m_x & 7 = (j & 3) + 4 (lane & 1)
   const uint32_t a2_base = smem_u32(A2) + (uint32_t)((((warp >> 1) * 4 + (warp & 1)) * 16 + 4 * (l & 1)) * 128) + (((uint32_t)(l >> 1) & 3u) << 2);
   uint32_t a2_sw[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) a2_sw[k] = ((((uint32_t)l >> 3) ^ (uint32_t)(k + 4 * (l & 1))) << 4);
-  const uint32_t a1_hi = smem_u32(A1) + (uint32_t)qyb * 128u + off_hi, a1_lo = smem_u32(A1) + (uint32_t)qyb * 128u + off_lo;
+  const uint32_t a1_hi = smem_u32(A1) + (uint32_t)qyb * 128u + off_hi;
 
   for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
     const float4 pl = __ldg(P.planes + b);
@@ -400,7 +400,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       float pcl[8][4];
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
-        const int f = (qyb + 8 * (r >> 1)) * SL_NQ + qx0 + (r & 1);
+        const int f = (qyb + 16 * (r >> 2)) * SL_NQ + qx0 + (r & 3);
         pcl[r][0] = kz_turns(kts[f], pl.x, pl.y);
         pcl[r][1] = pcl[r][2] = pcl[r][3] = 0.f;
       }
@@ -413,15 +413,17 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
           cnext = cfs[j + 1];                              // (one past the row at the end: the buffer has 16 floats)
           const float *zb = zbs + j * (SL_NQ * SL_NQ) + qyb * SL_NQ + qx0;
 #pragma unroll
-          for (int rr = 0; rr < 4; ++rr) {
-            const float2 z2 = *reinterpret_cast<const float2 *>(zb + 8 * rr * SL_NQ);
-            pcl[2 * rr][cls] = fmaf(cj, z2.x, pcl[2 * rr][cls]);
-            pcl[2 * rr + 1][cls] = fmaf(cj, z2.y, pcl[2 * rr + 1][cls]);
+          for (int rr = 0; rr < 2; ++rr) {
+            const float4 z4 = *reinterpret_cast<const float4 *>(zb + 16 * rr * SL_NQ);
+            pcl[4 * rr][cls] = fmaf(cj, z4.x, pcl[4 * rr][cls]);
+            pcl[4 * rr + 1][cls] = fmaf(cj, z4.y, pcl[4 * rr + 1][cls]);
+            pcl[4 * rr + 2][cls] = fmaf(cj, z4.z, pcl[4 * rr + 2][cls]);
+            pcl[4 * rr + 3][cls] = fmaf(cj, z4.w, pcl[4 * rr + 3][cls]);
           }
         }
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
-        const int qy = qyb + 8 * (r >> 1), qx = qx0 + (r & 1);
+        const int qy = qyb + 16 * (r >> 2), qx = qx0 + (r & 3);
         if (P.has_shift) {
           const float ux = (float)(2 * qx + 1 - N) / (float)N, uy = (float)(2 * qy + 1 - N) / (float)N;
           pcl[r][1] = fmaf(-ux, pl.z, pcl[r][1]);
@@ -491,16 +493,18 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       // ---- Q_g = sum_ab B_ab Phi_(g xor ab), scaled, split, into the two stage-1 operand tiles ----
       const int c0 = A.comp_start[c], c1 = A.comp_start[c + 1];
 #pragma unroll
-      for (int rr = 0; rr < 4; ++rr) {
-        float2 o[2][4];
-        o[0][0] = o[0][1] = o[0][2] = o[0][3] = o[1][0] = o[1][1] = o[1][2] = o[1][3] = make_float2(0.f, 0.f);
+      for (int rr = 0; rr < 2; ++rr) {
+        float2 o[4][4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) o[e][0] = o[e][1] = o[e][2] = o[e][3] = make_float2(0.f, 0.f);
         for (int ci = c0; ci < c1; ++ci) {
-          const float4 b2 = *reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + (qyb + 8 * rr) * SL_NQ + qx0]);
-          const float2 bv[2] = {make_float2(b2.x, b2.y), make_float2(b2.z, b2.w)};
-          // Phi index = g xor x; x is uniform: one branch per (q_y group, class), static register indices in every arm
+          const float4 *bp = reinterpret_cast<const float4 *>(&bcl[ci * (SL_NQ * SL_NQ) + (qyb + 16 * rr) * SL_NQ + qx0]);
+          const float4 b01 = bp[0], b23 = bp[1];
+          const float2 bv[4] = {make_float2(b01.x, b01.y), make_float2(b01.z, b01.w), make_float2(b23.x, b23.y), make_float2(b23.z, b23.w)};
+          // Phi index = g xor x; x is uniform: one branch per (q_y row, class), static register indices in every arm
 #define SL_ACC(i0, i1, i2, i3)                                                                                     \
-  _Pragma("unroll") for (int e = 0; e < 2; ++e) {                                                                  \
-    const int r = 2 * rr + e;                                                                                      \
+  _Pragma("unroll") for (int e = 0; e < 4; ++e) {                                                                  \
+    const int r = 4 * rr + e;                                                                                      \
     o[e][0] = cfma(bv[e], phi[r][i0], o[e][0]); o[e][1] = cfma(bv[e], phi[r][i1], o[e][1]);                        \
     o[e][2] = cfma(bv[e], phi[r][i2], o[e][2]); o[e][3] = cfma(bv[e], phi[r][i3], o[e][3]);                        \
   }
@@ -512,17 +516,19 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
           }
 #undef SL_ACC
         }
-        // class g = 2 a + xb -> tile xb, rows (2 a + ri) * 32 + qy; the pair (qx0, qx0 + 1) is one 32-bit word of the row
+        // class g = 2 a + xb -> tile xb, rows (2 a + ri) * 32 + qy; the four q_x are two 32-bit words of the row's hi half, two of its lo half
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
-          const uint32_t rel = (uint32_t)(g & 1) * ST_TILE + (uint32_t)(((g >> 1) * 2) * 32 + 8 * rr) * 128u;
-          uint32_t hi, lo;
-          split_f16x2(o[0][g].x, o[1][g].x, hi, lo);
-          st_shared_u32(a1_hi + rel, hi);
-          st_shared_u32(a1_lo + rel, lo);
-          split_f16x2(o[0][g].y, o[1][g].y, hi, lo);
-          st_shared_u32(a1_hi + rel + 32 * 128, hi);
-          st_shared_u32(a1_lo + rel + 32 * 128, lo);
+          const uint32_t at = a1_hi + (uint32_t)(g & 1) * ST_TILE + (uint32_t)(((g >> 1) * 2) * 32 + 16 * rr) * 128u;
+          uint32_t h0, l0, h1, l1;
+          split_f16x2(o[0][g].x, o[1][g].x, h0, l0);
+          split_f16x2(o[2][g].x, o[3][g].x, h1, l1);
+          st_shared_v2_u32(at, h0, h1);
+          st_shared_v2_u32(at ^ 0x40u, l0, l1);
+          split_f16x2(o[0][g].y, o[1][g].y, h0, l0);
+          split_f16x2(o[2][g].y, o[3][g].y, h1, l1);
+          st_shared_v2_u32(at + 32 * 128, h0, h1);
+          st_shared_v2_u32((at + 32 * 128) ^ 0x40u, l0, l1);
         }
       }
       fence_proxy_async_smem();
@@ -559,7 +565,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const int mxa = (j & 3) + 8 * (j >> 2), mxb = mxa + 4;
-          const float va = A.f1 * __uint_as_float(v[mxa]), vb = A.f1 * __uint_as_float(v[mxb]);
+          const float va = __uint_as_float(v[mxa]), vb = __uint_as_float(v[mxb]);
           const float send = (l & 1) ? va : vb;
           const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
           const float p0 = (l & 1) ? recv : va, p1 = (l & 1) ? vb : recv;      // (q_y even, q_y odd) of the lane's row
@@ -741,9 +747,9 @@ psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted) {
         rmax = std::max(rmax, rs);
       }
     auto pow2 = [](double v, double limit) { return v > 0 ? std::exp2(std::floor(std::log2(limit / v))) : 1.0; };
-    const double sQ = pow2(qmax, 16384.0), sT = pow2(rmax, 32768.0), sX = (double)ST_XSCALE;
+    // s_Q so that the stage-1 accumulator s_Q s_X T is the stage-2 operand as it stands (|s_Q s_X T| <= 2^15): no rescaling in the drain
+    const double sX = (double)ST_XSCALE, sQ = std::min(pow2(qmax, 16384.0), pow2(rmax, 32768.0 / sX)), sT = sQ * sX;
     t->sQ = (float)sQ;
-    t->f1 = (float)(sT / (sQ * sX));
     t->fs2 = (float)((1.0 / (sT * sX)) * (1.0 / (sT * sX)));
     std::vector<__half> xy((size_t)ST_XY / 2, __float2half_rn(0.f));
     for (int row = 0; row < 32; ++row) {
@@ -787,7 +793,7 @@ cudaError_t launch_smlm(const psf_plan *p, cudaStream_t st, float *intensity) {
     T.ncls = t->ncls; T.K = t->K;
     for (int i = 0; i < 6; ++i) T.comp_start[i] = t->comp_start[i];
     for (int i = 0; i < 12; ++i) T.cls_ab[i] = t->cls_ab[i];
-    T.f1 = t->f1; T.fs2 = t->fs2;
+    T.fs2 = t->fs2;
     const int L = t->lanes_tc, per = (p->dp.Z + L - 1) / L;
     const int grid = per < p->sm_count ? per : p->sm_count;
     if (L == 3) k_smlm_tc<3><<<grid, SL_THREADS * 3, t->smem_tc, st>>>(p->dp, T, intensity);

@@ -194,6 +194,7 @@ __device__ __forceinline__ void split_f16x2(float a, float b, uint32_t &hi, uint
       : "f"(a), "f"(b));
 }
 __device__ __forceinline__ void st_shared_f32(uint32_t saddr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(saddr), "f"(v) : "memory"); }
+__device__ __forceinline__ void st_shared_v2_u32(uint32_t saddr, uint32_t a, uint32_t b) { asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(saddr), "r"(a), "r"(b) : "memory"); }
 __device__ __forceinline__ void st_shared_u32(uint32_t saddr, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory"); }
 
 // byte offset of element (row, k) inside a K-major SWIZZLE_128B tile whose rows hold 32 floats (tile base 1024-B aligned)
