@@ -326,7 +326,7 @@ constexpr float ST_XSCALE = 256.f;
 
 struct SmlmTcArgs {
   const float2 *bcls;         // class tables, pre-scaled by s_Q
-  const uint4 *xy;            // the table, fp16 hi | lo, already swizzled: 4096 bytes
+  const uint4 *xy;            // the table, fp16 hi | lo, already swizzled: 4096 bytes in stage 1's K order, 4096 in stage 2's
   const float2 *ktp;
   const float *zbp;
   int ncls, K;
@@ -341,8 +341,8 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   constexpr uint32_t IDESC1 = umma_idesc_f16(128, 16), IDESC2 = umma_idesc_f16(128, 32);
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // (pointer arithmetic: the compiler keeps the shared address space)
-  uint8_t *xy = smem;
-  float2 *kts = reinterpret_cast<float2 *>(smem + ST_XY + LANES * ST_LANE_BYTES);
+  uint8_t *xy = smem, *xy2 = smem + ST_XY;             // the table in natural K order (stage 1) and in the drain's K order (stage 2)
+  float2 *kts = reinterpret_cast<float2 *>(smem + 2 * ST_XY + LANES * ST_LANE_BYTES);
   float2 *bcl = kts + SL_NQ * SL_NQ;
   float *zbs = reinterpret_cast<float *>(bcl + (size_t)A.ncls * SL_NQ * SL_NQ);
   float *cf_all = zbs + (size_t)A.K * SL_NQ * SL_NQ;
@@ -351,7 +351,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   // warp-uniform by construction (the broadcast tells the compiler so: addresses and descriptors derived from them stay in uniform registers)
   const int wu = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   const int lane_id = wu >> 2, warp = wu & 3, lt = threadIdx.x % SL_THREADS, l = threadIdx.x & 31;
-  uint8_t *A1 = smem + ST_XY + lane_id * ST_LANE_BYTES, *A2 = A1 + 2 * ST_TILE;
+  uint8_t *A1 = smem + 2 * ST_XY + lane_id * ST_LANE_BYTES, *A2 = A1 + 2 * ST_TILE;
   float *Fb = reinterpret_cast<float *>(A2);
   float *cfs = cf_all + lane_id * 16;
 
@@ -360,7 +360,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
     fence_barrier_init();
   }
   if (threadIdx.x < 32) tmem_alloc(&tmem_slot, 512);
-  for (int i = threadIdx.x; i < ST_XY / 16; i += blockDim.x) reinterpret_cast<uint4 *>(xy)[i] = __ldg(A.xy + i);
+  for (int i = threadIdx.x; i < 2 * ST_XY / 16; i += blockDim.x) reinterpret_cast<uint4 *>(xy)[i] = __ldg(A.xy + i);
   for (int i = threadIdx.x; i < SL_NQ * SL_NQ; i += blockDim.x) kts[i] = __ldg(A.ktp + i);
   for (int i = threadIdx.x; i < A.ncls * SL_NQ * SL_NQ; i += blockDim.x) bcl[i] = __ldg(A.bcls + i);
   for (int i = threadIdx.x; i < A.K * SL_NQ * SL_NQ; i += blockDim.x) zbs[i] = __ldg(A.zbp + i);
@@ -380,11 +380,22 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   // operand addresses of the thread's stores: the swizzle phase (q_y & 7) and the word inside the row do not change over the 4 q_y
   const uint32_t sw = (uint32_t)(qyb & 7);
   const uint32_t off_hi = ((((uint32_t)qxq >> 1) ^ sw) << 4) + (((uint32_t)qxq & 1u) << 3);     // the lo half sits at off_hi ^ 0x40
-  // drain stores: row = chain8 * 16 + m_x with m_x = mxa + 4 (lane & 1); the row's swizzle phase is m_x & 7 = (j & 3) + 4 (lane & 1)
-  const uint32_t a2_base = smem_u32(A2) + (uint32_t)((((warp >> 1) * 4 + (warp & 1)) * 16 + 4 * (l & 1)) * 128) + (((uint32_t)(l >> 1) & 3u) << 2);
-  uint32_t a2_sw[4];
+  // drain stores (fragment layout of tmem_ld_16x256b_x2): the thread holds q_y = rr, rr + 8, rr + 16, rr + 24 (rr = lane / 4) at
+  // m_x = 2 (lane % 4) + {0, 1, 8, 9}; the stage-2 contraction order puts q_y = rr, rr + 8 side by side (k = 2 rr, 2 rr + 1, and
+  // 16 + 2 rr, 17 + 2 rr for the upper pair), so a thread packs its own values into whole fp16 pairs: no exchange between lanes.
+  // row = chain8 * 16 + m_x; word rr (+ 8) of the row's hi half; the row's swizzle phase is m_x & 7 = 2 (lane % 4) + (column & 1)
+  uint32_t a2_off[2][2];
+  {
+    const uint32_t rrw = (uint32_t)(l >> 2);
 #pragma unroll
-  for (int k = 0; k < 4; ++k) a2_sw[k] = ((((uint32_t)l >> 3) ^ (uint32_t)(k + 4 * (l & 1))) << 4);
+    for (int jb = 0; jb < 2; ++jb)
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        const uint32_t mx = 2u * (uint32_t)(l & 3) + (uint32_t)jb;
+        a2_off[jb][half] = smem_u32(A2) + (uint32_t)(((warp >> 1) * 4 + (warp & 1)) * 16) * 128u + mx * 128u +
+                           ((((uint32_t)half * 2u + (rrw >> 2)) ^ (mx & 7u)) << 4) + ((rrw & 3u) << 2);
+      }
+  }
   const uint32_t a1_hi = smem_u32(A1) + (uint32_t)qyb * 128u + off_hi;
 
   for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
@@ -557,23 +568,21 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       // ---- drain D1: warp = chain (a, ri) of tile xb, lane = q_y; write T^T rows (class, ri, m_x), K = q_y ----
 #pragma unroll
       for (int xb = 0; xb < 2; ++xb) {
-        uint32_t v[16];
-        tmem_ld_32x32b_x16(tq + c * 32 + xb * 16, v);
+        uint32_t r[8], s[8];
+        tmem_ld_16x256b_x2(tq + c * 32 + xb * 16, r);
+        tmem_ld_16x256b_x2(tq + (16u << 16) + c * 32 + xb * 16, s);
         tmem_ld_wait();
-        // lane pairs exchange so that each lane owns two adjacent q_y of one row: even lanes row mxa, odd lanes row mxa + 4
-        const uint32_t dbase = a2_base + (uint32_t)xb * (2 * 16 * 128);        // chain8 = ((a 2 + xb) 2 + ri)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int mxa = (j & 3) + 8 * (j >> 2), mxb = mxa + 4;
-          const float va = __uint_as_float(v[mxa]), vb = __uint_as_float(v[mxb]);
-          const float send = (l & 1) ? va : vb;
-          const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
-          const float p0 = (l & 1) ? recv : va, p1 = (l & 1) ? vb : recv;      // (q_y even, q_y odd) of the lane's row
+        for (int j = 0; j < 4; ++j) {                                          // columns m_x = 2 (lane % 4) + {0, 1, 8, 9}
+          const int i0 = (j & 1) + 4 * (j >> 1);
+          const uint32_t rel = (uint32_t)xb * (2 * 16 * 128) + (uint32_t)(j >> 1) * (8 * 128);      // chain8 = ((a 2 + xb) 2 + ri)
           uint32_t hi, lo;
-          split_f16x2(p0, p1, hi, lo);
-          const uint32_t addr = dbase + (uint32_t)mxa * 128u + a2_sw[j & 3];
-          st_shared_u32(addr, hi);
-          st_shared_u32(addr ^ 0x40u, lo);                                     // the lo half sits four 16-byte chunks on: bit 6 after the swizzle
+          split_f16x2(__uint_as_float(r[i0]), __uint_as_float(r[i0 + 2]), hi, lo);      // q_y = rr, rr + 8
+          st_shared_u32(a2_off[j & 1][0] + rel, hi);
+          st_shared_u32((a2_off[j & 1][0] + rel) ^ 0x40u, lo);                 // the lo half sits four 16-byte chunks on: bit 6 after the swizzle
+          split_f16x2(__uint_as_float(s[i0]), __uint_as_float(s[i0 + 2]), hi, lo);      // q_y = rr + 16, rr + 24
+          st_shared_u32(a2_off[j & 1][1] + rel, hi);
+          st_shared_u32((a2_off[j & 1][1] + rel) ^ 0x40u, lo);
         }
       }
       fence_proxy_async_smem();
@@ -582,7 +591,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
       if (warp == 0 && elect_one()) {
         tcgen05_fence_after();
         const uint32_t d = tmem + c * 32;
-        const uint32_t a = smem_u32(A2), t = smem_u32(xy);
+        const uint32_t a = smem_u32(A2), t = smem_u32(xy2);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           const uint32_t o = k * 32;
@@ -751,23 +760,27 @@ psf_status smlm_setup(psf_plan *p, const std::vector<float> &zbq_sorted) {
     const double sX = (double)ST_XSCALE, sQ = std::min(pow2(qmax, 16384.0), pow2(rmax, 32768.0 / sX)), sT = sQ * sX;
     t->sQ = (float)sQ;
     t->fs2 = (float)((1.0 / (sT * sX)) * (1.0 / (sT * sX)));
-    std::vector<__half> xy((size_t)ST_XY / 2, __float2half_rn(0.f));
-    for (int row = 0; row < 32; ++row) {
-      const int mi = row & 15;
-      if (mi >= m) continue;
-      for (int q = 0; q < n; ++q) {
-        const double ph = p->phi[(size_t)mi * n + q];
-        const double v = sX * ((row >> 4) ? std::sin(ph) : std::cos(ph));
-        const __half hi = __float2half_rn((float)v);
-        const __half lo = __float2half_rn((float)(v - (double)__half2float(hi)));
-        const int bh = 2 * q, bl = 64 + 2 * q;          // byte offsets in the 128-byte row, before the swizzle
-        const int ph_hi = row * 128 + ((((bh >> 4) ^ (row & 7)) << 4) | (bh & 15));
-        const int ph_lo = row * 128 + ((((bl >> 4) ^ (row & 7)) << 4) | (bl & 15));
-        xy[ph_hi / 2] = hi;
-        xy[ph_lo / 2] = lo;
+    // two copies: K in natural order (stage 1: K = q_x) and in the order the drain writes T^T in (stage 2: K = q_y at position
+    // 16 (q / 16) + 2 (q % 8) + (q / 8) % 2, see the drain's comment in k_smlm_tc)
+    std::vector<__half> xy((size_t)ST_XY, __float2half_rn(0.f));
+    for (int copy = 0; copy < 2; ++copy)
+      for (int row = 0; row < 32; ++row) {
+        const int mi = row & 15;
+        if (mi >= m) continue;
+        for (int q = 0; q < n; ++q) {
+          const double ph = p->phi[(size_t)mi * n + q];
+          const double v = sX * ((row >> 4) ? std::sin(ph) : std::cos(ph));
+          const __half hi = __float2half_rn((float)v);
+          const __half lo = __float2half_rn((float)(v - (double)__half2float(hi)));
+          const int k = copy ? 16 * (q / 16) + 2 * (q % 8) + (q / 8) % 2 : q;
+          const int bh = 2 * k, bl = 64 + 2 * k;          // byte offsets in the 128-byte row, before the swizzle
+          const int ph_hi = row * 128 + ((((bh >> 4) ^ (row & 7)) << 4) | (bh & 15));
+          const int ph_lo = row * 128 + ((((bl >> 4) ^ (row & 7)) << 4) | (bl & 15));
+          xy[(size_t)copy * (ST_XY / 2) + ph_hi / 2] = hi;
+          xy[(size_t)copy * (ST_XY / 2) + ph_lo / 2] = lo;
+        }
       }
-    }
-    const size_t fixed_tc = (size_t)ST_XY + (size_t)SL_NQ * SL_NQ * 8 + (size_t)ncls * SL_NQ * SL_NQ * 8 + (size_t)K * SL_NQ * SL_NQ * 4 + 1024 + 256;
+    const size_t fixed_tc = 2 * (size_t)ST_XY + (size_t)SL_NQ * SL_NQ * 8 + (size_t)ncls * SL_NQ * SL_NQ * 8 + (size_t)K * SL_NQ * SL_NQ * 4 + 1024 + 256;
     const int lanes_tc = (fixed_tc + 3 * (size_t)ST_LANE_BYTES <= limit) ? 3 : (fixed_tc + 2 * (size_t)ST_LANE_BYTES <= limit) ? 2 : 0;
     std::vector<float2> bcls_s(bcls.size());
     for (size_t i = 0; i < bcls.size(); ++i) bcls_s[i] = make_float2((float)(sQ * bcls[i].x), (float)(sQ * bcls[i].y));   // power of two: exact

@@ -110,6 +110,15 @@ __device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)
                : "r"(taddr)
                : "memory");
 }
+// 16 lanes x 16 consecutive 32-bit columns in the accumulator-fragment layout (measured on B200 with a tcgen05.st / tcgen05.ld
+// round trip): thread t of the warp gets lanes base + t / 4 (r0, r1, r4, r5) and base + t / 4 + 8 (r2, r3, r6, r7), columns
+// 2 (t % 4), 2 (t % 4) + 1 (r0, r1 / r2, r3) and 8 + 2 (t % 4), 9 + 2 (t % 4) (r4, r5 / r6, r7).  The lane base is 0 or 16 of the warp's quarter.
+__device__ __forceinline__ void tmem_ld_16x256b_x2(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---- UMMA ----------------------------------------------------------------------------------------------------------
