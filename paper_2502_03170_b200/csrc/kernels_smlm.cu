@@ -415,22 +415,26 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
         pcl[r][0] = kz_turns(kts[f], pl.x, pl.y);
         pcl[r][1] = pcl[r][2] = pcl[r][3] = 0.f;
       }
+      // software pipeline: the coefficient and the basis values of term j + 1 are loaded while term j is accumulated (the last
+      // iteration re-reads its own basis row; the coefficient buffer has 16 floats for the read one past the row)
       int j = 0;
       float cnext = cfs[0];
+      const float *zb0 = zbs + qyb * SL_NQ + qx0;
+      float4 zn0 = make_float4(0.f, 0.f, 0.f, 0.f), zn1 = zn0;
+      if (K > 0) { zn0 = *reinterpret_cast<const float4 *>(zb0); zn1 = *reinterpret_cast<const float4 *>(zb0 + 16 * SL_NQ); }   // (no basis staged without terms)
 #pragma unroll
       for (int cls = 0; cls < 4; ++cls)
         for (int e = j + P.zcnt[cls]; j < e; ++j) {
           const float cj = cnext;
-          cnext = cfs[j + 1];                              // (one past the row at the end: the buffer has 16 floats)
-          const float *zb = zbs + j * (SL_NQ * SL_NQ) + qyb * SL_NQ + qx0;
-#pragma unroll
-          for (int rr = 0; rr < 2; ++rr) {
-            const float4 z4 = *reinterpret_cast<const float4 *>(zb + 16 * rr * SL_NQ);
-            pcl[4 * rr][cls] = fmaf(cj, z4.x, pcl[4 * rr][cls]);
-            pcl[4 * rr + 1][cls] = fmaf(cj, z4.y, pcl[4 * rr + 1][cls]);
-            pcl[4 * rr + 2][cls] = fmaf(cj, z4.z, pcl[4 * rr + 2][cls]);
-            pcl[4 * rr + 3][cls] = fmaf(cj, z4.w, pcl[4 * rr + 3][cls]);
-          }
+          const float4 z0 = zn0, z1 = zn1;
+          cnext = cfs[j + 1];
+          const float *zb = zb0 + (j + 1 < K ? j + 1 : j) * (SL_NQ * SL_NQ);
+          zn0 = *reinterpret_cast<const float4 *>(zb);
+          zn1 = *reinterpret_cast<const float4 *>(zb + 16 * SL_NQ);
+          pcl[0][cls] = fmaf(cj, z0.x, pcl[0][cls]); pcl[1][cls] = fmaf(cj, z0.y, pcl[1][cls]);
+          pcl[2][cls] = fmaf(cj, z0.z, pcl[2][cls]); pcl[3][cls] = fmaf(cj, z0.w, pcl[3][cls]);
+          pcl[4][cls] = fmaf(cj, z1.x, pcl[4][cls]); pcl[5][cls] = fmaf(cj, z1.y, pcl[5][cls]);
+          pcl[6][cls] = fmaf(cj, z1.z, pcl[6][cls]); pcl[7][cls] = fmaf(cj, z1.w, pcl[7][cls]);
         }
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
@@ -503,6 +507,42 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
     for (int c = 0; c < P.C; ++c) {
       // ---- Q_g = sum_ab B_ab Phi_(g xor ab), scaled, split, into the two stage-1 operand tiles ----
       const int c0 = A.comp_start[c], c1 = A.comp_start[c + 1];
+      if (c1 - c0 == 1) {
+        // one parity class in this component (a pure polarisation component): Q_g = B Phi_(g xor x), no sum.  The product with
+        // Phi_h goes to class g = h xor x: only the store address depends on x (uniform integer arithmetic, no branch)
+        const int x = A.cls_ab[c0];
+        uint32_t at_h[4];
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+          const int g = h ^ x;
+          at_h[h] = a1_hi + (uint32_t)(g & 1) * ST_TILE + (uint32_t)((g >> 1) * 2 * 32) * 128u;
+        }
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+          const float4 *bp = reinterpret_cast<const float4 *>(&bcl[c0 * (SL_NQ * SL_NQ) + (qyb + 16 * rr) * SL_NQ + qx0]);
+          const float4 b01 = bp[0], b23 = bp[1];
+          const float2 bv[4] = {make_float2(b01.x, b01.y), make_float2(b01.z, b01.w), make_float2(b23.x, b23.y), make_float2(b23.z, b23.w)};
+#pragma unroll
+          for (int h = 0; h < 4; ++h) {
+            float2 q[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const float2 f = phi[4 * rr + e][h];
+              q[e] = make_float2(fmaf(bv[e].x, f.x, -bv[e].y * f.y), fmaf(bv[e].x, f.y, bv[e].y * f.x));
+            }
+            const uint32_t at = at_h[h] + (uint32_t)(16 * rr) * 128u;
+            uint32_t h0, l0, h1, l1;
+            split_f16x2(q[0].x, q[1].x, h0, l0);
+            split_f16x2(q[2].x, q[3].x, h1, l1);
+            st_shared_v2_u32(at, h0, h1);
+            st_shared_v2_u32(at ^ 0x40u, l0, l1);
+            split_f16x2(q[0].y, q[1].y, h0, l0);
+            split_f16x2(q[2].y, q[3].y, h1, l1);
+            st_shared_v2_u32(at + 32 * 128, h0, h1);
+            st_shared_v2_u32((at + 32 * 128) ^ 0x40u, l0, l1);
+          }
+        }
+      } else {
 #pragma unroll
       for (int rr = 0; rr < 2; ++rr) {
         float2 o[4][4];
@@ -541,6 +581,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
           st_shared_v2_u32(at + 32 * 128, h0, h1);
           st_shared_v2_u32((at + 32 * 128) ^ 0x40u, l0, l1);
         }
+      }
       }
       fence_proxy_async_smem();
       tcgen05_fence_before();                            // (the previous component's TMEM reads of this lane are behind us)
