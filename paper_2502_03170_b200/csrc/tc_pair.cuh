@@ -577,6 +577,25 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
               issue_kstep2(sb, d, k, kc == 0 && k == 0);
+              // Happens-before chains of an operand slot `st`, edge by edge, and what each edge rests on:
+              //  read-after-write (producers -> tensor core):
+              //    st.shared of the operand rows (generic proxy)
+              //    -> fence.proxy.async.shared::cta in every writing thread (PTX ISA, async proxy: generic-proxy accesses before
+              //       the fence are ordered before later async-proxy accesses - the tcgen05.mma operand reads)
+              //    -> __syncwarp, lane 0: mbarrier.arrive on the LEADER's `full[st]` (default semantics: .release at .cta scope;
+              //       PSF_TUNE_K1P_HANDOFF = 1: .release.cluster)
+              //    -> this thread: mbarrier.try_wait (default .acquire.cta; HANDOFF = 1: .acquire.cluster)
+              //    -> tcgen05.fence::after_thread_sync -> tcgen05.mma.cta_group::2 (reads the slot in both CTAs).
+              //    For the leader's own producers every edge is in the memory model.  For the peer's producers the release /
+              //    acquire pair is morally strong only at cluster scope: HANDOFF = 1 is the chain the model guarantees, and it costs
+              //    17 % of the stage-1 time (the release compiles to MEMBAR.ALL.GPU + ERRBAR on the stage's critical path).  The
+              //    default rests on the hardware order "stores performed -> fence retires -> the remote arrive leaves the SM";
+              //    the operand rows of the peer live in the peer's own shared memory and are read by the peer's tensor core.
+              //  write-after-read (tensor core -> producers):
+              //    tcgen05.mma x 12 -> tcgen05.commit.cta_group::2 ... multicast::cluster on `empty[st]` of both CTAs (PTX ISA: the
+              //    arrive is triggered when all prior asynchronous tcgen05 operations of the issuing thread have completed)
+              //    -> producer: mbarrier.try_wait -> st.shared into the slot.  Every edge is in the model - and this is where the
+              //    measured failures sit (profiles/r1j_race_k1_pair.md, profiles/r2_race_k1_pair.md): hence the margin below.
               // Deferred release (profiles/r1j_race_k1_pair.md): the commit tracks the UMMAs of the issuing (leader) CTA; in
               // the peer, whose tensor core can trail by a little, producers with their rows ready in registers
               // overwrote the operand tile while it was still being read.  The previous stage's buffer is therefore
