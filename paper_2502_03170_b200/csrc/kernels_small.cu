@@ -51,6 +51,37 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
   const int b = blockIdx.x;
   const int n = P.n, m = P.m, N = P.N, M = P.M;
 
+  // A short stack is nothing but the latencies of its first touches: after other work has gone through the L2 (bench.py flushes
+  // it between steps) every table is a DRAM access, and the tables are read in phases that depend on one another (tables ->
+  // phasors -> per component the base pupil).  In static mode the thread therefore issues, now, every global load of its
+  // prologue - plane, kappa, the base pupil of component 0 - ahead of the table staging (whose loop is fully unrolled as
+  // well), and the base pupil of component c + 1 is loaded into registers before the two DFT stages of component c: one
+  // overlapped round trip at the start instead of one per phase and per component.
+  constexpr int NSAMP = (NQ * NQ) / SM_THREADS;
+  float4 bq[PER_PLANE ? 1 : 2 * NSAMP];
+  float2 ktv[PER_PLANE ? 1 : NSAMP];
+  auto load_bq = [&](int c) {
+#pragma unroll
+    for (int r = 0; r < NSAMP; ++r) {
+      const int f = tid + SM_THREADS * r;
+      const int qy = f >> 5, qx = f & 31;
+      const bool ok = qy < n && qx < n;
+      const size_t s = ok ? ((size_t)c * n * n + (size_t)qy * n + qx) * 2 : 0;
+      bq[PER_PLANE ? 0 : 2 * r] = ok ? __ldg(P.bfold + s) : make_float4(0.f, 0.f, 0.f, 0.f);
+      bq[PER_PLANE ? 0 : 2 * r + 1] = ok ? __ldg(P.bfold + s + 1) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  };
+  const float4 pl = __ldg(P.planes + b);
+  if (!PER_PLANE) {
+#pragma unroll
+    for (int r = 0; r < NSAMP; ++r) {
+      const int f = tid + SM_THREADS * r;
+      const int qy = f >> 5, qx = f & 31;
+      ktv[PER_PLANE ? 0 : r] = (qy < n && qx < n) ? __ldg(P.kt + (size_t)qy * n + qx) : make_float2(0.f, 0.f);
+    }
+    load_bq(0);
+  }
+#pragma unroll
   for (int i = tid; i < NQ * MQ; i += SM_THREADS) {
     const int q = i / MQ, mi = i % MQ;
     const bool ok = q < n && mi < m;
@@ -59,18 +90,17 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
   }
 
   // ---- phase 0: phasors -------------------------------------------------------------------------------------------
-  const float4 pl = __ldg(P.planes + b);
   // phasors (cos, sin) of this thread's 8 samples at their (up to) four mirror images, kept in registers: a thread reads
   // back only the phasors it wrote, and without the 32 KB they took in shared memory more CTAs fit an SM
   float2 phr[PER_PLANE ? (NQ * NQ) / SM_THREADS : 1][PER_PLANE ? 4 : 1];
-#pragma unroll (PER_PLANE ? 8 : 2)
+#pragma unroll 8
   for (int r = 0; r < (NQ * NQ) / SM_THREADS; ++r) {
     const int f = tid + SM_THREADS * r;
     const int qy = f >> 5, qx = f & 31;
     float2 ph[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
     if (qy < n && qx < n) {
       const size_t s = (size_t)qy * n + qx;
-      const float t0 = kz_turns(__ldg(P.kt + s), pl.x, pl.y);
+      const float t0 = kz_turns(PER_PLANE ? __ldg(P.kt + s) : ktv[PER_PLANE ? 0 : r], pl.x, pl.y);
       if (PER_PLANE) {
         // parity classes of the phase: even/even, x-odd, y-odd, odd/odd
         float pee = t0, pxo = 0.f, pyo = 0.f, poo = 0.f;
@@ -121,7 +151,7 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
   for (int c = 0; c < P.C; ++c) {
     __syncthreads();                             // Qs / Ts of the previous component are free (and the tables are in)
     // ---- Q: base pupil x phasor, folded (a thread reads back only the phasors it wrote) ----
-#pragma unroll (PER_PLANE ? 8 : 2)
+#pragma unroll 8
     for (int r = 0; r < (NQ * NQ) / SM_THREADS; ++r) {
       const int f = tid + SM_THREADS * r;
       const int qy = f >> 5, qx = f & 31;
@@ -151,8 +181,7 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
           o[4] = selfy ? 0.f : e0.x - e1.x;  o[5] = selfy ? 0.f : e0.y - e1.y;           // oe
           o[6] = (selfx || selfy) ? 0.f : o0.x - o1.x;  o[7] = (selfx || selfy) ? 0.f : o0.y - o1.y;   // oo
         } else {
-          const size_t s = ((size_t)c * n * n + (size_t)qy * n + qx) * 2;
-          const float4 b0 = __ldg(P.bfold + s), b1 = __ldg(P.bfold + s + 1);
+          const float4 b0 = bq[PER_PLANE ? 0 : 2 * r], b1 = bq[PER_PLANE ? 0 : 2 * r + 1];
           const float2 e = S.Ph0[PER_PLANE ? 0 : f];
           o[0] = b0.x * e.x - b0.y * e.y;  o[1] = b0.x * e.y + b0.y * e.x;
           o[2] = b0.z * e.x - b0.w * e.y;  o[3] = b0.z * e.y + b0.w * e.x;
@@ -164,6 +193,7 @@ __global__ void __launch_bounds__(SM_THREADS, PER_PLANE ? 4 : 1) k_small(const D
       dst[0] = make_float4(o[0], o[1], o[2], o[3]);
       dst[1] = make_float4(o[4], o[5], o[6], o[7]);
     }
+    if (!PER_PLANE && c + 1 < P.C) load_bq(c + 1);     // in flight under the two DFT stages of this component
     __syncthreads();
 
     // ---- stage 1: rows.  thread = (qy, group of 4 mx) ----
