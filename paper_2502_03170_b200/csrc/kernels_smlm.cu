@@ -77,6 +77,26 @@ __device__ __forceinline__ float2 cfma(float2 a, float2 b, float2 c) {   // c + 
   return make_float2(fmaf(a.x, b.x, fmaf(-a.y, b.y, c.x)), fmaf(a.x, b.y, fmaf(a.y, b.x, c.y)));
 }
 
+// Stages `count16` 16-byte words of a table into shared memory with the whole CTA, eight loads in flight per thread (a plain loop
+// is one DRAM round trip per iteration when the tables are cold).
+__device__ __forceinline__ void sl_stage16(void *dst, const void *src, int count16) {
+  uint4 *d = reinterpret_cast<uint4 *>(dst);
+  const uint4 *g = reinterpret_cast<const uint4 *>(src);
+  for (int i0 = threadIdx.x; i0 < count16; i0 += 8 * blockDim.x) {
+    uint4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int i = i0 + u * blockDim.x;
+      if (i < count16) v[u] = __ldg(g + i);
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int i = i0 + u * blockDim.x;
+      if (i < count16) d[i] = v[u];
+    }
+  }
+}
+
 template <int MQ, int LANES>
 __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, const SmlmArgs A, float *__restrict__ I) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
@@ -93,10 +113,10 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, 
   float *cfs = Ts + SL_NQ * TS_ROW;             // the emitter's coefficient row (16 floats)
 
   // ---- stage the static tables (whole CTA) ----
-  for (int i = threadIdx.x; i < SL_NQ * MQ; i += blockDim.x) Xd[i] = __ldg(A.xd + i);
-  for (int i = threadIdx.x; i < SL_NQ * SL_NQ; i += blockDim.x) kts[i] = __ldg(A.ktp + i);
-  for (int i = threadIdx.x; i < A.ncls * SL_NQ * SL_NQ; i += blockDim.x) bcl[i] = __ldg(A.bcls + i);
-  for (int i = threadIdx.x; i < A.K * SL_NQ * SL_NQ; i += blockDim.x) zbs[i] = __ldg(A.zbp + i);
+  sl_stage16(Xd, A.xd, SL_NQ * MQ / 2);
+  sl_stage16(kts, A.ktp, SL_NQ * SL_NQ / 2);
+  sl_stage16(bcl, A.bcls, A.ncls * SL_NQ * SL_NQ / 2);
+  sl_stage16(zbs, A.zbp, A.K * SL_NQ * SL_NQ / 4);
   __syncthreads();
 
   const int m = P.m, M = P.M, N = P.N, K = A.K;
@@ -105,6 +125,17 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, 
   for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
     const float4 pl = __ldg(P.planes + b);
     if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
+    {
+      // the lane's next emitter: its plane entry and coefficient row into L1 now, so that the two loads above are hits then
+      const int bn = b + gridDim.x * LANES;
+      if (bn < P.Z) {
+        if (lt == 32) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.planes + bn));
+        if (lt == 64) {
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(P.coefq + (size_t)bn * K));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(P.coefq + (size_t)bn * K + (K > 0 ? K - 1 : 0)));
+        }
+      }
+    }
     sl_bar(lane_id);
 
     // ---- phase 0: the parity transform Phi_g of the emitter's phasor field, 8 folded samples per thread, in registers ----
@@ -360,10 +391,10 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
     fence_barrier_init();
   }
   if (threadIdx.x < 32) tmem_alloc(&tmem_slot, 512);
-  for (int i = threadIdx.x; i < 2 * ST_XY / 16; i += blockDim.x) reinterpret_cast<uint4 *>(xy)[i] = __ldg(A.xy + i);
-  for (int i = threadIdx.x; i < SL_NQ * SL_NQ; i += blockDim.x) kts[i] = __ldg(A.ktp + i);
-  for (int i = threadIdx.x; i < A.ncls * SL_NQ * SL_NQ; i += blockDim.x) bcl[i] = __ldg(A.bcls + i);
-  for (int i = threadIdx.x; i < A.K * SL_NQ * SL_NQ; i += blockDim.x) zbs[i] = __ldg(A.zbp + i);
+  sl_stage16(xy, A.xy, 2 * ST_XY / 16);
+  sl_stage16(kts, A.ktp, SL_NQ * SL_NQ / 2);
+  sl_stage16(bcl, A.bcls, A.ncls * SL_NQ * SL_NQ / 2);
+  sl_stage16(zbs, A.zbp, A.K * SL_NQ * SL_NQ / 4);
   fence_proxy_async_smem();                    // the table is read by the async proxy
   tcgen05_fence_before();
   __syncthreads();
@@ -402,6 +433,17 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
     const float4 pl = __ldg(P.planes + b);
     sl_bar(lane_id);                                     // the previous emitter's reads of cfs are done
     if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
+    {
+      // the lane's next emitter: its plane entry and coefficient row into L1 now, so that the two loads above are hits then
+      const int bn = b + gridDim.x * LANES;
+      if (bn < P.Z) {
+        if (lt == 32) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.planes + bn));
+        if (lt == 64) {
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(P.coefq + (size_t)bn * K));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(P.coefq + (size_t)bn * K + (K > 0 ? K - 1 : 0)));     // (a row can straddle two sectors)
+        }
+      }
+    }
     sl_bar(lane_id);
 
     // ---- phase 0: parity transform Phi_g of the emitter's phasor field at the thread's 8 folded samples ----
