@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm(const DevPlan P, 
   const int m = P.m, M = P.M, N = P.N, K = A.K;
   constexpr int PASS1 = MQ / 16, PASS2 = (MQ / 2) * (MQ / 2) / 64;
 
-  for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
+  for (int b = lane_id * gridDim.x + blockIdx.x; b < P.Z; b += gridDim.x * LANES) {   // lane-major rounds: the emitters of a partial last round go to one lane each of as many CTAs
     const float4 pl = __ldg(P.planes + b);
     if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
     {
@@ -429,7 +429,7 @@ __global__ void __launch_bounds__(SL_THREADS *LANES, 1) k_smlm_tc(const DevPlan 
   }
   const uint32_t a1_hi = smem_u32(A1) + (uint32_t)qyb * 128u + off_hi;
 
-  for (int b = blockIdx.x * LANES + lane_id; b < P.Z; b += gridDim.x * LANES) {
+  for (int b = lane_id * gridDim.x + blockIdx.x; b < P.Z; b += gridDim.x * LANES) {   // lane-major rounds: the emitters of a partial last round go to one lane each of as many CTAs
     const float4 pl = __ldg(P.planes + b);
     sl_bar(lane_id);                                     // the previous emitter's reads of cfs are done
     if (lt < K) cfs[lt] = __ldg(P.coefq + (size_t)b * K + lt);
