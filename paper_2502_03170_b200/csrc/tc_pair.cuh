@@ -429,7 +429,9 @@ k2_pair(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ CUt
         const __grid_constant__ CUtensorMap map_thi, const __grid_constant__ CUtensorMap map_tlo, const K2PArgs P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
+  // (pointer arithmetic on the shared array: the compiler keeps the address space, the epilogue's staging accesses are LDS / STS
+  // instead of generic loads and stores)
+  float *staging = reinterpret_cast<float *>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + K2P_NST * P_STAGE);
   __shared__ K2PShared S;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
@@ -944,7 +946,7 @@ k12_fused(const __grid_constant__ CUtensorMap map_xhi, const __grid_constant__ C
       setmaxnreg_dec<24>();
     }
   } else {
-    float *staging = reinterpret_cast<float *>(smem + K2P_NST * P_STAGE);
+    float *staging = reinterpret_cast<float *>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) + K2P_NST * P_STAGE);   // (shared address space kept)
     const int nk = P2.n_pad / 64;
     const int tiles_yp = (P2.m_pad / 128 + 1) / 2, tiles_x = P2.m_pad / 64;
     const int ntiles = P2.zc * tiles_yp * tiles_x;
