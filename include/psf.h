@@ -190,7 +190,9 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_K1P_HANDOFF   : stage-1 pair kernel, how the non-leader CTA's producer warps signal the leader's barrier:
  *                            0 (default) plain remote arrive, 1 cluster-scope release per warp;
  *   PSF_TUNE_K1P_DEFER     : producer-written operand slots are released that many K-steps (three UMMAs each) after the stage's
- *                            last UMMA: 1 (default), 0 = at once (the A/B setting of profiles/r2_race_k1_pair.md; unsafe), up to 4;
+ *                            last UMMA: 2 (default; 0 wrong stacks in 200000 calls), 1 (round 2's first setting: one wrong plane in
+ *                            about 25000 calls), 0 = at once (about one call in 100: the A/B setting of profiles/r2_race_k1_pair.md),
+ *                            up to 4; profiles/r5_soak.md has the measured rates and the cost (about 1 % of the config-5 step);
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
  *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;

@@ -98,7 +98,7 @@ struct psf_plan {
   int tune_fused = 1;            // 1: both stages in one launch (k12_fused) where eligible; 0: always two launches
   int tune_k1p_handoff = 0;      // k1_pair: 0 plain remote arrive, 1 .release.cluster arrive per producer warp of the non-leader CTA
   int tune_k1p_asplit = 1;       // k1_pair: 1 = the TMA-written table half of a stage buffer is released right behind its own stage
-  int tune_k1p_defer = 1;        // k1_pair: K = 16 steps of the next stage issued before a stage buffer is released
+  int tune_k1p_defer = 2;        // k1_pair: K = 16 steps of the next stage issued before a stage buffer is released (profiles/r5_soak.md)
   cudaEvent_t done_ev = nullptr; // recorded on the caller's stream after the last launch of every compute call: table
                                  // refreshes wait for it before they overwrite tables a launch in flight may still read
   long long table_version = 0;   // bumped by every table refresh (psf_set_*): derived copies check it

@@ -479,9 +479,10 @@ def _repeat_bit_identical(psf, case, calls, tune=None, flush_every=2):
 
 def test_pair_kernels_are_deterministic_under_repetition(psf):
     """Guards the cross-CTA hand-off of the producer-written operand rows in k1_pair.  Without the deferred release of
-    the operand buffers about 0.5-4 % of config-5 calls have one plane computed from wrong rows of one stage; the cause is
-    not established (profiles/r1j_race_k1_pair.md, profiles/r2_race_k1_pair.md: a write-after-read window in the non-leader
-    CTA is the working hypothesis), so this is a statistical guard: 2000 calls over config 5 as bench.py launches it, a
+    the operand buffers about 1 % of config-5 calls have one plane computed from wrong rows of one stage; released one
+    K-step late it is one call in 25000, two K-steps late (the default) none in 200000 (profiles/r5_soak.md: a write-after-read
+    window whose mechanism is a hypothesis), so this is a statistical guard that catches a regression to the 1e-3 level, and
+    test_pair_kernels_soak is the tool for the rest: 2000 calls over config 5 as bench.py launches it, a
     pupil above 512 (the producers recompute the phasors per stage: another cadence), and config 5 in 6-plane launch pairs
     (short grids: every cluster starts and drains 43 times per call)."""
     assert _repeat_bit_identical(psf, W.config5(), 1200) == 0
