@@ -188,7 +188,9 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_TC_SCRATCH_MB : budget in MB of the stage-1 -> stage-2 scratch (default 0 = 4096): a smaller value splits a
  *                            stack into several launch pairs;
  *   PSF_TUNE_K1P_HANDOFF   : stage-1 pair kernel, how the non-leader CTA's producer warps signal the leader's barrier:
- *                            0 (default) plain remote arrive, 1 cluster-scope release per warp;
+ *                            0 (default) plain remote arrive, 1 cluster-scope release per warp; 2 / 3 = diagnosis settings of
+ *                            profiles/r5_soak.md (plain arrive; the operand slot of the leader / of the peer is released one K-step late,
+ *                            the other's two, whatever PSF_TUNE_K1P_DEFER says): not for use;
  *   PSF_TUNE_K1P_DEFER     : producer-written operand slots are released that many K-steps (three UMMAs each) after the stage's
  *                            last UMMA: 2 (default; 0 wrong stacks in 200000 calls), 1 (round 2's first setting: one wrong plane in
  *                            about 25000 calls), 0 = at once (about one call in 100: the A/B setting of profiles/r2_race_k1_pair.md),

@@ -625,7 +625,7 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_DEVICE_REFRESH: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_dev_refresh = (int)value;
     } else if (knob == PSF_TUNE_K1P_HANDOFF) {
-      if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..1"; return PSF_ERR_INVALID_ARG; }
+      if (value < 0 || value > 3) { p->err = "PSF_TUNE_K1P_HANDOFF: 0..3"; return PSF_ERR_INVALID_ARG; }
       p->tune_k1p_handoff = (int)value;
     } else if (knob == PSF_TUNE_K1P_DEFER) {
       if (value < 0 || value > 4) { p->err = "PSF_TUNE_K1P_DEFER: 0..4"; return PSF_ERR_INVALID_ARG; }

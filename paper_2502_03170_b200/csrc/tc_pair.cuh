@@ -107,9 +107,9 @@ __device__ __forceinline__ void umma2_f16(uint32_t d_tmem, uint64_t a_desc, uint
       : "memory");
 }
 // arrive on the barrier at the same shared-memory offset in both CTAs once the pair's previously issued UMMAs are done
-__device__ __forceinline__ void umma2_commit(uint64_t *bar) {
+__device__ __forceinline__ void umma2_commit(uint64_t *bar, uint16_t cta_mask = 3) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-               ::"r"(smem_u32(bar)), "h"((uint16_t)3)
+               ::"r"(smem_u32(bar)), "h"(cta_mask)
                : "memory");
 }
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
@@ -572,7 +572,7 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
           tcgen05_fence_after();
           const uint32_t d = tmem + g * 256;
           for (int kc = 0; kc < G.nk; ++kc) {
-            if (P.handoff) mbar_wait_acquire_cluster(&S.full[st], ph);
+            if (P.handoff == 1) mbar_wait_acquire_cluster(&S.full[st], ph);
             else mbar_wait(&S.full[st], ph);
             tcgen05_fence_after();
             const uint32_t sb = smem_u32(smem + st * P_STAGE);
@@ -605,7 +605,17 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
               // overwrote the operand tile while it was still being read.  The previous stage's buffer is therefore
               // released only after K1P_DEFER K-steps of this stage have been issued behind it: the commit then also
               // waits for those, which gives the peer that much tensor time of slack.
-              if (k == P.defer - 1 && pending >= 0) { umma2_commit(&S.empty[pending]); pending = -1; }
+              if (pending >= 0) {
+                // (diagnosis settings HANDOFF = 2 / 3, profiles/r5_soak.md: the slot of one CTA released one K-step late, the other's two)
+                const int dl = P.handoff == 2 ? 1 : (P.handoff == 3 ? 2 : P.defer), dp = P.handoff == 2 ? 2 : (P.handoff == 3 ? 1 : P.defer);
+                if (dl == dp) {
+                  if (k == dl - 1) { umma2_commit(&S.empty[pending]); pending = -1; }
+                } else {
+                  if (k == dl - 1) umma2_commit(&S.empty[pending], 1);
+                  if (k == dp - 1) umma2_commit(&S.empty[pending], 2);
+                  if (k == (dl > dp ? dl : dp) - 1) pending = -1;
+                }
+              }
             }
             if (P.asplit) umma2_commit(&S.a_empty[st]);          // the TMA-written table tiles: free as soon as these UMMAs are done
             if (P.defer == 0) umma2_commit(&S.empty[st]);
@@ -708,7 +718,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           fence_proxy_async_smem();                                // every writer fences its own stores; no load is in flight here
           __syncwarp();
           if (lane == 0) {
-            if (rank == 0 || P.handoff == 0) mbar_arrive_cluster(full_leader0 + st * 8);
+            if (rank == 0 || P.handoff != 1) mbar_arrive_cluster(full_leader0 + st * 8);
             else mbar_arrive_cluster_release(full_leader0 + st * 8);
           }
           if (++st == K1P_NST) { st = 0; ph ^= 1; }
