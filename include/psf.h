@@ -216,10 +216,13 @@ int psf_grad_terms(const psf_plan *plan);
  *   PSF_TUNE_PDL           : 1 (default) = on the two-kernel tensor path the stage-2 kernel is a programmatic dependent launch of
  *                            stage 1: its CTAs take the SMs stage 1 leaves, run their prologue (barriers, TMEM, table loads) and
  *                            wait (griddepcontrol.wait) for the stage-1 grid to complete before the first read of its output;
- *                            0 = plain stream order. */
+ *                            0 = plain stream order;
+ *   PSF_TUNE_K1P_WAITFIRST : 1 (default) = the stage-1 producers wait for their operand slot before they compute its rows, so that the
+ *                            computation lies between the observed release and the first store into the slot; 0 = they compute
+ *                            first and wait with the rows in registers (round 2's earlier order; profiles/r5_soak.md). */
 enum { PSF_TUNE_TC_PAIR_MASK = 1, PSF_TUNE_TC_SCRATCH_MB = 2, PSF_TUNE_K1P_HANDOFF = 3, PSF_TUNE_K1P_DEFER = 4, PSF_TUNE_TC_FUSED = 5,
        PSF_TUNE_SMLM = 6, PSF_TUNE_GRAD_TENSOR = 7, PSF_TUNE_K1P_ASPLIT = 8,
-       PSF_TUNE_FUSED_WINDOW = 9, PSF_TUNE_DEVICE_REFRESH = 10, PSF_TUNE_PDL = 11 };
+       PSF_TUNE_FUSED_WINDOW = 9, PSF_TUNE_DEVICE_REFRESH = 10, PSF_TUNE_PDL = 11, PSF_TUNE_K1P_WAITFIRST = 12 };
 psf_status psf_plan_tune(psf_plan *plan, int knob, long long value);
 
 /* Last error message of `plan`, or (plan == NULL) of the calling thread's last failed psf_plan_create /

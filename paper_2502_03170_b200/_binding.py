@@ -23,7 +23,7 @@ EXPORTS = ["psf_plan_create", "psf_set_zernike", "psf_set_shifts", "psf_set_phas
            "psf_last_error", "psf_launches_per_compute", "psf_path_name", "psf_host_tables",
            "psf_profile_enable", "psf_profile_read", "psf_last_upload_bytes", "psf_plan_tune", "psf_grad_terms", "psf_kernel_names", "psf_grad_path_name",
            "psf_propagate_static"]
-TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER, TUNE_TC_FUSED, TUNE_SMLM, TUNE_GRAD_TENSOR, TUNE_K1P_ASPLIT, TUNE_FUSED_WINDOW, TUNE_DEVICE_REFRESH, TUNE_PDL = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
+TUNE_TC_PAIR_MASK, TUNE_TC_SCRATCH_MB, TUNE_K1P_HANDOFF, TUNE_K1P_DEFER, TUNE_TC_FUSED, TUNE_SMLM, TUNE_GRAD_TENSOR, TUNE_K1P_ASPLIT, TUNE_FUSED_WINDOW, TUNE_DEVICE_REFRESH, TUNE_PDL, TUNE_K1P_WAITFIRST = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12
 
 
 class PsfError(RuntimeError):

@@ -618,6 +618,9 @@ psf_status psf_plan_tune(psf_plan *p, int knob, long long value) {
     } else if (knob == PSF_TUNE_SMLM) {
       if (value < 0 || value > 2) { p->err = "PSF_TUNE_SMLM: 0..2"; return PSF_ERR_INVALID_ARG; }
       p->tune_smlm = (int)value;
+    } else if (knob == PSF_TUNE_K1P_WAITFIRST) {
+      if (value < 0 || value > 1) { p->err = "PSF_TUNE_K1P_WAITFIRST: 0..1"; return PSF_ERR_INVALID_ARG; }
+      p->tune_k1p_waitfirst = (int)value;
     } else if (knob == PSF_TUNE_PDL) {
       if (value < 0 || value > 1) { p->err = "PSF_TUNE_PDL: 0..1"; return PSF_ERR_INVALID_ARG; }
       p->tune_pdl = (int)value;

@@ -105,6 +105,7 @@ struct psf_plan {
   long long static_version = 0;  // bumped by every full (host) refresh: a device-side refresh of the shared phase leaves it alone
   long long phase_mask_version = 0;   // bumped by psf_set_phase_mask (device copies of the mask check it)
   bool host_base_stale = false;  // the last refresh ran on the device (tc_refresh_device): h_base / h_bfold are behind; see host_base()
+  int tune_k1p_waitfirst = 1;    // k1_pair producers await the operand slot before computing its rows (0: after, round 2's earlier order)
   int tune_pdl = 1;              // 1: stage-2 kernels of the two-kernel tensor path are launched as programmatic dependents of stage 1
   int tune_dev_refresh = 1;      // 1: shared-phase changes of a 3xFP16 pair plan are refreshed on the device; 0: always the host path
   std::vector<double> phi;       // zoomed-DFT phase table [m][n] (fp64)

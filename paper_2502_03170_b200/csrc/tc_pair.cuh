@@ -480,6 +480,7 @@ struct K1PArgs {
   float f1;             // epilogue factor s_T / (s_Q s_X)
   int handoff;          // how the non-leader CTA's producer warps signal the leader's barrier: 0 plain arrive, 1 cluster-scope release
   int defer;            // K = 16 steps of the next stage issued before a stage buffer is released (0 = released right behind its own stage)
+  int waitfirst;        // 1: producers wait for the operand slot before they compute its rows (see k1p_produce)
   int asplit;           // 1: the table half of a stage buffer (refilled by TMA, no hazard) has its own barrier and is released right
                         // behind its own stage; only the producer-written half waits for the deferred release
 };
@@ -693,6 +694,11 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
               sc[k4][i] = make_float4(__cosf(t0), __sinf(t0), __cosf(t1), __sinf(t1));
             }
           }
+          // The operand slot is awaited BEFORE the rows are computed (P.waitfirst, default): the producers are the slower side
+          // of the pipeline, so the slot is almost always free already and nothing is lost - but when it is not, the math and
+          // the split below (about 600 cycles) now lie between the moment the release is observed and the first store into
+          // the slot, on top of the deferral of the release itself (profiles/r5_soak.md).
+          if (P.waitfirst) mbar_wait(&S.empty[st], ph ^ 1);
           mbar_wait(&S.bb_full[bs], bph);
           uint32_t hi[4][4], lo[4][4];                             // [slot][pair of q_x]
 #pragma unroll
@@ -708,7 +714,7 @@ __device__ __forceinline__ void k1p_produce(uint8_t *smem, K1PShared &S, const K
           __syncwarp();
           if (lane == 0) mbar_arrive(&S.bb_empty[bs]);             // the ring slot is in registers
           if (++bs == K1P_BB_SLOTS) { bs = 0; bph ^= 1; }
-          mbar_wait(&S.empty[st], ph ^ 1);
+          if (!P.waitfirst) mbar_wait(&S.empty[st], ph ^ 1);
           const uint32_t bh = smem0 + st * P_STAGE + 2 * TILE16K + off0, bl = bh + TILE16K;
 #pragma unroll
           for (int s = 0; s < 4; ++s) {
