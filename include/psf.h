@@ -192,9 +192,10 @@ int psf_grad_terms(const psf_plan *plan);
  *                            profiles/r5_soak.md (plain arrive; the operand slot of the leader / of the peer is released one K-step late,
  *                            the other's two, whatever PSF_TUNE_K1P_DEFER says): not for use;
  *   PSF_TUNE_K1P_DEFER     : producer-written operand slots are released that many K-steps (three UMMAs each) after the stage's
- *                            last UMMA: 2 (default; 0 wrong stacks in 200000 calls), 1 (round 2's first setting: one wrong plane in
- *                            about 25000 calls), 0 = at once (about one call in 100: the A/B setting of profiles/r2_race_k1_pair.md),
- *                            up to 4; profiles/r5_soak.md has the measured rates and the cost (about 1 % of the config-5 step);
+ *                            last UMMA: 2 (default), 1 (round 2's first setting: alone, one wrong plane in about 25000 calls),
+ *                            0 = at once (alone, about one call in 100: the A/B setting of profiles/r2_race_k1_pair.md), up to 4.
+ *                            The margin alone is not robust (two K-steps failed once in 150000 calls in one build): it is
+ *                            combined with PSF_TUNE_K1P_WAITFIRST; profiles/r5_soak.md has the measured rates and costs;
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
  *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;

@@ -599,8 +599,10 @@ __device__ __forceinline__ void k1p_feed(uint8_t *smem, K1PShared &S, uint32_t t
               //    arrive is triggered when all prior asynchronous tcgen05 operations of the issuing thread have completed)
               //    -> producer: mbarrier.try_wait -> st.shared into the slot.  Every edge is in the model - and this is where the
               //    measured failures sit (profiles/r5_soak.md: the cluster-scope pair above still fails without the deferral, so
-              //    the read-after-write side is not it): hence the margin below, P.defer K-steps (default 2: 0 wrong stacks in
-              //    200000 calls; 1: one in 25000; 0: one in 100).
+              //    the read-after-write side is not it): hence the margin below, P.defer K-steps (default 2; alone: 1 -> one
+              //    wrong stack in 25000 calls, 0 -> one in 100, and 2 failed once in 150000 in one build), and the producers'
+              //    wait-first order (P.waitfirst in k1p_produce), which puts their computation between the observed release
+              //    and the first store.
               // Deferred release (profiles/r1j_race_k1_pair.md): the commit tracks the UMMAs of the issuing (leader) CTA; in
               // the peer, whose tensor core can trail by a little, producers with their rows ready in registers
               // overwrote the operand tile while it was still being read.  The previous stage's buffer is therefore
