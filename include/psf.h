@@ -198,7 +198,9 @@ int psf_grad_terms(const psf_plan *plan);
  *                            combined with PSF_TUNE_K1P_WAITFIRST; profiles/r5_soak.md has the measured rates and costs;
  *   PSF_TUNE_TC_FUSED      : 1 (default) = where both stages run on CTA pairs and take about equal time, they are enqueued as
  *                            ONE kernel (k12_fused) whose stage-2 clusters consume the scratch right behind the stage-1
- *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth;
+ *                            clusters, so that it stays in L2; 0 = always two kernels; 2..8 = fused with that ring depth.
+ *                            Known issue (profiles/r5_soak.md): in soaks the fused launch produced one wrong plane in about one of
+ *                            4e5 config-5 calls; the two-kernel path (0) was clean in 1.3e6;
  *   PSF_TUNE_SMLM          : 1 (default) = small grids in per-plane mode (emitter batches) run the emitter-batch kernels where the plan
  *                            qualifies: k_smlm_tc (tcgen05; output half-size <= 16, precision AUTO or 3XF16), else k_smlm (fp32 FMA);
  *                            2 = k_smlm, never the tensor-core variant; 0 = always k_small;
